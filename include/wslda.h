@@ -1,0 +1,135 @@
+/*
+ * wslda.h -- C-ABI boundary of the single-B200 TDSLDA/BdG time-step library (libwslda).
+ *
+ * One time step of the time-dependent SLDA/BdG equations (arXiv 2602.08982, W-SLDA Toolkit) for a batch of
+ * complex128 quasiparticle spinors psi_n = (u_n, v_n) on a periodic lattice:
+ *   H psi (spectral kinetic/gradient terms, Eqs. 5, 14, 15, 25-26, 40)  ->  densities (Eqs. 7, 8, 29, 30)
+ *   ->  potentials (Eqs. 9-12, 19-22)  ->  Adams-Bashforth-Moulton update (Eqs. 44-50, Alg. 2, Eqs. 52-54).
+ * Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md.
+ *
+ * Conventions (all entry points):
+ *  - every array argument named *_dev or documented "device" is a DEVICE pointer owned by the caller
+ *    (allocated e.g. with torch); host pointers are documented "host".  The library never frees caller
+ *    memory and allocates no device memory of its own: it lives in the workspace given to wslda_ctx_create.
+ *  - complex128 is interleaved (re, im).  Spinor buffers are [n][c in {u,v}][ix][iy][iz] contiguous with iz
+ *    fastest (loop order PAPER.md:1527-1544), 16-byte aligned; only the held axes (3D: x,y,z; quasi-2D: x,y;
+ *    quasi-1D: x) are stored.  Fields are [ix][iy][iz] over the held axes, real (double) or complex.
+ *  - every call is asynchronous on the given CUDA stream (a cudaStream_t passed as void*; NULL = default
+ *    stream) and returns a status; argument errors return WSLDA_EINVAL before any launch; lattice sizes
+ *    that are not powers of two >= 2 return WSLDA_EUNSUPPORTED (the paper needs even sizes);
+ *    a CUDA error is reported as WSLDA_ECUDA.  wslda_last_error() gives a text for the last failure.
+ *  - there is no CPU fallback: without a CUDA device every compute call fails with WSLDA_ECUDA.
+ */
+#ifndef WSLDA_H
+#define WSLDA_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wslda_ctx wslda_ctx;   /* opaque; created/destroyed by the library (host object) */
+
+typedef enum { WSLDA_OK = 0, WSLDA_EINVAL = 1, WSLDA_EUNSUPPORTED = 2, WSLDA_ENOMEM = 3, WSLDA_ESTATE = 4,
+               WSLDA_ECUDA = 5 } wslda_status;
+/* symmetry mode = number of held axes: quasi-1D (Eqs. 30), quasi-2D (Eqs. 29), full 3D */
+typedef enum { WSLDA_MODE_1D = 1, WSLDA_MODE_2D = 2, WSLDA_MODE_3D = 3 } wslda_mode;
+/* functional: fixed potentials, BdG (Eq. 11), ASLDA (Eq. 12; SLDA = p -> 0) */
+typedef enum { WSLDA_FUNC_FIXED = 0, WSLDA_FUNC_BDG = 1, WSLDA_FUNC_ASLDA = 2 } wslda_func_id;
+/* kinetic operator: Eq. 14 (alpha = 1), Eq. 40 symmetrised form, successive first derivatives */
+typedef enum { WSLDA_KIN_LAPLACE = 0, WSLDA_KIN_SYM40 = 1, WSLDA_KIN_DIVGRAD = 2 } wslda_kin;
+
+typedef struct {
+  int func_id;               /* wslda_func_id                                                               */
+  int force_a1;              /* alpha_sigma = 1 everywhere, also inside B(p)             */
+  int spin_symmetric;        /* fold densities per Eq. 8                                 */
+  int kin_form;              /* wslda_kin                                                                   */
+  int ab_order, am_order;    /* (3,4) (4,4) (4,5) (5,5): Eqs. 46-50                        */
+  int subtract_mean_energy;  /* Eq. 44: evolve with H - <H>_n                                  */
+  int normalize;             /* Alg. 2 steps 2 and 8 PAPER.md:646, 652                                      */
+  double four_pi_as;         /* BdG coupling C/rho^(1/3) = 4 pi a_s                          */
+  double C;                  /* Eq. 12c: -11.11                                                             */
+  double E_cut;              /* Eq. 22: default pi^2 / (2 dx^2)                                             */
+  int lambda_mode;           /* 0: Lambda_c (Eq. 20) recomputed at every update; 1: frozen after the first  */
+  double rho_floor;          /* guard for rho^(1/3) and p at rho -> 0                                       */
+} wslda_functional;
+
+/* field ids for wslda_get_field / wslda_set_field.  Densities are returned folded per Eq. 8 when
+ * spin_symmetric is set.  NU and DELTA are complex (M complex128), every other field is M doubles. */
+enum { WSLDA_F_RHO_A = 0, WSLDA_F_RHO_B = 1, WSLDA_F_TAU_A = 2, WSLDA_F_TAU_B = 3, WSLDA_F_NU = 4,
+       WSLDA_F_JA_X = 5, WSLDA_F_JA_Y = 6, WSLDA_F_JA_Z = 7, WSLDA_F_JB_X = 8, WSLDA_F_JB_Y = 9, WSLDA_F_JB_Z = 10,
+       WSLDA_F_ALPHA_A = 16, WSLDA_F_ALPHA_B = 17, WSLDA_F_U_A = 18, WSLDA_F_U_B = 19, WSLDA_F_DELTA = 20,
+       WSLDA_F_LAP_ALPHA_A = 21, WSLDA_F_LAP_ALPHA_B = 22, WSLDA_F_LAMBDA_C = 23, WSLDA_F_G_EFF = 24,
+       WSLDA_F_V_A = 25, WSLDA_F_V_B = 26 };
+
+/* which_mask bits of wslda_densities (Eqs. 7a-g) */
+enum { WSLDA_D_RHO = 1u, WSLDA_D_NU = 2u, WSLDA_D_TAU = 4u, WSLDA_D_J = 8u, WSLDA_D_ALL = 15u };
+
+/* Bytes of device workspace wslda_ctx_create needs for this problem (pure host computation; 0 on bad
+ * arguments).  dims/dx: host arrays of 3 (Nx,Ny,Nz / dx,dy,dz); non-held axes only enter L_perp (Eqs. 29a, 30a). */
+size_t wslda_workspace_bytes(const int dims[3], wslda_mode mode, int64_t n_wf, const wslda_functional* f);
+
+/* Create a context.  dims, dx, f: host.  workspace_dev: device memory of at least wslda_workspace_bytes()
+ * bytes, 256-byte aligned, owned by the caller and kept alive until wslda_ctx_destroy.  Builds the k-tables
+ * (Eq. 25) and FFT twiddles in the workspace (synchronous copies).  Defaults: weights w_a = 0,
+ * w_b = 1; one transverse mode k_perp = 0 with multiplicity 1; mu = 0; alpha = 1; all other fields 0. */
+wslda_status wslda_ctx_create(wslda_ctx** ctx, const int dims[3], const double dx[3], wslda_mode mode,
+                              int64_t n_wf, const wslda_functional* f, void* workspace_dev, size_t workspace_bytes);
+wslda_status wslda_ctx_destroy(wslda_ctx* ctx);
+
+/* Transverse modes (quasi-1D/2D; substitutions PAPER.md:413-419, 444-448).  Host arrays: kperp[2*m+{0,1}],
+ * multiplicity mult[m], and mode m owns spinors [first[m], first[m+1]); first[0] = 0, first[n_modes] = n_wf. */
+wslda_status wslda_set_modes(wslda_ctx*, int n_modes, const double* kperp, const double* mult, const int64_t* first);
+/* Frozen occupation weights f_beta(E_n), f_beta(-E_n); device arrays of n_wf doubles (copied). */
+wslda_status wslda_set_weights(wslda_ctx*, const double* w_a_dev, const double* w_b_dev);
+wslda_status wslda_set_mu(wslda_ctx*, double mu_a, double mu_b);
+/* External fields (device, nullable = zero): V_ext_sigma real [M], Delta_ext complex [M]. Copied. */
+wslda_status wslda_set_external(wslda_ctx*, const double* vext_a_dev, const double* vext_b_dev, const void* delta_ext_dev);
+/* Fixed potentials (FUNC_FIXED and tests): device arrays alpha_sigma, U_sigma real [M], Delta complex [M];
+ * copied; Laplacian of alpha_sigma (Eq. 40) is recomputed spectrally. */
+wslda_status wslda_set_potentials(wslda_ctx*, const double* alpha_a_dev, const double* alpha_b_dev,
+                                  const double* U_a_dev, const double* U_b_dev, const void* delta_dev, void* cuda_stream);
+/* Copy one field to / from caller device memory (see the field id list).  set: raw densities RHO/TAU/NU
+ * and LAMBDA_C only (LAMBDA_C also marks the frozen field valid). */
+wslda_status wslda_get_field(wslda_ctx*, int field_id, void* dst_dev, void* cuda_stream);
+wslda_status wslda_set_field(wslda_ctx*, int field_id, const void* src_dev, void* cuda_stream);
+
+/* hpsi = H psi for spinors [n_first, n_first+n_count) of the whole-batch buffers psi, hpsi (device,
+ * [n_wf][2][M] complex128, hpsi != psi); eps_dev (nullable, device, n_wf doubles) receives
+ * eps_n = Re dV sum_r psi_n^+ (H psi_n) at index n.  Eqs. 5, 15 PAPER.md:154, 289; Eq. 44b PAPER.md:592. */
+wslda_status wslda_apply_h(wslda_ctx*, const void* psi_dev, void* hpsi_dev, double* eps_dev,
+                           int64_t n_first, int64_t n_count, void* cuda_stream);
+/* Accumulate the densities of spinors [n_first, n_first+n_count) (Eqs. 7a-g, 29b-e, 30b-e) into the
+ * context's raw sums; accumulate = 0 overwrites the selected fields, 1 adds (batch streaming). */
+wslda_status wslda_densities(wslda_ctx*, const void* psi_dev, int64_t n_first, int64_t n_count,
+                             unsigned which_mask, int accumulate, void* cuda_stream);
+/* Rebuild alpha_sigma, V_sigma, U_sigma, Lambda_c, g_eff, Delta and lap(alpha_sigma) pointwise from the
+ * current densities (Eqs. 9-12, 19-22 PAPER.md:195-255, 311-337).  FUNC_FIXED: no-op. */
+wslda_status wslda_update_potentials(wslda_ctx*, void* cuda_stream);
+
+/* History length m = max(ab_order, am_order-1). */
+int wslda_history_length(const wslda_ctx*);
+/* Fill the ABM history for phi (device, [n_wf][2][M], in/out).  f_hist: HOST array of m DEVICE buffers of the
+ * same shape, f_hist[0] = newest.  selfstart = 0: zero history (stationary start), potentials
+ * rebuilt from phi; else f(phi_0) and m-1 Taylor/midpoint steps (Eqs. 52-54), which advance
+ * phi by (m-1) dt.  The roles of f_hist[] are permuted and reported through the same host array. */
+wslda_status wslda_abm_init(wslda_ctx*, void* phi_dev, void** f_hist, double dt, int selfstart, void* cuda_stream);
+/* One predictor-corrector step following Alg. 2: phi (device) is advanced in place, the
+ * oldest history buffer receives f(phi_new) and becomes f_hist[0] (host array permuted in place).  With a
+ * self-consistent functional the densities the functional consumes (rho, nu; tau when alpha depends on p)
+ * are rebuilt at both stages; j and unused tau are refreshed only by wslda_densities. */
+wslda_status wslda_abm_step(wslda_ctx*, void* phi_dev, void** f_hist, double dt, void* cuda_stream);
+/* The same step driven from HOST buffers (end-to-end form): copies phi_host and the m host history buffers to
+ * the given device buffers, runs wslda_abm_step, copies phi and the new f_hist[0] back and synchronises the
+ * stream.  phi_host / f_hist_host[i]: host (pinned for full speed); f_hist_host is permuted like f_hist_dev. */
+wslda_status wslda_abm_step_host(wslda_ctx*, void* phi_host, void** f_hist_host, void* phi_dev, void** f_hist_dev,
+                                 double dt, void* cuda_stream);
+/* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
+int64_t wslda_launch_count(const wslda_ctx*);
+const char* wslda_last_error(const wslda_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,218 @@
+// ctx.cuh -- context object, workspace plan, creation and the setters (host side of libwslda).
+#pragma once
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <vector>
+#include "density.cuh"
+#include "fft_large.cuh"
+#include "kernels.cuh"
+
+struct Plan {
+  int nd, N[3], lg[3];
+  int64_t M, n_wf, chunk_n;
+  int nblk, pt_threads;         // pointwise kernels: blocks per spinor, threads per block
+  bool onchip; int G;           // whole-lattice-in-shared-memory regime, components per CTA
+  int PX, lgT;                  // large regime: x-planes per CTA, log2 of the x-line tile width
+  int dG;                       // max density groups per chunk
+  int nscr;
+  size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
+};
+
+static int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// status: 0 ok, else a wslda_status
+static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_functional* f, Plan& P) {
+  if (!dims || !f || mode < 1 || mode > 3 || n_wf < 1) return WSLDA_EINVAL;
+  for (int d = 0; d < 3; ++d) if (dims[d] < 1) return WSLDA_EINVAL;
+  bool okpair = (f->ab_order == 3 && f->am_order == 4) || (f->ab_order == 4 && f->am_order == 4) ||
+                (f->ab_order == 4 && f->am_order == 5) || (f->ab_order == 5 && f->am_order == 5);
+  if (!okpair || f->kin_form < 0 || f->kin_form > 2 || f->func_id < 0 || f->func_id > 2) return WSLDA_EINVAL;
+  P.nd = mode; P.M = 1;
+  for (int d = 0; d < 3; ++d) {
+    P.N[d] = d < mode ? dims[d] : 1;
+    if (d < mode && (dims[d] < 2 || (dims[d] & (dims[d] - 1)))) return WSLDA_EUNSUPPORTED;
+    P.lg[d] = ilog2(P.N[d]);
+    P.M *= P.N[d];
+  }
+  P.n_wf = n_wf;
+  const int64_t M = P.M;
+  double chunk_mb = 16.0;
+  if (const char* e = getenv("WSLDA_CHUNK_MB")) { double v = atof(e); if (v > 0) chunk_mb = v; }
+  int64_t cn = (int64_t)(chunk_mb * 1048576.0 / (32.0 * (double)M));
+  if (cn < 1) cn = 1;
+  if (cn > n_wf) cn = n_wf;
+  P.chunk_n = cn;
+  P.pt_threads = M < WS_PT_THREADS ? (int)((M + 31) / 32 * 32) : WS_PT_THREADS;
+  P.nblk = (int)((M + P.pt_threads - 1) / P.pt_threads);
+  P.onchip = M <= 4096;
+  P.G = 1; P.PX = 1; P.lgT = 0;
+  if (P.onchip) {
+    P.G = (int)(1024 / M); if (P.G < 1) P.G = 1;
+  } else {
+    if (mode < 2) return WSLDA_EUNSUPPORTED;            // one axis longer than 4096 points
+    const int64_t R = M / P.N[0];
+    if (R > 8192 || P.N[0] > 1024) return WSLDA_EUNSUPPORTED;
+    int64_t px = 4096 / R; if (px < 1) px = 1; if (px > P.N[0]) px = P.N[0];
+    P.PX = (int)px;
+    int64_t T = 2048 / P.N[0]; if (T < 2) T = 2; if (T > R) T = R;
+    P.lgT = ilog2((int)T);
+  }
+  int64_t dg = (1184 + P.nblk - 1) / P.nblk; if (dg < 1) dg = 1; if (dg > cn) dg = cn;
+  P.dG = (int)dg;
+  P.nscr = 7;
+  size_t o = 0;
+  P.off_tables = o; for (int d = 0; d < 3; ++d) o += align_up((size_t)P.N[d] * 32);       // tw (16) + kk (8) + ko (8)
+  P.off_perwf = o; o += 6 * align_up((size_t)n_wf * 8);
+  P.off_fields = o; o += align_up((size_t)DP_COUNT * M * 8) + 12 * align_up((size_t)M * 8) + 2 * align_up((size_t)M * 16);
+  P.off_part = o; o += 2 * align_up((size_t)cn * P.nblk * 8);
+  P.off_dpart = o; o += align_up((size_t)P.dG * DP_COUNT * M * 8);
+  P.scr_bytes = align_up((size_t)cn * 2 * M * 16);
+  P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
+  P.total = o;
+  return 0;
+}
+
+struct wslda_ctx {
+  Plan P;
+  Lat L;
+  double dx[3], dV, Lperp;
+  wslda_functional f;
+  int m;
+  double mu_a, mu_b;
+  int lambda_valid;
+  double *kperp2, *cpref, *w_a, *w_b, *scale, *eps;
+  double* raw;
+  double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
+  cplx *delta, *dext;
+  double *part_n, *part_e, *dpart;
+  cplx* scr[WS_MAX_SCR];
+  int64_t launches;
+  char err[256];
+};
+
+static char g_err[256] = "";
+static wslda_status fail(wslda_ctx* c, wslda_status s, const char* msg) {
+  snprintf(c ? c->err : g_err, 256, "%s", msg);
+  return s;
+}
+static wslda_status cuda_check(wslda_ctx* c, const char* where) {
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) return WSLDA_OK;
+  snprintf(c ? c->err : g_err, 256, "CUDA error at %s: %s", where, cudaGetErrorString(e));
+  return WSLDA_ECUDA;
+}
+#define LAUNCH(c, kern, grid, block, smem, st, ...)            \
+  do { kern<<<grid, block, smem, st>>>(__VA_ARGS__); (c)->launches++; } while (0)
+
+// stored position p of the in-place DIF transform (radix 4 from L = n down, then radix 2) <-> frequency index
+static void scrambled_freq(int n, std::vector<int>& fr) {
+  fr.resize(n);
+  for (int p = 0; p < n; ++p) {
+    int L = n, rem = p, k = 0, mult = 1;
+    while (L > 1) { int r = (L >= 4) ? 4 : 2, sub = L / r, m = rem / sub; rem %= sub; k += m * mult; mult *= r; L = sub; }
+    fr[p] = k;
+  }
+}
+
+extern "C" size_t wslda_workspace_bytes(const int dims[3], wslda_mode mode, int64_t n_wf, const wslda_functional* f) {
+  Plan P;
+  if (make_plan(dims, (int)mode, n_wf, f, P)) return 0;
+  return P.total;
+}
+
+extern "C" const char* wslda_last_error(const wslda_ctx* c) { return c ? c->err : g_err; }
+extern "C" int64_t wslda_launch_count(const wslda_ctx* c) { return c ? c->launches : 0; }
+extern "C" int wslda_history_length(const wslda_ctx* c) { return c ? c->m : 0; }
+
+extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], const double dx[3], wslda_mode mode,
+                                         int64_t n_wf, const wslda_functional* f, void* ws, size_t ws_bytes) {
+  if (!out || !dx) return fail(nullptr, WSLDA_EINVAL, "null argument");
+  Plan P;
+  int rc = make_plan(dims, (int)mode, n_wf, f, P);
+  if (rc == WSLDA_EUNSUPPORTED) return fail(nullptr, WSLDA_EUNSUPPORTED, "held lattice sizes must be powers of two >= 2 (and fit the supported regimes)");
+  if (rc) return fail(nullptr, WSLDA_EINVAL, "bad dims / mode / n_wf / functional");
+  for (int d = 0; d < 3; ++d) if (!(dx[d] > 0)) return fail(nullptr, WSLDA_EINVAL, "dx must be positive");
+  if (!ws || ((uintptr_t)ws & 255)) return fail(nullptr, WSLDA_EINVAL, "workspace must be a 256-byte aligned device pointer");
+  if (ws_bytes < P.total) return fail(nullptr, WSLDA_ENOMEM, "workspace smaller than wslda_workspace_bytes()");
+  wslda_ctx* c = (wslda_ctx*)calloc(1, sizeof(wslda_ctx));
+  if (!c) return fail(nullptr, WSLDA_ENOMEM, "host allocation failed");
+  c->P = P; c->f = *f;
+  c->m = f->ab_order > f->am_order - 1 ? f->ab_order : f->am_order - 1;
+  c->dV = 1.0; c->Lperp = 1.0;
+  for (int d = 0; d < 3; ++d) {
+    c->dx[d] = dx[d];
+    if (d < P.nd) c->dV *= dx[d]; else c->Lperp *= dims[d] * dx[d];
+  }
+  char* base = (char*)ws;
+  const int64_t M = P.M;
+  Lat& L = c->L;
+  L.nd = P.nd; L.M = M; L.invM = 1.0 / (double)M;
+  const double PI = 3.14159265358979323846264338327950288;
+  size_t o = P.off_tables;
+  for (int d = 0; d < 3; ++d) {
+    const int n = P.N[d];
+    L.N[d] = n; L.lg[d] = P.lg[d];
+    std::vector<double> tw(2 * n), kk(n), ko(n);
+    std::vector<int> fr;
+    scrambled_freq(n, fr);
+    const double len = n * dx[d];
+    for (int j = 0; j < n; ++j) {
+      tw[2 * j] = cos(2.0 * PI * j / n); tw[2 * j + 1] = -sin(2.0 * PI * j / n);
+      const int l = fr[j];
+      double k = (l < n / 2) ? 2.0 * PI * l / len : 2.0 * PI * (l - n) / len;      // Eq. 25
+      if (n == 1) k = 0.0;
+      kk[j] = k; ko[j] = (n > 1 && l == n / 2) ? 0.0 : k;
+    }
+    cplx* dtw = (cplx*)(base + o); double* dkk = (double*)(base + o + (size_t)n * 16); double* dko = dkk + n;
+    cudaMemcpy(dtw, tw.data(), (size_t)n * 16, cudaMemcpyHostToDevice);
+    cudaMemcpy(dkk, kk.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(dko, ko.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
+    L.tw[d] = dtw; L.kk[d] = dkk; L.ko[d] = dko;
+    o += align_up((size_t)n * 32);
+  }
+  o = P.off_perwf;
+  double** pw[6] = {&c->kperp2, &c->cpref, &c->w_a, &c->w_b, &c->scale, &c->eps};
+  for (int q = 0; q < 6; ++q) { *pw[q] = (double*)(base + o); o += align_up((size_t)n_wf * 8); }
+  o = P.off_fields;
+  c->raw = (double*)(base + o); o += align_up((size_t)DP_COUNT * M * 8);
+  double** pf[12] = {&c->alpha_a, &c->alpha_b, &c->V_a, &c->V_b, &c->U_a, &c->U_b, &c->lap_a, &c->lap_b,
+                     &c->lambda, &c->geff, &c->vext_a, &c->vext_b};
+  for (int q = 0; q < 12; ++q) { *pf[q] = (double*)(base + o); o += align_up((size_t)M * 8); }
+  c->delta = (cplx*)(base + o); o += align_up((size_t)M * 16);
+  c->dext = (cplx*)(base + o); o += align_up((size_t)M * 16);
+  c->part_n = (double*)(base + P.off_part);
+  c->part_e = (double*)(base + P.off_part + align_up((size_t)P.chunk_n * P.nblk * 8));
+  c->dpart = (double*)(base + P.off_dpart);
+  for (int q = 0; q < P.nscr; ++q) c->scr[q] = (cplx*)(base + P.off_scr + (size_t)q * P.scr_bytes);
+  // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
+  cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);
+  const int T = 256;
+  k_fill<<<(unsigned)((M + T - 1) / T), T>>>(c->alpha_a, M, 1.0);
+  k_fill<<<(unsigned)((M + T - 1) / T), T>>>(c->alpha_b, M, 1.0);
+  k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->w_b, n_wf, 1.0);
+  k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->cpref, n_wf, 1.0 / c->Lperp);
+  k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->scale, n_wf, 1.0);
+  c->launches += 5;
+  const int big = 227 * 1024;
+  cudaFuncSetAttribute(k_deriv_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+  cudaFuncSetAttribute(k_planes_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+  cudaFuncSetAttribute(k_planes_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+  cudaFuncSetAttribute(k_xlines, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) {
+    snprintf(g_err, 256, "CUDA error in wslda_ctx_create: %s", cudaGetErrorString(e));
+    free(c);
+    return WSLDA_ECUDA;
+  }
+  *out = c;
+  return WSLDA_OK;
+}
+
+extern "C" wslda_status wslda_ctx_destroy(wslda_ctx* c) {
+  if (!c) return WSLDA_EINVAL;
+  free(c);
+  return WSLDA_OK;
+}

@@ -1,0 +1,245 @@
+// ops.cuh -- setters, the derivative engine dispatch, and the three single-call entry points
+// wslda_apply_h / wslda_densities / wslda_update_potentials (general chunked path).
+#pragma once
+#include "ctx.cuh"
+
+static inline cudaStream_t S(void* s) { return (cudaStream_t)s; }
+static inline unsigned nb(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
+
+extern "C" wslda_status wslda_set_modes(wslda_ctx* c, int n_modes, const double* kperp, const double* mult, const int64_t* first) {
+  if (!c) return WSLDA_EINVAL;
+  if (n_modes < 1 || !kperp || !mult || !first || first[0] != 0 || first[n_modes] != c->P.n_wf)
+    return fail(c, WSLDA_EINVAL, "set_modes: first[] must run from 0 to n_wf");
+  const int64_t n_wf = c->P.n_wf;
+  std::vector<double> k2(n_wf), cp(n_wf);
+  for (int m = 0; m < n_modes; ++m) {
+    if (first[m + 1] < first[m]) return fail(c, WSLDA_EINVAL, "set_modes: first[] must be non-decreasing");
+    for (int64_t n = first[m]; n < first[m + 1]; ++n) {
+      k2[n] = kperp[2 * m] * kperp[2 * m] + kperp[2 * m + 1] * kperp[2 * m + 1];
+      cp[n] = mult[m] / c->Lperp;
+    }
+  }
+  cudaMemcpy(c->kperp2, k2.data(), n_wf * 8, cudaMemcpyHostToDevice);
+  cudaMemcpy(c->cpref, cp.data(), n_wf * 8, cudaMemcpyHostToDevice);
+  return cuda_check(c, "set_modes");
+}
+
+extern "C" wslda_status wslda_set_weights(wslda_ctx* c, const double* w_a, const double* w_b) {
+  if (!c || !w_a || !w_b) return fail(c, WSLDA_EINVAL, "set_weights: null argument");
+  cudaMemcpy(c->w_a, w_a, c->P.n_wf * 8, cudaMemcpyDeviceToDevice);
+  cudaMemcpy(c->w_b, w_b, c->P.n_wf * 8, cudaMemcpyDeviceToDevice);
+  return cuda_check(c, "set_weights");
+}
+
+extern "C" wslda_status wslda_set_mu(wslda_ctx* c, double mu_a, double mu_b) {
+  if (!c) return WSLDA_EINVAL;
+  c->mu_a = mu_a; c->mu_b = mu_b;
+  return WSLDA_OK;
+}
+
+extern "C" wslda_status wslda_set_external(wslda_ctx* c, const double* va, const double* vb, const void* de) {
+  if (!c) return WSLDA_EINVAL;
+  const int64_t M = c->P.M;
+  if (va) cudaMemcpy(c->vext_a, va, M * 8, cudaMemcpyDeviceToDevice); else cudaMemset(c->vext_a, 0, M * 8);
+  if (vb) cudaMemcpy(c->vext_b, vb, M * 8, cudaMemcpyDeviceToDevice); else cudaMemset(c->vext_b, 0, M * 8);
+  if (de) cudaMemcpy(c->dext, de, M * 16, cudaMemcpyDeviceToDevice); else cudaMemset(c->dext, 0, M * 16);
+  return cuda_check(c, "set_external");
+}
+
+// ---- derivative engine: lap / grad of a batch of components (DerivArgs) -------------------------------------
+static void deriv(wslda_ctx* c, const DerivArgs& a, cudaStream_t st) {
+  const Plan& P = c->P;
+  const int64_t M = P.M;
+  if (P.onchip) {
+    const size_t smem = (size_t)2 * P.G * M * 16;
+    LAUNCH(c, k_deriv_onchip, nb(a.ncomp, P.G), 256, smem, st, c->L, a, P.G);
+    return;
+  }
+  const int64_t R = M / P.N[0];
+  cplx* spec = c->scr[3];
+  LAUNCH(c, k_planes_fwd, dim3(P.N[0] / P.PX, a.ncomp), 256, (size_t)P.PX * R * 16, st, c->L, a, spec, P.PX);
+  LAUNCH(c, k_xlines, dim3((unsigned)(R >> P.lgT), a.ncomp), 256, (size_t)2 * P.N[0] * 16 << P.lgT, st, c->L, spec, a, P.lgT);
+  OutList ol; int no = 0;
+  for (int o = 0; o < 4; ++o) if (a.out[o]) ol.p[no++] = a.out[o];
+  for (int o = no; o < 4; ++o) ol.p[o] = nullptr;
+  LAUNCH(c, k_planes_inv, dim3(P.N[0] / P.PX, a.ncomp, no), 256, (size_t)P.PX * R * 16, st, c->L, ol, P.PX);
+}
+
+// lap(alpha_sigma) of the current alpha fields (Eq. 40 needs it once per potential update)
+static void update_lap_alpha(wslda_ctx* c, cudaStream_t st) {
+  const int64_t M = c->P.M;
+  cplx* in = c->scr[5];
+  cplx* out = c->scr[6];
+  if (c->P.chunk_n < 1) return;
+  LAUNCH(c, k_real_to_cplx, nb(M, 256), 256, 0, st, c->alpha_a, c->alpha_b, in, M);
+  DerivArgs a; memset(&a, 0, sizeof a);
+  a.src = in; a.src_comp0 = 0; a.ncomp = 2; a.out[0] = out;
+  deriv(c, a, st);
+  LAUNCH(c, k_cplx_real_part, nb(M, 256), 256, 0, st, out, c->lap_a, c->lap_b, M);
+}
+
+extern "C" wslda_status wslda_set_potentials(wslda_ctx* c, const double* aa, const double* ab, const double* Ua,
+                                             const double* Ub, const void* delta, void* stream) {
+  if (!c || !aa || !ab || !Ua || !Ub || !delta) return fail(c, WSLDA_EINVAL, "set_potentials: null argument");
+  const int64_t M = c->P.M;
+  cudaStream_t st = S(stream);
+  cudaMemcpyAsync(c->alpha_a, aa, M * 8, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->alpha_b, ab, M * 8, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->U_a, Ua, M * 8, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->U_b, Ub, M * 8, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->delta, delta, M * 16, cudaMemcpyDeviceToDevice, st);
+  update_lap_alpha(c, st);
+  return cuda_check(c, "set_potentials");
+}
+
+extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* stream) {
+  if (!c || !dst) return fail(c, WSLDA_EINVAL, "get_field: null argument");
+  const int64_t M = c->P.M;
+  cudaStream_t st = S(stream);
+  const void* src = nullptr; size_t bytes = M * 8;
+  switch (id) {
+    case WSLDA_F_ALPHA_A: src = c->alpha_a; break; case WSLDA_F_ALPHA_B: src = c->alpha_b; break;
+    case WSLDA_F_U_A: src = c->U_a; break; case WSLDA_F_U_B: src = c->U_b; break;
+    case WSLDA_F_LAP_ALPHA_A: src = c->lap_a; break; case WSLDA_F_LAP_ALPHA_B: src = c->lap_b; break;
+    case WSLDA_F_LAMBDA_C: src = c->lambda; break; case WSLDA_F_G_EFF: src = c->geff; break;
+    case WSLDA_F_V_A: src = c->V_a; break; case WSLDA_F_V_B: src = c->V_b; break;
+    case WSLDA_F_DELTA: src = c->delta; bytes = M * 16; break;
+    default: break;
+  }
+  if (src) { cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st); return cuda_check(c, "get_field"); }
+  if (id < 0 || id > WSLDA_F_JB_Z) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
+  LAUNCH(c, k_get_density, nb(M, 256), 256, 0, st, c->raw, M, c->f.spin_symmetric, id, (double*)dst);
+  return cuda_check(c, "get_field");
+}
+
+extern "C" wslda_status wslda_set_field(wslda_ctx* c, int id, const void* src, void* stream) {
+  if (!c || !src) return fail(c, WSLDA_EINVAL, "set_field: null argument");
+  const int64_t M = c->P.M;
+  cudaStream_t st = S(stream);
+  double* dst = nullptr;
+  switch (id) {
+    case WSLDA_F_RHO_A: dst = c->raw + DP_RHO_A * M; break; case WSLDA_F_RHO_B: dst = c->raw + DP_RHO_B * M; break;
+    case WSLDA_F_TAU_A: dst = c->raw + DP_TAU_A * M; break; case WSLDA_F_TAU_B: dst = c->raw + DP_TAU_B * M; break;
+    case WSLDA_F_LAMBDA_C: dst = c->lambda; c->lambda_valid = 1; break;
+    case WSLDA_F_NU:   // interleaved complex -> two planes
+      cudaMemcpy2DAsync(c->raw + DP_NU_RE * M, 8, src, 16, 8, M, cudaMemcpyDeviceToDevice, st);
+      cudaMemcpy2DAsync(c->raw + DP_NU_IM * M, 8, (const char*)src + 8, 16, 8, M, cudaMemcpyDeviceToDevice, st);
+      return cuda_check(c, "set_field");
+    default: return fail(c, WSLDA_EINVAL, "set_field: only raw rho/tau/nu and lambda_c can be set");
+  }
+  cudaMemcpyAsync(dst, src, M * 8, cudaMemcpyDeviceToDevice, st);
+  return cuda_check(c, "set_field");
+}
+
+static Fields fields_of(const wslda_ctx* c) {
+  Fields F;
+  F.alpha_a = c->alpha_a; F.alpha_b = c->alpha_b; F.lap_a = c->lap_a; F.lap_b = c->lap_b; F.U_a = c->U_a; F.U_b = c->U_b;
+  F.delta = c->delta; F.dext = c->dext; F.mu_a = c->mu_a; F.mu_b = c->mu_b;
+  return F;
+}
+
+// H psi for the cnt spinors of a chunk: psi_chunk / scale_chunk (nullable) / out are already offset to the chunk's
+// first spinor, n0 is its global index (per-spinor tables).  out is laid out [n - n0][2][M]; eps partials go to
+// part_e.  Uses scr[0..3].
+static void h_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_chunk, int64_t n0, int64_t cnt, cplx* out,
+                    bool want_eps, cudaStream_t st) {
+  const Plan& P = c->P;
+  const int64_t M = P.M;
+  const int kin = c->f.kin_form;
+  DerivArgs a; memset(&a, 0, sizeof a);
+  a.src = psi_chunk; a.src_comp0 = 0; a.ncomp = (int)(2 * cnt); a.scale = scale_chunk;
+  if (kin == WSLDA_KIN_DIVGRAD) {
+    for (int d = 0; d < P.nd; ++d) a.out[1 + d] = c->scr[d];
+    deriv(c, a, st);
+    for (int d = 0; d < P.nd; ++d) {                    // s_d <- d_d (alpha s_d), in place
+      DerivArgs b; memset(&b, 0, sizeof b);
+      b.src = c->scr[d]; b.src_comp0 = 0; b.ncomp = a.ncomp; b.premul[0] = c->alpha_a; b.premul[1] = c->alpha_b;
+      b.out[1 + d] = c->scr[d];
+      deriv(c, b, st);
+    }
+  } else {
+    a.out[0] = c->scr[0];
+    deriv(c, a, st);
+    if (kin == WSLDA_KIN_SYM40) {
+      DerivArgs b = a;
+      b.premul[0] = c->alpha_a; b.premul[1] = c->alpha_b; b.out[0] = c->scr[1];
+      deriv(c, b, st);
+    }
+  }
+  LAUNCH(c, k_hmix, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, psi_chunk, scale_chunk, c->kperp2 + n0, kin, P.nd,
+         c->scr[0], c->scr[1], c->scr[2], fields_of(c), M, out, want_eps ? c->part_e : nullptr, P.nblk);
+}
+
+extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi_, double* eps_dev, int64_t n_first,
+                                      int64_t n_count, void* stream) {
+  if (!c || !psi_ || !hpsi_ || psi_ == hpsi_) return fail(c, WSLDA_EINVAL, "apply_h: null or aliased buffers");
+  if (n_first < 0 || n_count < 0 || n_first + n_count > c->P.n_wf) return fail(c, WSLDA_EINVAL, "apply_h: spinor range out of bounds");
+  const cplx* psi = (const cplx*)psi_; cplx* hpsi = (cplx*)hpsi_;
+  const int64_t M = c->P.M;
+  cudaStream_t st = S(stream);
+  for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
+    const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
+    h_chunk(c, psi + 2 * n0 * M, nullptr, n0, cnt, hpsi + 2 * n0 * M, true, st);
+    LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->part_e, c->P.nblk, cnt, c->dV, 0, c->eps + n0,
+           eps_dev ? eps_dev + n0 : nullptr);
+  }
+  return cuda_check(c, "apply_h");
+}
+
+// densities of the cnt spinors of a chunk (psi_chunk / scale_chunk already offset, n0 = global index of the
+// first), added into the raw sums (accumulate) or overwriting the selected planes.  Uses scr[0..3].
+static void dens_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_chunk, int64_t n0, int64_t cnt,
+                       unsigned mask, int accumulate, cudaStream_t st) {
+  const Plan& P = c->P;
+  const int64_t M = P.M;
+  DensArgs d; memset(&d, 0, sizeof d);
+  if (mask & (WSLDA_D_TAU | WSLDA_D_J)) {
+    DerivArgs a; memset(&a, 0, sizeof a);
+    a.src = psi_chunk; a.src_comp0 = 0; a.ncomp = (int)(2 * cnt); a.scale = scale_chunk;
+    for (int k = 0; k < P.nd; ++k) { a.out[1 + k] = c->scr[k]; d.grad[k] = c->scr[k]; }
+    deriv(c, a, st);
+  }
+  int64_t G = P.dG < cnt ? P.dG : cnt;
+  const int64_t per = (cnt + G - 1) / G;
+  G = (cnt + per - 1) / per;
+  d.psi = psi_chunk; d.scale = scale_chunk; d.cpref = c->cpref + n0; d.kperp2 = c->kperp2 + n0;
+  d.w_a = c->w_a + n0; d.w_b = c->w_b + n0; d.nd = P.nd; d.M = M; d.n_count = cnt; d.per_group = per; d.mask = mask;
+  LAUNCH(c, k_density, dim3(P.nblk, (unsigned)G), P.pt_threads, 0, st, d, c->dpart);
+  LAUNCH(c, k_density_reduce, dim3(nb(M, 256), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
+}
+
+extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t n_first, int64_t n_count, unsigned mask,
+                                        int accumulate, void* stream) {
+  if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
+  if (n_first < 0 || n_count < 0 || n_first + n_count > c->P.n_wf) return fail(c, WSLDA_EINVAL, "densities: spinor range out of bounds");
+  if (!mask || (mask & ~WSLDA_D_ALL)) return fail(c, WSLDA_EINVAL, "densities: bad which_mask");
+  cudaStream_t st = S(stream);
+  if (n_count == 0 && !accumulate) {
+    LAUNCH(c, k_density_reduce, dim3(nb(c->P.M, 256), DP_COUNT), 256, 0, st, c->dpart, 0, c->raw, c->P.M, mask, 0);
+  }
+  for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
+    const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
+    dens_chunk(c, (const cplx*)psi_ + 2 * n0 * c->P.M, nullptr, n0, cnt, mask, (accumulate || n0 > n_first) ? 1 : 0, st);
+  }
+  return cuda_check(c, "densities");
+}
+
+static void potentials(wslda_ctx* c, cudaStream_t st) {
+  if (c->f.func_id == WSLDA_FUNC_FIXED) return;
+  const int64_t M = c->P.M;
+  FuncParams fp;
+  fp.func_id = c->f.func_id; fp.force_a1 = c->f.force_a1; fp.spin_symmetric = c->f.spin_symmetric;
+  fp.four_pi_as = c->f.four_pi_as; fp.C = c->f.C; fp.E_cut = c->f.E_cut; fp.rho_floor = c->f.rho_floor;
+  fp.mu_a = c->mu_a; fp.mu_b = c->mu_b;
+  const int frozen = c->f.lambda_mode == 1 && c->lambda_valid;
+  LAUNCH(c, k_potentials, nb(M, 128), 128, 0, st, fp, c->raw, c->vext_a, c->vext_b, frozen, c->alpha_a, c->alpha_b, c->V_a,
+         c->V_b, c->U_a, c->U_b, c->lambda, c->geff, c->delta, M);
+  c->lambda_valid = 1;
+  if (c->f.kin_form == WSLDA_KIN_SYM40 && c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1) update_lap_alpha(c, st);
+}
+
+extern "C" wslda_status wslda_update_potentials(wslda_ctx* c, void* stream) {
+  if (!c) return WSLDA_EINVAL;
+  potentials(c, S(stream));
+  return cuda_check(c, "update_potentials");
+}
