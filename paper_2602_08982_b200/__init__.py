@@ -1,0 +1,250 @@
+"""Thin ctypes binding of libwslda (include/wslda.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``csrc/``; PyTorch is used for device memory and streams.
+There is no CPU fallback: without the built library or without a CUDA device the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libwslda.so")
+_SRC_DIR = os.path.join(_HERE, "csrc")
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
+              "-Xcompiler", "-fPIC"]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/wslda.cu for sm_100a into libwslda.so (in-tree)."""
+    srcs = [os.path.join(_SRC_DIR, f) for f in os.listdir(_SRC_DIR)]
+    srcs.append(os.path.join(os.path.dirname(_HERE), "include", "wslda.h"))
+    if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= max(os.path.getmtime(s) for s in srcs):
+        return _SO
+    nvcc = os.environ.get("NVCC", "nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(_SRC_DIR, "wslda.cu"), "-o", _SO]
+    subprocess.run(cmd, check=True)
+    return _SO
+
+
+class Functional(C.Structure):
+    _fields_ = [("func_id", C.c_int), ("force_a1", C.c_int), ("spin_symmetric", C.c_int), ("kin_form", C.c_int),
+                ("ab_order", C.c_int), ("am_order", C.c_int), ("subtract_mean_energy", C.c_int), ("normalize", C.c_int),
+                ("four_pi_as", C.c_double), ("C", C.c_double), ("E_cut", C.c_double), ("lambda_mode", C.c_int),
+                ("rho_floor", C.c_double)]
+
+
+FIELD = dict(rho_a=0, rho_b=1, tau_a=2, tau_b=3, nu=4, ja_x=5, ja_y=6, ja_z=7, jb_x=8, jb_y=9, jb_z=10,
+             alpha_a=16, alpha_b=17, U_a=18, U_b=19, delta=20, lap_alpha_a=21, lap_alpha_b=22, lambda_c=23,
+             g_eff=24, V_a=25, V_b=26)
+_COMPLEX = {4, 20}
+D_RHO, D_NU, D_TAU, D_J, D_ALL = 1, 2, 4, 8, 15
+SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "wslda_set_modes", "wslda_set_weights",
+           "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
+           "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
+           "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error"]
+
+_lib = None
+
+
+def lib():
+    """Load libwslda.so (building it if the sources are newer); raises if that fails."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            build()
+        L = C.CDLL(_SO)
+        L.wslda_workspace_bytes.restype = C.c_size_t
+        L.wslda_workspace_bytes.argtypes = [C.POINTER(C.c_int), C.c_int, C.c_int64, C.POINTER(Functional)]
+        L.wslda_ctx_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.POINTER(C.c_double), C.c_int,
+                                       C.c_int64, C.POINTER(Functional), C.c_void_p, C.c_size_t]
+        L.wslda_ctx_destroy.argtypes = [C.c_void_p]
+        L.wslda_set_modes.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_mu.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.wslda_set_external.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_potentials.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        L.wslda_get_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.wslda_set_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.wslda_apply_h.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
+        L.wslda_densities.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_uint, C.c_int, C.c_void_p]
+        L.wslda_update_potentials.argtypes = [C.c_void_p, C.c_void_p]
+        L.wslda_history_length.argtypes = [C.c_void_p]
+        L.wslda_abm_init.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_int, C.c_void_p]
+        L.wslda_abm_step.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
+        L.wslda_abm_step_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p,
+                                          C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
+        L.wslda_launch_count.restype = C.c_int64
+        L.wslda_launch_count.argtypes = [C.c_void_p]
+        L.wslda_last_error.restype = C.c_char_p
+        L.wslda_last_error.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+class WsldaError(RuntimeError):
+    pass
+
+
+def make_functional(func_id=0, force_a1=0, spin_symmetric=0, kin_form=0, ab_order=4, am_order=5,
+                    subtract_mean_energy=1, normalize=1, four_pi_as=-1.0, C_=-11.11, E_cut=None, lambda_mode=0,
+                    rho_floor=1e-14, dx0=1.0):
+    if E_cut is None:
+        E_cut = 3.141592653589793 ** 2 / (2 * dx0 ** 2)      # Eq. 22
+    return Functional(func_id, force_a1, spin_symmetric, kin_form, ab_order, am_order, subtract_mean_energy, normalize,
+                      four_pi_as, C_, E_cut, lambda_mode, rho_floor)
+
+
+def workspace_bytes(dims, mode, n_wf, functional) -> int:
+    d = (C.c_int * 3)(*(list(dims) + [1] * (3 - len(dims))))
+    return int(lib().wslda_workspace_bytes(d, int(mode), int(n_wf), C.byref(functional)))
+
+
+class Context:
+    """One wslda context on the current CUDA device.  Spinor buffers are torch complex128 CUDA tensors of shape
+    [n_wf, 2, *held_dims]; fields are float64 / complex128 CUDA tensors of shape held_dims."""
+
+    def __init__(self, mode, dims, dx, n_wf, **fkw):
+        import torch
+        if not torch.cuda.is_available():
+            raise WsldaError("wslda needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        dims = list(dims) + [1] * (3 - len(dims))
+        dx = list(dx) + [1.0] * (3 - len(dx))
+        self.f = make_functional(dx0=dx[0], **fkw)
+        self.mode, self.dims, self.dx, self.n_wf = int(mode), dims, dx, int(n_wf)
+        self.shape = tuple(dims[:mode])
+        self.M = 1
+        for s in self.shape:
+            self.M *= s
+        nbytes = workspace_bytes(dims, mode, n_wf, self.f)
+        if nbytes == 0:
+            raise WsldaError("wslda_workspace_bytes rejected the problem (dims must be powers of two >= 2)")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        self.ctx = C.c_void_p()
+        d = (C.c_int * 3)(*dims)
+        x = (C.c_double * 3)(*dx)
+        rc = lib().wslda_ctx_create(C.byref(self.ctx), d, x, self.mode, self.n_wf, C.byref(self.f),
+                                    self.workspace.data_ptr(), nbytes)
+        if rc:
+            raise WsldaError(f"wslda_ctx_create failed ({rc}): {lib().wslda_last_error(None).decode()}")
+        self.m = lib().wslda_history_length(self.ctx)
+
+    def __del__(self):
+        if getattr(self, "ctx", None):
+            lib().wslda_ctx_destroy(self.ctx)
+            self.ctx = None
+
+    # -- helpers
+    def _chk(self, rc, what):
+        if rc:
+            raise WsldaError(f"{what} failed ({rc}): {lib().wslda_last_error(self.ctx).decode()}")
+
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream().cuda_stream)
+
+    def _dev(self, a, dtype):
+        t = self.torch
+        if a is None:
+            return None
+        if not isinstance(a, t.Tensor):
+            a = t.as_tensor(a)
+        return a.to(device="cuda", dtype=dtype).contiguous()
+
+    @staticmethod
+    def _ptr(t):
+        return None if t is None else C.c_void_p(t.data_ptr())
+
+    # -- setters
+    def set_modes(self, kperp, mult, first):
+        import numpy as np
+        kperp = np.ascontiguousarray(kperp, dtype=np.float64)
+        mult = np.ascontiguousarray(mult, dtype=np.float64)
+        first = np.ascontiguousarray(first, dtype=np.int64)
+        self._chk(lib().wslda_set_modes(self.ctx, len(mult), kperp.ctypes.data, mult.ctypes.data, first.ctypes.data),
+                  "set_modes")
+
+    def set_weights(self, w_a, w_b):
+        t = self.torch
+        a, b = self._dev(w_a, t.float64), self._dev(w_b, t.float64)
+        self._chk(lib().wslda_set_weights(self.ctx, self._ptr(a), self._ptr(b)), "set_weights")
+
+    def set_mu(self, mu_a, mu_b):
+        self._chk(lib().wslda_set_mu(self.ctx, float(mu_a), float(mu_b)), "set_mu")
+
+    def set_external(self, vext_a=None, vext_b=None, delta_ext=None):
+        t = self.torch
+        a, b, d = self._dev(vext_a, t.float64), self._dev(vext_b, t.float64), self._dev(delta_ext, t.complex128)
+        self._chk(lib().wslda_set_external(self.ctx, self._ptr(a), self._ptr(b), self._ptr(d)), "set_external")
+
+    def set_potentials(self, alpha_a, alpha_b, U_a, U_b, delta):
+        t = self.torch
+        args = [self._dev(x, t.float64) for x in (alpha_a, alpha_b, U_a, U_b)] + [self._dev(delta, t.complex128)]
+        self._chk(lib().wslda_set_potentials(self.ctx, *[self._ptr(x) for x in args], self._stream()), "set_potentials")
+        t.cuda.current_stream().synchronize()
+
+    def get_field(self, name):
+        t = self.torch
+        fid = FIELD[name]
+        out = t.empty(self.shape, dtype=t.complex128 if fid in _COMPLEX else t.float64, device="cuda")
+        self._chk(lib().wslda_get_field(self.ctx, fid, self._ptr(out), self._stream()), "get_field")
+        return out
+
+    def set_field(self, name, value):
+        t = self.torch
+        fid = FIELD[name]
+        v = self._dev(value, t.complex128 if fid in _COMPLEX else t.float64)
+        self._chk(lib().wslda_set_field(self.ctx, fid, self._ptr(v), self._stream()), "set_field")
+        t.cuda.current_stream().synchronize()
+
+    # -- the path
+    def apply_h(self, psi, hpsi=None, eps=None, n_first=0, n_count=None):
+        t = self.torch
+        n_count = self.n_wf - n_first if n_count is None else n_count
+        if hpsi is None:
+            hpsi = t.zeros_like(psi)
+        if eps is None:
+            eps = t.zeros(self.n_wf, dtype=t.float64, device="cuda")
+        self._chk(lib().wslda_apply_h(self.ctx, self._ptr(psi), self._ptr(hpsi), self._ptr(eps), n_first, n_count,
+                                      self._stream()), "apply_h")
+        return hpsi, eps
+
+    def densities(self, psi, n_first=0, n_count=None, which=D_ALL, accumulate=0):
+        n_count = self.n_wf - n_first if n_count is None else n_count
+        self._chk(lib().wslda_densities(self.ctx, self._ptr(psi), n_first, n_count, which, accumulate, self._stream()),
+                  "densities")
+
+    def update_potentials(self):
+        self._chk(lib().wslda_update_potentials(self.ctx, self._stream()), "update_potentials")
+
+    def _hist(self, f_hist):
+        assert len(f_hist) == self.m, f"need {self.m} history buffers"
+        return (C.c_void_p * self.m)(*[x.data_ptr() for x in f_hist])
+
+    @staticmethod
+    def _reorder(f_hist, ptrs):
+        by = {x.data_ptr(): x for x in f_hist}
+        return [by[p] for p in ptrs]
+
+    def abm_init(self, phi, f_hist, dt, selfstart=1):
+        ptrs = self._hist(f_hist)
+        self._chk(lib().wslda_abm_init(self.ctx, self._ptr(phi), ptrs, float(dt), int(selfstart), self._stream()), "abm_init")
+        return self._reorder(f_hist, list(ptrs))
+
+    def abm_step(self, phi, f_hist, dt):
+        ptrs = self._hist(f_hist)
+        self._chk(lib().wslda_abm_step(self.ctx, self._ptr(phi), ptrs, float(dt), self._stream()), "abm_step")
+        return self._reorder(f_hist, list(ptrs))
+
+    def abm_step_host(self, phi_host, f_hist_host, phi, f_hist, dt):
+        """End-to-end step from (pinned) host tensors; returns the permuted (host, device) history lists."""
+        hp = (C.c_void_p * self.m)(*[x.data_ptr() for x in f_hist_host])
+        dp = self._hist(f_hist)
+        self._chk(lib().wslda_abm_step_host(self.ctx, C.c_void_p(phi_host.data_ptr()), hp, self._ptr(phi), dp, float(dt),
+                                            self._stream()), "abm_step_host")
+        byh = {x.data_ptr(): x for x in f_hist_host}
+        return [byh[p] for p in hp], self._reorder(f_hist, list(dp))
+
+    def launch_count(self):
+        return int(lib().wslda_launch_count(self.ctx))

@@ -1,0 +1,188 @@
+"""GPU-vs-oracle parity through the C-ABI (run with -m gpu on a B200).
+
+Tolerances are north_star's: one H-apply 1e-12, densities 1e-11, 100 ABM steps 1e-9, all as
+max|x - ref| / max|ref| over the returned array.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+from harness import make_gpu, make_oracle, relerr, to_gpu, to_np
+
+pytestmark = pytest.mark.gpu
+
+TOL_H, TOL_D, TOL_ABM = 1e-12, 1e-11, 1e-9
+DENS = ["rho_a", "rho_b", "tau_a", "tau_b", "nu", "ja_x", "ja_y", "ja_z", "jb_x", "jb_y", "jb_z"]
+POTS = ["alpha_a", "alpha_b", "V_a", "V_b", "U_a", "U_b", "delta", "lambda_c", "g_eff", "lap_alpha_a", "lap_alpha_b"]
+
+
+def random_fields(seed, shape):
+    M = int(np.prod(shape))
+    z = wl.normal(seed, 0, 6 * M).reshape(6, *shape)
+    return dict(alpha_a=1.1 + 0.2 * np.tanh(z[0]), alpha_b=0.9 + 0.2 * np.tanh(z[1]), U_a=0.3 * z[2], U_b=0.3 * z[3],
+                delta=0.2 + 0.1 * (z[4] + 1j * z[5]))
+
+
+def generic(shape, dx, n_wf, kin_form, func_id=0, seed=5, n_modes=1, full_dims=None, **kw):
+    """A small random workload on an arbitrary lattice (fixed random fields, random weights, random modes)."""
+    mode = len(shape)
+    dims = tuple(shape) + (1,) * (3 - mode) if full_dims is None else full_dims
+    dxs = tuple(dx) + (1.0,) * (3 - mode)
+    u = wl.uniform01(seed + 1, 0, 2 * n_wf)
+    base = dict(ab_order=4, am_order=5, dt=0.004, n_steps=10, mu=(0.4, 0.3))
+    base.update(kw)
+    w = wl.Workload(f"generic{shape}", mode, dims, dxs, n_wf, func_id, base.pop("force_a1", 0),
+                    base.pop("spin_symmetric", 0), kin_form, base.pop("ab_order"), base.pop("am_order"), base.pop("dt"),
+                    base.pop("n_steps"), base.pop("mu"), w_a=u[:n_wf], w_b=u[n_wf:], **base)
+    if func_id == 0:
+        w.fixed = random_fields(seed + 2, shape)
+    if n_modes > 1 or mode < 3:
+        n_modes = max(n_modes, 1)
+        kp = 0.3 * wl.normal(seed + 3, 0, 2 * n_modes).reshape(n_modes, 2)
+        if mode == 2:
+            kp[:, 1] = 0.0
+        w.kperp, w.mult = kp, 1.0 + np.arange(n_modes) % 2
+        w.first = np.linspace(0, n_wf, n_modes + 1).astype(np.int64)
+    return w
+
+
+def spinors(w, seed=9):
+    return wl.random_spinors(seed, w.n_wf, w.shape, w.dV)
+
+
+SHAPES = [((8, 4, 8), (1.0, 0.9, 1.1)), ((16, 8), (1.0, 1.2)), ((32,), (0.8,)), ((2, 2, 4), (1.0, 1.0, 1.0)),
+          ((32, 16, 16), (1.0, 1.0, 0.9)),      # 8192 points: the multi-pass (large lattice) regime
+          ((128, 64), (1.0, 1.1))]              # 2-D lattice in the large regime
+
+
+@pytest.mark.parametrize("kin_form", [0, 1, 2])
+@pytest.mark.parametrize("shape,dx", SHAPES)
+def test_apply_h_matches_oracle(shape, dx, kin_form):
+    n_wf = 7 if np.prod(shape) > 4096 else 19            # ragged against every chunk / group size
+    w = generic(shape, dx, n_wf, kin_form, n_modes=3)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi)
+    h, e = g.apply_h(to_gpu(psi))
+    assert relerr(to_np(h), ref) < TOL_H
+    assert relerr(to_np(e), eref) < TOL_H
+    # sub-range call leaves the other spinors untouched
+    h2, _ = g.apply_h(to_gpu(psi), n_first=2, n_count=3)
+    h2 = to_np(h2)
+    assert relerr(h2[2:5], ref[2:5]) < TOL_H and not h2[:2].any() and not h2[5:].any()
+
+
+@pytest.mark.parametrize("shape,dx", SHAPES)
+@pytest.mark.parametrize("sym", [0, 1])
+def test_densities_match_oracle(shape, dx, sym):
+    n_wf = 9 if np.prod(shape) > 4096 else 37
+    w = generic(shape, dx, n_wf, 0, n_modes=4, spin_symmetric=sym)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    o.densities(psi)
+    gp = to_gpu(psi)
+    g.densities(gp)
+    names = DENS[:5] + [f"j{s}_{'xyz'[d]}" for s in "ab" for d in range(len(shape))]
+    for name in names:
+        assert relerr(to_np(g.get_field(name)), o.get_field(name)) < TOL_D, name
+    # batch streaming: two accumulating calls give the same sums
+    g.densities(gp, 0, 4, accumulate=0)
+    g.densities(gp, 4, n_wf - 4, accumulate=1)
+    for name in names:
+        assert relerr(to_np(g.get_field(name)), o.get_field(name)) < TOL_D, name
+
+
+@pytest.mark.parametrize("func_id,force_a1,sym", [(1, 0, 0), (2, 0, 0), (2, 1, 0), (2, 0, 1), (2, 1, 1)])
+@pytest.mark.parametrize("kin_form", [0, 1])
+def test_potentials_match_oracle(func_id, force_a1, sym, kin_form):
+    shape, dx = (8, 8, 4), (1.0, 1.0, 1.0)
+    n_wf = 64
+    w = generic(shape, dx, n_wf, kin_form, func_id=func_id, force_a1=force_a1, spin_symmetric=sym, mu=(0.5, 0.35))
+    X = np.meshgrid(*[np.arange(s) - s // 2 for s in shape], indexing="ij")
+    w.vext_a = 0.02 * sum(x * x for x in X).astype(float)
+    w.vext_b = w.vext_a * 1.1
+    # realistic density scale: 64 spinors on 256 points, weights of order one, times 1/dV
+    psi = spinors(w) * 1.5
+    o, g = make_oracle(w), make_gpu(w)
+    o.densities(psi); o.update_potentials()
+    g.densities(to_gpu(psi)); g.update_potentials()
+    for name in POTS:
+        ref = o.get_field(name)
+        got = to_np(g.get_field(name))
+        scale = max(np.max(np.abs(ref)), 1e-300)
+        assert np.max(np.abs(got - ref)) / scale < TOL_D or np.max(np.abs(got - ref)) < 1e-13, name
+    # frozen Lambda_c: second update with lambda_mode = 1 reuses the field
+    o2, g2 = make_oracle(w, lambda_mode=1), make_gpu(w, lambda_mode=1)
+    lam = np.abs(wl.normal(3, 0, int(np.prod(shape)))).reshape(shape) * 0.05
+    o2.set_field("lambda_c", lam); g2.set_field("lambda_c", lam)
+    o2.densities(psi); o2.update_potentials()
+    g2.densities(to_gpu(psi)); g2.update_potentials()
+    assert relerr(to_np(g2.get_field("delta")), o2.get_field("delta")) < TOL_D
+    assert relerr(to_np(g2.get_field("lambda_c")), lam) == 0.0
+
+
+def run_both(w, psi0, n_steps, selfstart=1, n_wf=None):
+    """abm_init + n_steps abm_steps on both sides; returns (phi_gpu, phi_oracle, f0_gpu, f0_oracle, o, g)."""
+    import torch
+    o, g = make_oracle(w, n_wf), make_gpu(w, n_wf)
+    phi_o = psi0.copy()
+    hist_o = [np.zeros_like(psi0) for _ in range(o.m)]
+    phi_g = to_gpu(psi0)
+    hist_g = [torch.zeros_like(phi_g) for _ in range(g.m)]
+    assert g.m == o.m
+    hist_o = o.abm_init(phi_o, hist_o, w.dt, selfstart)
+    hist_g = g.abm_init(phi_g, hist_g, w.dt, selfstart)
+    for _ in range(n_steps):
+        hist_o = o.abm_step(phi_o, hist_o, w.dt)
+        hist_g = g.abm_step(phi_g, hist_g, w.dt)
+    return to_np(phi_g), phi_o, to_np(hist_g[0]), hist_o[0], o, g
+
+
+def test_cfg1_100_steps_bdg_8cubed():
+    """configs[0]: full basis of 1024 spinors on 8^3, AB4AM4, 100 steps (3 Taylor + 97 ABM), fixed potentials."""
+    w = wl.cfg1()
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps - (w.history - 1))
+    assert relerr(pg, po) < TOL_ABM
+    assert relerr(fg, fo) < TOL_ABM
+
+
+@pytest.mark.parametrize("ab,am", [(3, 4), (4, 4), (4, 5), (5, 5)])
+@pytest.mark.parametrize("selfstart,normalize,shift", [(1, 1, 1), (0, 1, 1), (1, 0, 0), (1, 1, 0)])
+def test_abm_fixed_potentials_all_orders(ab, am, selfstart, normalize, shift):
+    w = generic((8, 4, 8), (1.0, 0.9, 1.1), 21, 1, ab_order=ab, am_order=am, normalize=normalize,
+                subtract_mean_energy=shift, dt=0.004)
+    pg, po, fg, fo, _, _ = run_both(w, spinors(w), 12, selfstart)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4_sym40", "cfg4_divgrad", "bdg_large", "aslda_polarised"])
+def test_abm_selfconsistent_reduced_configs(name):
+    """Self-consistent stepping on reduced versions of configs[1..3] (same recipes, fewer modes / points)."""
+    if name == "cfg2":
+        w = wl.cfg2(n_modes_side=4, nx=32, n_steps=20)              # 16 modes x 64 spinors, quasi-1D
+    elif name == "cfg3":
+        w = wl.cfg3(n_side=16, n_kz=3, nz=8, n_steps=20)            # 3 kz x 256 spinors, quasi-2D, vortex
+    elif name == "cfg4_sym40":
+        w = wl.cfg4(n_side=8, kin_form=1, n_steps=20)               # 256 spinors on 8^3, trap, general alpha
+    elif name == "cfg4_divgrad":
+        w = wl.cfg4(n_side=8, kin_form=2, n_steps=20)
+    elif name == "bdg_large":
+        w = generic((32, 16, 16), (1.0, 1.0, 1.0), 24, 0, func_id=1, four_pi_as=-2.0, dt=0.005)
+        w.n_steps = 6
+    else:
+        w = generic((8, 8, 8), (1.0, 1.0, 1.0), 96, 1, func_id=2, mu=(0.5, 0.3), dt=0.005)
+        w.n_steps = 12
+    psi0 = w.spinors() if w.kidx is not None else spinors(w)
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("delta", "U_a", "U_b", "alpha_a"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+
+
+def test_run_to_run_bit_reproducible():
+    w = wl.cfg3(n_side=16, n_kz=2, nz=8, n_steps=5)
+    psi0 = w.spinors()
+    a = run_both(w, psi0, 5)[0]
+    b = run_both(w, psi0, 5)[0]
+    assert np.array_equal(a, b)
