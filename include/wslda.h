@@ -104,8 +104,9 @@ wslda_status wslda_apply_h(wslda_ctx*, const void* psi_dev, void* hpsi_dev, doub
  * context's raw sums; accumulate = 0 overwrites the selected fields, 1 adds (batch streaming). */
 wslda_status wslda_densities(wslda_ctx*, const void* psi_dev, int64_t n_first, int64_t n_count,
                              unsigned which_mask, int accumulate, void* cuda_stream);
-/* Rebuild alpha_sigma, V_sigma, U_sigma, Lambda_c, g_eff, Delta and lap(alpha_sigma) pointwise from the
- * current densities (Eqs. 9-12, 19-22 PAPER.md:195-255, 311-337).  FUNC_FIXED: no-op. */
+/* Rebuild alpha_sigma, V_sigma, U_sigma, Lambda_c, g_eff, Delta pointwise from the current densities
+ * (Eqs. 9-12, 19-22 PAPER.md:195-255, 311-337) and, for kin_form = SYM40 with a density-dependent alpha,
+ * lap(alpha_sigma) spectrally.  FUNC_FIXED: no-op. */
 wslda_status wslda_update_potentials(wslda_ctx*, void* cuda_stream);
 
 /* History length m = max(ab_order, am_order-1). */

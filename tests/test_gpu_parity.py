@@ -107,6 +107,8 @@ def test_potentials_match_oracle(func_id, force_a1, sym, kin_form):
     o.densities(psi); o.update_potentials()
     g.densities(to_gpu(psi)); g.update_potentials()
     for name in POTS:
+        if name.startswith("lap_alpha") and kin_form != 1:
+            continue                      # lap(alpha) is only built (and consumed) by the Eq. 40 form
         ref = o.get_field(name)
         got = to_np(g.get_field(name))
         scale = max(np.max(np.abs(ref)), 1e-300)
