@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- whole ABM steps of the TDSLDA/BdG path on B200 (see DESIGN.md section 7 for every definition).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4|cfg5|cfg3|cfg2|cfg1] [--n-wf n]
+    python bench.py --impl reference ...       # the CPU oracle on the host cores (rank 0 only)
+
+One "step" = one complete wslda_abm_step (Alg. 2: predictor, H P, corrector, H phi, with the densities and
+potentials rebuilt at both stages when the functional is self-consistent) over the whole resident spinor
+batch.  metric = quasiparticle-wavefunction time steps per second = n_wf * K / time.  Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+import workloads as wl  # noqa: E402
+
+METRIC = "qp_wavefunction_time_steps_per_s"
+UNIT = "spinor-steps/s"
+
+
+def make_workload(name, n_wf=None):
+    if name == "cfg1":
+        return wl.cfg1(n_wf), "configs[0]: 3D BdG 8^3, fixed potentials, AB4AM4"
+    if name == "cfg2":
+        w = wl.cfg2()
+        return w, "configs[1]: quasi-1D SLDA Nx=128, 32x32 modes x 256 spinors, self-consistent, AB4AM5"
+    if name == "cfg3":
+        w = wl.cfg3()
+        return w, "configs[2]: quasi-2D SLDA vortex 64^2 x 16 kz, self-consistent, AB4AM5"
+    if name == "cfg4":
+        return wl.cfg4(n_wf=n_wf), "configs[3]: 3D SLDA 32^3 trap, general-alpha Eq.40 operator, self-consistent, AB4AM5"
+    if name == "cfg5":
+        return wl.cfg5(n_wf=n_wf or 2048), "configs[4]: 3D ASLDA-like 64^3, h_a != h_b, fixed smooth potentials, AB4AM5"
+    raise SystemExit(f"unknown config {name}")
+
+
+def restrict(w, n_wf):
+    """The same workload on its first n_wf spinors (mode table clipped)."""
+    import copy
+    v = copy.copy(w)
+    v.n_wf = n_wf
+    for k in ("kidx", "branch", "mode_of", "w_a", "w_b", "E"):
+        a = getattr(w, k)
+        if a is not None:
+            setattr(v, k, a[:n_wf])
+    if w.first is not None:
+        v.first = np.minimum(np.asarray(w.first), n_wf)
+    return v
+
+
+def alg_bytes_per_spinor_step(w):
+    """full-buffer accesses Alg. 2 itself needs, x 32 M bytes."""
+    m = w.history
+    if w.func_id == 0:
+        acc = (1 + m) + 2                       # read phi, f_1..f_m; write phi_new, f_new
+    else:
+        acc = (1 + m) + 2 + 3 + 2               # + write P, C_part | read P, C_part, write phi | read phi, write f
+    return acc * 32 * w.M
+
+
+def ffts_per_spinor_step(w):
+    """Transforms Alg. 2 needs per spinor-step: per component and H-apply 2 (Eq. 14), 4 (Eq. 40: w and alpha w,
+    forward and inverse) or 1 + 3 nd (successive first derivatives); x 2 components x 2 H-applies."""
+    per_comp = {0: 2, 1: 4, 2: 1 + 3 * w.mode}[w.kin_form]
+    return 2 * 2 * per_comp
+
+
+def alg_flops_per_spinor_step(w):
+    return ffts_per_spinor_step(w) * 5.0 * w.M * math.log2(w.M) + 300.0 * w.M
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled in the background during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if val.strip().lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(w, budget_s=20.0, steps=2):
+    """The oracle as it stands on the host cores: abm steps on the first n_sub spinors of the workload."""
+    import oracle as orc
+    from harness import make_oracle
+    threads = orc.num_threads()
+    n_sub = min(w.n_wf, max(threads, 1) * 2)
+    best = None
+    while True:
+        ws_ = restrict(w, n_sub)
+        o = make_oracle(ws_)
+        phi = ws_.spinors()
+        hist = [np.zeros_like(phi) for _ in range(o.m)]
+        hist = o.abm_init(phi, hist, ws_.dt, 0)
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            hist = o.abm_step(phi, hist, ws_.dt)
+        dt = time.perf_counter() - t0
+        best = (n_sub, dt)
+        if dt >= budget_s / 4 or n_sub >= w.n_wf or n_sub * 32 * w.M * (o.m + 2) > 8e9:
+            break
+        n_sub = min(w.n_wf, int(n_sub * min(8.0, max(2.0, budget_s / 2 / max(dt, 1e-3)))))
+    n_sub, dt = best
+    return {"value": n_sub * steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{steps} abm steps on the first {n_sub} of {w.n_wf} spinors (zero-history start), {dt:.2f} s; "
+                      f"cost is linear in n_wf (PAPER.md:1053)"}, dt / steps * 1e3
+
+
+def run_reference(args):
+    """--impl reference: W + K abm steps of the oracle on a bounded sample of the workload (host cores)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, desc = make_workload(args.config, args.n_wf)
+    import oracle as orc
+    from harness import make_oracle
+    orc.build()
+    cal, _ = time_oracle(w, budget_s=4.0, steps=1)                 # calibration: spinor-steps/s
+    total = args.steps + args.warmup
+    n_sub = int(min(w.n_wf, max(orc.num_threads(), cal["value"] * 90.0 / total)))
+    n_sub = int(min(n_sub, 8e9 / (32 * w.M * (w.history + 2))))
+    ws_ = restrict(w, n_sub)
+    o = make_oracle(ws_)
+    phi = ws_.spinors()
+    hist = [np.zeros_like(phi) for _ in range(o.m)]
+    hist = o.abm_init(phi, hist, ws_.dt, 0)
+    for _ in range(args.warmup):
+        hist = o.abm_step(phi, hist, ws_.dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        hist = o.abm_step(phi, hist, ws_.dt)
+    dt = time.perf_counter() - t0
+    v = n_sub * args.steps / dt
+    sample = f"{args.steps} abm steps on the first {n_sub} of {w.n_wf} spinors (zero-history start), {dt:.2f} s"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128",
+                      "data": "synthetic", "config": {"workload": desc, "n_wf": w.n_wf, "M": w.M},
+                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                                       "sample": sample},
+                      "gpu_launches": 0,
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2602_08982_b200 as ws
+    from harness import make_gpu
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ws.build()
+    w, desc = make_workload(args.config, args.n_wf)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md 6.65 TB/s)"
+    fp64_peak = 35.2e12            # measured DFMA-chain rate on this pool's B200 (148 SMs x 64 lanes x 2 x 1.965 GHz = 37.2 nominal)
+
+    # ---- resident state: every rank holds its own replica of the workload ("replicas only")
+    g = make_gpu(w)
+    shape = (w.n_wf, 2) + w.shape
+    phi = torch.empty(shape, dtype=torch.complex128, device="cuda")
+    wl.spinors_device(w, 0, w.n_wf, phi)
+    hist = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(g.m)]
+    torch.cuda.synchronize()
+    hist = g.abm_init(phi, hist, w.dt, 0)            # zero-history start: the timed steps are plain Alg. 2 steps
+    for _ in range(args.warmup):
+        hist = g.abm_step(phi, hist, w.dt)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    l0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        hist = g.abm_step(phi, hist, w.dt)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    finite = bool(torch.isfinite(torch.view_as_real(phi[:: max(1, w.n_wf // 64)])).all())
+    value = world * w.n_wf * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel device times (separate pass, event pairs around every launch) -> dominant kernel
+    prof_steps = min(args.steps, 2)
+    g.profile(True)
+    for _ in range(prof_steps):
+        hist = g.abm_step(phi, hist, w.dt)
+    rep = g.profile_report()
+    g.profile(False)
+    tot_ms = sum(v[1] for v in rep.values()) or 1.0
+    kern = sorted(rep.items(), key=lambda kv: -kv[1][1])
+    top, (top_cnt, top_ms, top_bytes, top_flops) = kern[0]
+    t_b, t_f = top_bytes / (hbm_peak * 1e9), top_flops / fp64_peak
+    if t_b >= t_f:
+        ach = top_bytes / (top_ms * 1e-3) / 1e9
+        roof = {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "traffic": None, "peak_source": peak_src}
+    else:
+        ach = top_flops / (top_ms * 1e-3) / 1e12
+        roof = {"kernel": top, "bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+                "frac": ach / (fp64_peak / 1e12), "traffic": None,
+                "peak_source": "measured FP64 DFMA chain on this pool's B200 (DESIGN.md 7)"}
+    roof.update({"share_of_step": top_ms / tot_ms, "launches_per_step": top_cnt / prof_steps,
+                 "avg_launch_ms": top_ms / top_cnt, "alg_bytes_per_launch": top_bytes / top_cnt,
+                 "alg_flops_per_launch": top_flops / top_cnt})
+    B, F = alg_bytes_per_spinor_step(w), alg_flops_per_spinor_step(w)
+    t_roof = max(B / (hbm_peak * 1e9), F / fp64_peak)
+    step_roof = {"bound": "hbm" if B / (hbm_peak * 1e9) >= F / fp64_peak else "alu",
+                 "t_roof_us_per_spinor_step": t_roof * 1e6, "t_measured_us_per_spinor_step": 1e6 * world / value,
+                 "frac": t_roof * value / world, "bytes_per_spinor_step": B, "flops_per_spinor_step": F,
+                 "hbm_gbs_achieved": B * value / world / 1e9, "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak / 1e12}
+    kernels = {k: {"launches_per_step": v[0] / prof_steps, "ms_per_step": round(v[1] / prof_steps, 4),
+                   "share": round(v[1] / tot_ms, 4)} for k, v in kern}
+    del hist, phi
+    torch.cuda.empty_cache()
+
+    # ---- end to end: the same step through wslda_abm_step_host (pinned HOST buffers, copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        n_e = min(w.n_wf, max(1, int(2 ** 31 // (32 * w.M))))          # <= 2 GiB per buffer on the host
+        we = restrict(w, n_e)
+        del g
+        torch.cuda.empty_cache()
+        ge = make_gpu(we)
+        shp = (n_e, 2) + w.shape
+        dphi = torch.empty(shp, dtype=torch.complex128, device="cuda")
+        wl.spinors_device(we, 0, n_e, dphi)
+        dh = [torch.zeros(shp, dtype=torch.complex128, device="cuda") for _ in range(ge.m)]
+        dh = ge.abm_init(dphi, dh, w.dt, 0)
+        hphi = torch.empty(shp, dtype=torch.complex128).pin_memory()
+        hphi.copy_(dphi)
+        hh = [torch.zeros(shp, dtype=torch.complex128).pin_memory() for _ in range(ge.m)]
+        hh, dh = ge.abm_step_host(hphi, hh, dphi, dh, w.dt)               # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        n_e2e_steps = max(1, min(args.steps, 3))
+        for _ in range(n_e2e_steps):
+            hh, dh = ge.abm_step_host(hphi, hh, dphi, dh, w.dt)
+        e1.record()
+        barrier()
+        ms_e = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms_e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        buf = n_e * 32 * w.M
+        e2e = {"value": world * n_e * n_e2e_steps / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": buf * (1 + ge.m),
+               "d2h_bytes_per_step": 2 * buf, "n_wf": n_e, "steps": n_e2e_steps,
+               "note": "wslda_abm_step_host: phi + m history buffers copied host->device, phi_new and f_new device->host, every step"}
+        del ge, dphi, dh, hphi, hh
+        torch.cuda.empty_cache()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        import oracle as orc
+        orc.build()
+        cpu, _ = time_oracle(w, budget_s=20.0, steps=2)
+
+    if rank == 0:
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "c128", "data": "synthetic",
+               "config": {"workload": desc, "name": w.name, "n_wf_per_gpu": w.n_wf, "M": w.M, "mode": w.mode,
+                          "kin_form": w.kin_form, "func_id": w.func_id, "ab_am": [w.ab_order, w.am_order], "dt": w.dt,
+                          "resident_bytes": (1 + w.history) * w.n_wf * 32 * w.M, "parallelism": f"replicas x{world}",
+                          "l2": "inputs larger than L2 (no flush)" if (1 + w.history) * w.n_wf * 32 * w.M > 4e8
+                                else "working set near L2 size: numbers are L2-assisted"},
+               "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof,
+               "kernels": kernels, "cpu_baseline": cpu, "finite": finite}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="wslda", choices=["wslda", "reference"])
+    ap.add_argument("--config", default="cfg4")
+    ap.add_argument("--n-wf", type=int, default=None)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

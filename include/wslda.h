@@ -126,6 +126,15 @@ wslda_status wslda_abm_step(wslda_ctx*, void* phi_dev, void** f_hist, double dt,
  * stream.  phi_host / f_hist_host[i]: host (pinned for full speed); f_hist_host is permuted like f_hist_dev. */
 wslda_status wslda_abm_step_host(wslda_ctx*, void* phi_host, void** f_hist_host, void* phi_dev, void** f_hist_dev,
                                  double dt, void* cuda_stream);
+/* Per-kernel device timing for the bench's roofline accounting: while enabled (enable = 1 also clears the
+ * record) every kernel launch is bracketed by a CUDA event pair on its own stream (at most 20000 launches are
+ * recorded).  wslda_profile_report synchronises the device and writes one line
+ *   "kernel_name launches total_ms algorithmic_bytes algorithmic_flops"
+ * per kernel into buf (host, buf_bytes long); the last two are the sums of the compulsory HBM bytes and the
+ * 5 N log2 N FFT flops the library attributes to those launches.  Returns the number
+ * of kernels, -1 on bad arguments. */
+wslda_status wslda_profile(wslda_ctx*, int enable);
+int wslda_profile_report(wslda_ctx*, char* buf, size_t buf_bytes);
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 int64_t wslda_launch_count(const wslda_ctx*);
 const char* wslda_last_error(const wslda_ctx*);

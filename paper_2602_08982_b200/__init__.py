@@ -43,7 +43,8 @@ D_RHO, D_NU, D_TAU, D_J, D_ALL = 1, 2, 4, 8, 15
 SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "wslda_set_modes", "wslda_set_weights",
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
-           "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error"]
+           "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
+           "wslda_profile_report"]
 
 _lib = None
 
@@ -75,6 +76,8 @@ def lib():
         L.wslda_abm_step.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
         L.wslda_abm_step_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p,
                                           C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
+        L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
+        L.wslda_profile_report.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.wslda_launch_count.restype = C.c_int64
         L.wslda_launch_count.argtypes = [C.c_void_p]
         L.wslda_last_error.restype = C.c_char_p
@@ -245,6 +248,19 @@ class Context:
                                             self._stream()), "abm_step_host")
         byh = {x.data_ptr(): x for x in f_hist_host}
         return [byh[p] for p in hp], self._reorder(f_hist, list(dp))
+
+    def profile(self, enable=True):
+        self._chk(lib().wslda_profile(self.ctx, int(bool(enable))), "profile")
+
+    def profile_report(self):
+        """{kernel name: (launches, total_ms, algorithmic bytes, algorithmic flops)} recorded since profile(True); synchronises the device."""
+        buf = C.create_string_buffer(1 << 16)
+        lib().wslda_profile_report(self.ctx, buf, len(buf))
+        out = {}
+        for line in buf.value.decode().splitlines():
+            name, cnt, ms, nbytes, flops = line.split()
+            out[name] = (int(cnt), float(ms), float(nbytes), float(flops))
+        return out
 
     def launch_count(self):
         return int(lib().wslda_launch_count(self.ctx))

@@ -90,6 +90,12 @@ struct wslda_ctx {
   double *part_n, *part_e, *dpart;
   cplx* scr[WS_MAX_SCR];
   int64_t launches;
+  // optional per-kernel timing (wslda_profile): event pairs around every launch while enabled
+  int prof_on, prof_n;
+  std::vector<cudaEvent_t>* prof_ev;
+  std::vector<const char*>* prof_name;
+  std::vector<double>* prof_work;    // per recorded launch: algorithmic bytes, flops (set with WORK() before LAUNCH)
+  double work_bytes, work_flops;
   char err[256];
 };
 
@@ -104,8 +110,25 @@ static wslda_status cuda_check(wslda_ctx* c, const char* where) {
   snprintf(c ? c->err : g_err, 256, "CUDA error at %s: %s", where, cudaGetErrorString(e));
   return WSLDA_ECUDA;
 }
-#define LAUNCH(c, kern, grid, block, smem, st, ...)            \
-  do { kern<<<grid, block, smem, st>>>(__VA_ARGS__); (c)->launches++; } while (0)
+#define WS_PROF_MAX 20000
+static inline bool prof_begin(wslda_ctx* c, const char* name, cudaStream_t st) {
+  if (!c->prof_on || c->prof_n >= WS_PROF_MAX) return false;
+  if ((int)c->prof_ev->size() < 2 * (c->prof_n + 1)) {
+    cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+    c->prof_ev->push_back(a); c->prof_ev->push_back(b);
+  }
+  c->prof_name->push_back(name);
+  c->prof_work->push_back(c->work_bytes); c->prof_work->push_back(c->work_flops);
+  cudaEventRecord((*c->prof_ev)[2 * c->prof_n], st);
+  return true;
+}
+static inline void prof_end(wslda_ctx* c, cudaStream_t st) { cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], st); c->prof_n++; }
+#define LAUNCH(c, kern, grid, block, smem, st, ...)                                   \
+  do { bool pr_ = prof_begin(c, #kern, st); kern<<<grid, block, smem, st>>>(__VA_ARGS__); \
+       if (pr_) prof_end(c, st); (c)->launches++; (c)->work_bytes = 0; (c)->work_flops = 0; } while (0)
+// algorithmic work of the NEXT launch (compulsory HBM bytes: unique full-buffer inputs + outputs; FFT flops as
+// 5 N log2 N per line transform) -- only used by the profile report
+#define WORK(c, bytes, flops) do { (c)->work_bytes = (double)(bytes); (c)->work_flops = (double)(flops); } while (0)
 
 // stored position p of the in-place DIF transform (radix 4 from L = n down, then radix 2) <-> frequency index
 static void scrambled_freq(int n, std::vector<int>& fr) {
@@ -140,6 +163,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   wslda_ctx* c = (wslda_ctx*)calloc(1, sizeof(wslda_ctx));
   if (!c) return fail(nullptr, WSLDA_ENOMEM, "host allocation failed");
   c->P = P; c->f = *f;
+  c->prof_ev = new std::vector<cudaEvent_t>(); c->prof_name = new std::vector<const char*>();
+  c->prof_work = new std::vector<double>();
   c->m = f->ab_order > f->am_order - 1 ? f->ab_order : f->am_order - 1;
   c->dV = 1.0; c->Lperp = 1.0;
   for (int d = 0; d < 3; ++d) {
@@ -211,8 +236,38 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   return WSLDA_OK;
 }
 
+// ---- per-kernel timing ------------------------------------------------------------------------------------
+extern "C" wslda_status wslda_profile(wslda_ctx* c, int enable) {
+  if (!c) return WSLDA_EINVAL;
+  if (enable) { c->prof_n = 0; c->prof_name->clear(); c->prof_work->clear(); }
+  c->prof_on = enable ? 1 : 0;
+  return WSLDA_OK;
+}
+extern "C" int wslda_profile_report(wslda_ctx* c, char* buf, size_t buf_bytes) {
+  if (!c || !buf || !buf_bytes) return -1;
+  cudaDeviceSynchronize();
+  std::vector<const char*> names; std::vector<double> ms, by, fl; std::vector<long> cnt;
+  for (int i = 0; i < c->prof_n; ++i) {
+    float t = 0.f;
+    cudaEventElapsedTime(&t, (*c->prof_ev)[2 * i], (*c->prof_ev)[2 * i + 1]);
+    size_t k = 0;
+    while (k < names.size() && strcmp(names[k], (*c->prof_name)[i])) ++k;
+    if (k == names.size()) { names.push_back((*c->prof_name)[i]); ms.push_back(0.0); by.push_back(0.0); fl.push_back(0.0); cnt.push_back(0); }
+    ms[k] += t; cnt[k]++; by[k] += (*c->prof_work)[2 * i]; fl[k] += (*c->prof_work)[2 * i + 1];
+  }
+  size_t o = 0; buf[0] = 0;
+  for (size_t k = 0; k < names.size(); ++k) {
+    int w = snprintf(buf + o, buf_bytes - o, "%s %ld %.6f %.6e %.6e\n", names[k], cnt[k], ms[k], by[k], fl[k]);
+    if (w < 0 || (size_t)w >= buf_bytes - o) break;
+    o += w;
+  }
+  return (int)names.size();
+}
+
 extern "C" wslda_status wslda_ctx_destroy(wslda_ctx* c) {
   if (!c) return WSLDA_EINVAL;
+  for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e);
+  delete c->prof_ev; delete c->prof_name; delete c->prof_work;
   free(c);
   return WSLDA_OK;
 }

@@ -50,18 +50,26 @@ extern "C" wslda_status wslda_set_external(wslda_ctx* c, const double* va, const
 static void deriv(wslda_ctx* c, const DerivArgs& a, cudaStream_t st) {
   const Plan& P = c->P;
   const int64_t M = P.M;
+  int n_out = 0;
+  for (int o = 0; o < 4; ++o) n_out += a.out[o] != nullptr;
+  const double lgM = (double)(P.lg[0] + P.lg[1] + P.lg[2]);
+  const double fl_fwd = 5.0 * M * lgM * a.ncomp, fl_x = 5.0 * M * P.lg[0] * a.ncomp, by_in = 16.0 * M * a.ncomp;
   if (P.onchip) {
     const size_t smem = (size_t)2 * P.G * M * 16;
+    WORK(c, by_in, fl_fwd * (1 + n_out));
     LAUNCH(c, k_deriv_onchip, nb(a.ncomp, P.G), 256, smem, st, c->L, a, P.G);
     return;
   }
   const int64_t R = M / P.N[0];
   cplx* spec = c->scr[3];
+  WORK(c, by_in, fl_fwd - fl_x);
   LAUNCH(c, k_planes_fwd, dim3(P.N[0] / P.PX, a.ncomp), 256, (size_t)P.PX * R * 16, st, c->L, a, spec, P.PX);
+  WORK(c, 0, fl_x * (1 + n_out));
   LAUNCH(c, k_xlines, dim3((unsigned)(R >> P.lgT), a.ncomp), 256, (size_t)2 * P.N[0] * 16 << P.lgT, st, c->L, spec, a, P.lgT);
   OutList ol; int no = 0;
   for (int o = 0; o < 4; ++o) if (a.out[o]) ol.p[no++] = a.out[o];
   for (int o = no; o < 4; ++o) ol.p[o] = nullptr;
+  WORK(c, 0, (fl_fwd - fl_x) * n_out);
   LAUNCH(c, k_planes_inv, dim3(P.N[0] / P.PX, a.ncomp, no), 256, (size_t)P.PX * R * 16, st, c->L, ol, P.PX);
 }
 
@@ -166,6 +174,7 @@ static void h_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_chu
       deriv(c, b, st);
     }
   }
+  WORK(c, 64.0 * M * cnt, 0);      // reads psi, writes H psi
   LAUNCH(c, k_hmix, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, psi_chunk, scale_chunk, c->kperp2 + n0, kin, P.nd,
          c->scr[0], c->scr[1], c->scr[2], fields_of(c), M, out, want_eps ? c->part_e : nullptr, P.nblk);
 }
@@ -204,6 +213,7 @@ static void dens_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_
   G = (cnt + per - 1) / per;
   d.psi = psi_chunk; d.scale = scale_chunk; d.cpref = c->cpref + n0; d.kperp2 = c->kperp2 + n0;
   d.w_a = c->w_a + n0; d.w_b = c->w_b + n0; d.nd = P.nd; d.M = M; d.n_count = cnt; d.per_group = per; d.mask = mask;
+  WORK(c, 32.0 * M * cnt, 0);
   LAUNCH(c, k_density, dim3(P.nblk, (unsigned)G), P.pt_threads, 0, st, d, c->dpart);
   LAUNCH(c, k_density_reduce, dim3(nb(M, 256), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
 }

@@ -49,6 +49,7 @@ static void rhs_chunk(wslda_ctx* c, cplx* psi_chunk, const double* scale_chunk, 
   const Plan& P = c->P;
   h_chunk(c, psi_chunk, scale_chunk, n0, cnt, c->scr[4], c->f.subtract_mean_energy != 0, st);
   const double* eps = eps_chunk(c, n0, cnt, st);
+  WORK(c, 64.0 * P.M * cnt, 0);    // reads psi (H psi is scratch), writes f
   LAUNCH(c, k_rhs, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, psi_chunk, scale_chunk, c->scr[4], eps, 0, write_back,
          f_chunk, (const cplx*)nullptr, 0.0, P.M, (double*)nullptr, P.nblk);
 }
@@ -138,6 +139,7 @@ static void stage1(wslda_ctx* c, const StepBufs& b, int64_t n0, int64_t cnt, cud
   const int64_t off = 2 * n0 * P.M;
   HistPtrs h = b.h;
   for (int j = 0; j < 5; ++j) if (h.f[j]) h.f[j] += off;
+  WORK(c, 32.0 * P.M * cnt * (1 + c->m + 2), 0);   // reads phi, f_1..f_m; writes P, C_part
   LAUNCH(c, k_abm_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, b.phi + off, h, b.cpart + off, b.k, P.M,
          c->f.normalize ? c->part_n : (double*)nullptr, P.nblk);
   if (c->f.normalize) scale_chunk_from_partials(c, n0, cnt, st);
@@ -149,6 +151,7 @@ static void stage2(wslda_ctx* c, const StepBufs& b, int64_t n0, int64_t cnt, cud
   const double* sc = c->f.normalize ? c->scale + n0 : nullptr;
   h_chunk(c, b.phi + off, sc, n0, cnt, c->scr[4], c->f.subtract_mean_energy != 0, st);
   const double* eps = eps_chunk(c, n0, cnt, st);
+  WORK(c, 96.0 * P.M * cnt, 0);    // reads P, C_part; writes phi_new
   LAUNCH(c, k_rhs, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, b.phi + off, sc, c->scr[4], eps, 1, 0, (cplx*)nullptr,
          b.cpart + off, b.c0dt, P.M, c->f.normalize ? c->part_n : (double*)nullptr, P.nblk);
   if (c->f.normalize) scale_chunk_from_partials(c, n0, cnt, st);

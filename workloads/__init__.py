@@ -144,6 +144,45 @@ class Workload:
         return out
 
 
+def spinors_device(w: "Workload", n0: int, n1: int, out):
+    """Fill the torch CUDA tensor `out` ([n1-n0, 2, *shape] complex128) with spinors n0..n1-1 of the recipe of
+    Workload.spinors, generated on the device (bench-sized batches; the noise comes from torch's seeded
+    generator instead of SplitMix64, so the bits differ from the numpy path but the distribution is the same)."""
+    import torch
+    dev = out.device
+    shape, nd = w.shape, w.mode
+    vol = w.M * w.dV
+    g = torch.Generator(device=dev)
+    step = max(1, (1 << 24) // w.M)
+    for a in range(n0, n1, step):
+        b = min(n1, a + step)
+        kidx = np.asarray(w.kidx[a:b])
+        kk = [kgrid(shape[d], w.dx[d])[kidx[:, d]] for d in range(nd)]
+        kp2 = np.zeros(b - a) if w.kperp is None else np.sum(np.asarray(w.kperp)[w.mode_of[a:b]] ** 2, axis=1)
+        eps = w.alpha0 * (sum(k * k for k in kk) + kp2) / 2.0 - w.mu_eff
+        En = np.sqrt(eps * eps + w.delta0 ** 2)
+        u, v = np.sqrt(0.5 * (1 + eps / En)), np.sqrt(0.5 * (1 - eps / En))
+        neg = np.asarray(w.branch[a:b]) < 0
+        u, v = np.where(neg, -v, u), np.where(neg, u, v)
+        phase = torch.zeros((b - a,) + shape, dtype=torch.float64, device=dev)
+        for d in range(nd):
+            pos = torch.arange(shape[d], dtype=torch.float64, device=dev) * w.dx[d]
+            view = [1] * (nd + 1); view[d + 1] = shape[d]
+            kd = torch.as_tensor(kk[d], device=dev).view([-1] + [1] * nd)
+            phase = phase + kd * pos.view(view)
+        pw = torch.polar(torch.full_like(phase, 1.0 / np.sqrt(vol)), phase)
+        o = out[a - n0:b - n0]
+        o[:, 0] = torch.as_tensor(u, device=dev).view([-1] + [1] * nd) * pw
+        o[:, 1] = torch.as_tensor(v, device=dev).view([-1] + [1] * nd) * pw
+        if w.noise > 0:
+            g.manual_seed(w.noise_seed * 1000003 + a)
+            z = torch.randn((b - a, 2) + shape + (2,), dtype=torch.float64, device=dev, generator=g)
+            o += (w.noise / np.sqrt(vol)) * torch.view_as_complex(z)
+            nrm = torch.sqrt(torch.sum(o.real ** 2 + o.imag ** 2, dim=tuple(range(1, nd + 2)), keepdim=True) * w.dV)
+            o /= nrm
+    return out
+
+
 def _coords_centered(shape, dx):
     ax = [dx[d] * (np.arange(shape[d]) - shape[d] // 2) for d in range(len(shape))]   # PAPER.md:1529
     return np.meshgrid(*ax, indexing="ij")
