@@ -7,6 +7,7 @@
 #include <vector>
 #include "density.cuh"
 #include "fft_large.cuh"
+#include "fast3d.cuh"
 #include "kernels.cuh"
 
 struct Plan {
@@ -17,6 +18,9 @@ struct Plan {
   int PX, lgT;                  // large regime: x-planes per CTA, log2 of the x-line tile width
   int dG;                       // max density groups per chunk
   int nscr;
+  // fused 3-D path (fast3d.cuh): enabled flag, spinors per chunk, concurrent streams, per-stream scratch
+  int fast, fc, ns;
+  size_t off_fast, fast_spec_bytes, fast_part_bytes, fast_stream_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -64,13 +68,28 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.dG = (int)dg;
   P.nscr = 7;
   size_t o = 0;
-  P.off_tables = o; for (int d = 0; d < 3; ++d) o += align_up((size_t)P.N[d] * 32);       // tw (16) + kk (8) + ko (8)
-  P.off_perwf = o; o += 6 * align_up((size_t)n_wf * 8);
+  P.off_tables = o; for (int d = 0; d < 3; ++d) o += align_up((size_t)P.N[d] * 40);       // tw (16) + kk (8) + ko (8) + k^2 natural (8)
+  P.off_perwf = o; o += 7 * align_up((size_t)n_wf * 8);
   P.off_fields = o; o += align_up((size_t)DP_COUNT * M * 8) + 12 * align_up((size_t)M * 8) + 2 * align_up((size_t)M * 16);
   P.off_part = o; o += 2 * align_up((size_t)cn * P.nblk * 8);
   P.off_dpart = o; o += align_up((size_t)P.dG * DP_COUNT * M * 8);
   P.scr_bytes = align_up((size_t)cn * 2 * M * 16);
   P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
+  // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
+  P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
+           f->kin_form != WSLDA_KIN_DIVGRAD;
+  if (const char* e = getenv("WSLDA_FAST")) if (atoi(e) == 0) P.fast = 0;
+  P.fc = 16; P.ns = 3;
+  if (const char* e = getenv("WSLDA_FAST_CHUNK")) { int v = atoi(e); if (v > 0) P.fc = v; }
+  if (const char* e = getenv("WSLDA_FAST_STREAMS")) { int v = atoi(e); if (v > 0 && v <= 4) P.ns = v; }
+  if (P.fc > n_wf) P.fc = (int)n_wf;
+  P.off_fast = o; P.fast_spec_bytes = P.fast_part_bytes = P.fast_stream_bytes = 0;
+  if (P.fast) {
+    P.fast_spec_bytes = align_up((size_t)P.fc * 2 * M * 16);
+    P.fast_part_bytes = align_up((size_t)F3_NPART * P.fc * P.N[0] * 8) + align_up((size_t)P.fc * P.nblk * 8);
+    P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
+    o += (size_t)P.ns * P.fast_stream_bytes;
+  }
   P.total = o;
   return 0;
 }
@@ -83,7 +102,13 @@ struct wslda_ctx {
   int m;
   double mu_a, mu_b;
   int lambda_valid;
-  double *kperp2, *cpref, *w_a, *w_b, *scale, *eps;
+  double *kperp2, *cpref, *w_a, *w_b, *scale, *eps, *scale2;
+  double* k2n[3];                  // k_d^2 in natural index order
+  double hk2[3][64];               // host copy (kernel parameters)
+  cudaStream_t aux[4];             // fused path: concurrent chunk streams (created by the library)
+  cudaEvent_t ev_fork, ev_join[4];
+  cplx *f_spec0[4], *f_spec1[4], *f_X[4];
+  double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
   cplx *delta, *dext;
@@ -123,9 +148,10 @@ static inline bool prof_begin(wslda_ctx* c, const char* name, cudaStream_t st) {
   return true;
 }
 static inline void prof_end(wslda_ctx* c, cudaStream_t st) { cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], st); c->prof_n++; }
-#define LAUNCH(c, kern, grid, block, smem, st, ...)                                   \
-  do { bool pr_ = prof_begin(c, #kern, st); kern<<<grid, block, smem, st>>>(__VA_ARGS__); \
+#define LAUNCHN(c, name, kern, grid, block, smem, st, ...)                             \
+  do { bool pr_ = prof_begin(c, name, st); kern<<<grid, block, smem, st>>>(__VA_ARGS__); \
        if (pr_) prof_end(c, st); (c)->launches++; (c)->work_bytes = 0; (c)->work_flops = 0; } while (0)
+#define LAUNCH(c, kern, grid, block, smem, st, ...) LAUNCHN(c, #kern, kern, grid, block, smem, st, __VA_ARGS__)
 // algorithmic work of the NEXT launch (compulsory HBM bytes: unique full-buffer inputs + outputs; FFT flops as
 // 5 N log2 N per line transform) -- only used by the profile report
 #define WORK(c, bytes, flops) do { (c)->work_bytes = (double)(bytes); (c)->work_flops = (double)(flops); } while (0)
@@ -180,7 +206,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   for (int d = 0; d < 3; ++d) {
     const int n = P.N[d];
     L.N[d] = n; L.lg[d] = P.lg[d];
-    std::vector<double> tw(2 * n), kk(n), ko(n);
+    std::vector<double> tw(2 * n), kk(n), ko(n), k2(n);
     std::vector<int> fr;
     scrambled_freq(n, fr);
     const double len = n * dx[d];
@@ -190,17 +216,23 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       double k = (l < n / 2) ? 2.0 * PI * l / len : 2.0 * PI * (l - n) / len;      // Eq. 25
       if (n == 1) k = 0.0;
       kk[j] = k; ko[j] = (n > 1 && l == n / 2) ? 0.0 : k;
+      double kn = (j < n / 2) ? 2.0 * PI * j / len : 2.0 * PI * (j - n) / len;       // natural order, Nyquist kept
+      if (n == 1) kn = 0.0;
+      k2[j] = kn * kn;
+      if (j < 64) c->hk2[d][j] = k2[j];
     }
     cplx* dtw = (cplx*)(base + o); double* dkk = (double*)(base + o + (size_t)n * 16); double* dko = dkk + n;
     cudaMemcpy(dtw, tw.data(), (size_t)n * 16, cudaMemcpyHostToDevice);
     cudaMemcpy(dkk, kk.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
     cudaMemcpy(dko, ko.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(dko + n, k2.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
+    c->k2n[d] = dko + n;
     L.tw[d] = dtw; L.kk[d] = dkk; L.ko[d] = dko;
-    o += align_up((size_t)n * 32);
+    o += align_up((size_t)n * 40);
   }
   o = P.off_perwf;
-  double** pw[6] = {&c->kperp2, &c->cpref, &c->w_a, &c->w_b, &c->scale, &c->eps};
-  for (int q = 0; q < 6; ++q) { *pw[q] = (double*)(base + o); o += align_up((size_t)n_wf * 8); }
+  double** pw[7] = {&c->kperp2, &c->cpref, &c->w_a, &c->w_b, &c->scale, &c->eps, &c->scale2};
+  for (int q = 0; q < 7; ++q) { *pw[q] = (double*)(base + o); o += align_up((size_t)n_wf * 8); }
   o = P.off_fields;
   c->raw = (double*)(base + o); o += align_up((size_t)DP_COUNT * M * 8);
   double** pf[12] = {&c->alpha_a, &c->alpha_b, &c->V_a, &c->V_b, &c->U_a, &c->U_b, &c->lap_a, &c->lap_b,
@@ -212,6 +244,23 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   c->part_e = (double*)(base + P.off_part + align_up((size_t)P.chunk_n * P.nblk * 8));
   c->dpart = (double*)(base + P.off_dpart);
   for (int q = 0; q < P.nscr; ++q) c->scr[q] = (cplx*)(base + P.off_scr + (size_t)q * P.scr_bytes);
+  if (P.fast) {
+    for (int q = 0; q < P.ns; ++q) {
+      char* b = base + P.off_fast + (size_t)q * P.fast_stream_bytes;
+      c->f_spec0[q] = (cplx*)b; c->f_spec1[q] = (cplx*)(b + P.fast_spec_bytes); c->f_X[q] = (cplx*)(b + 2 * P.fast_spec_bytes);
+      b += 3 * P.fast_spec_bytes;
+      c->f_part[q] = (double*)b; c->f_partn[q] = (double*)(b + align_up((size_t)F3_NPART * P.fc * P.N[0] * 8));
+      c->f_acc[q] = (double*)(b + P.fast_part_bytes);
+      if (q > 0 || P.ns > 1) cudaStreamCreateWithFlags(&c->aux[q], cudaStreamNonBlocking);
+      cudaEventCreateWithFlags(&c->ev_join[q], cudaEventDisableTiming);
+    }
+    cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+    cudaFuncSetAttribute(k_f3_pass_a<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+    cudaFuncSetAttribute(k_f3_pass_a<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+    cudaFuncSetAttribute(k_f3_pass_c<true, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
+    cudaFuncSetAttribute(k_f3_pass_c<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
+    cudaFuncSetAttribute(k_f3_pass_c<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
+  }
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
   cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);
   const int T = 256;
@@ -266,6 +315,10 @@ extern "C" int wslda_profile_report(wslda_ctx* c, char* buf, size_t buf_bytes) {
 
 extern "C" wslda_status wslda_ctx_destroy(wslda_ctx* c) {
   if (!c) return WSLDA_EINVAL;
+  if (c->P.fast) {
+    for (int q = 0; q < c->P.ns; ++q) { if (c->aux[q]) cudaStreamDestroy(c->aux[q]); cudaEventDestroy(c->ev_join[q]); }
+    cudaEventDestroy(c->ev_fork);
+  }
   for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e);
   delete c->prof_ev; delete c->prof_name; delete c->prof_work;
   free(c);

@@ -1,0 +1,183 @@
+// fast_step.cuh -- host side of the fused 3-D path (fast3d.cuh): H psi in three passes per chunk, and the
+// Alg. 2 step as chunk pipelines on up to four concurrent streams so that the passes of
+// different chunks overlap (HBM-bound, L2-bound and FP64-bound phases run side by side on the SMs).
+#pragma once
+#include "ops.cuh"
+
+static F3Fields f3_fields(const wslda_ctx* c) {
+  F3Fields F;
+  F.alpha[0] = c->alpha_a; F.alpha[1] = c->alpha_b; F.lap[0] = c->lap_a; F.lap[1] = c->lap_b;
+  F.U[0] = c->U_a; F.U[1] = c->U_b; F.delta = c->delta; F.dext = c->dext; F.mu[0] = c->mu_a; F.mu[1] = c->mu_b;
+  return F;
+}
+
+// out = APPLY: H psi | CORR: C_part - i kappa H psi | RHS: -i H psi  for the cnt spinors of a chunk (psi_chunk,
+// scale_chunk, out, cpart already offset to the chunk; n0 = global index of its first spinor); pass-C partial
+// sums go to f_part[q].  q = scratch slot, st = the stream that owns it.
+static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk, const double* scale_chunk, int64_t n0,
+                    int cnt, int mode, cplx* out, const cplx* cpart, double kappa) {
+  const Plan& P = c->P;
+  const int NX = P.N[0];
+  const int64_t M = P.M;
+  const bool sym = c->f.kin_form == WSLDA_KIN_SYM40;
+  const int nspec = sym ? 2 : 1;
+  const double fl_plane = 5.0 * M * 10.0 * 2 * cnt * nspec, fl_x = 5.0 * M * P.lg[0] * 2.0 * 2 * cnt * nspec;
+  F3PassA a;
+  a.psi = psi_chunk; a.scale = scale_chunk; a.alpha[0] = c->alpha_a; a.alpha[1] = c->alpha_b;
+  a.spec0 = c->f_spec0[q]; a.spec1 = c->f_spec1[q]; a.n_items = cnt * 2 * NX; a.NX = NX;
+  WORK(c, 32.0 * M * cnt, fl_plane);                       // reads psi once
+  auto ka = sym ? k_f3_pass_a<true> : k_f3_pass_a<false>;
+  LAUNCHN(c, "k_f3_pass_a", ka, (a.n_items + 3) / 4, 128, 4 * F3_TILE_BYTES, st, a);
+  F3PassB b;
+  b.spec[0] = c->f_spec0[q]; b.spec[1] = c->f_spec1[q]; b.n_spec = nspec; b.n_items = cnt * 2 * F3_N;
+  b.ky2 = c->k2n[1]; b.kz2 = c->k2n[2]; b.invM = c->L.invM;
+  for (int j = 0; j < 32; ++j) b.kx2[j] = j < NX ? c->hk2[0][j] : 0.0;
+  WORK(c, 0, fl_x);
+  auto kb = NX == 32 ? k_f3_pass_b<32> : NX == 16 ? k_f3_pass_b<16> : k_f3_pass_b<8>;
+  LAUNCHN(c, "k_f3_pass_b", kb, (b.n_items + 3) / 4, 128, 0, st, b);
+  F3PassC k;
+  k.spec0 = c->f_spec0[q]; k.spec1 = c->f_spec1[q]; k.psi = psi_chunk; k.scale = scale_chunk; k.kperp2 = c->kperp2 + n0;
+  k.F = f3_fields(c); k.out = out; k.cpart = cpart; k.kappa = kappa; k.part = c->f_part[q]; k.n_items = cnt * NX; k.NX = NX;
+  const int grid = (k.n_items + 1) / 2;
+  const size_t sm_sym = 2 * (F3_TILE_BYTES + F3_PLANE * 16), sm_lap = 2 * F3_TILE_BYTES;
+  WORK(c, mode == F3_CORR ? 32.0 * M * cnt : (mode == F3_APPLY ? 32.0 * M * cnt : 0.0), fl_plane);
+  void (*kc)(F3PassC);
+  if (sym) kc = mode == F3_APPLY ? k_f3_pass_c<true, F3_APPLY> : mode == F3_CORR ? k_f3_pass_c<true, F3_CORR> : k_f3_pass_c<true, F3_RHS>;
+  else kc = mode == F3_APPLY ? k_f3_pass_c<false, F3_APPLY> : mode == F3_CORR ? k_f3_pass_c<false, F3_CORR> : k_f3_pass_c<false, F3_RHS>;
+  LAUNCHN(c, "k_f3_pass_c", kc, grid, 64, sym ? sm_sym : sm_lap, st, k);
+}
+
+static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, int mode, int use_shift, double kappa,
+                    double* eps_user) {
+  F3Scal s;
+  s.part = c->f_part[q]; s.cnt = cnt; s.NX = c->P.N[0]; s.mode = mode; s.use_shift = use_shift; s.normalize = c->f.normalize;
+  s.dV = c->dV; s.kappa = kappa; s.eps = c->eps + n0; s.eps_user = eps_user; s.scale_new = c->scale2 + n0;
+  LAUNCH(c, k_f3_scal, (cnt + 3) / 4, 128, 0, st, s);
+}
+
+static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
+                               cudaStream_t st) {
+  const int64_t M = c->P.M;
+  for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.fc) {
+    const int cnt = (int)((n_first + n_count - n0 < c->P.fc) ? n_first + n_count - n0 : c->P.fc);
+    f3_hpsi(c, 0, st, psi + 2 * n0 * M, nullptr, n0, cnt, F3_APPLY, hpsi + 2 * n0 * M, nullptr, 0.0);
+    f3_scal(c, 0, st, n0, cnt, F3_APPLY, 1, 0.0, eps_dev ? eps_dev + n0 : nullptr);
+  }
+  return cuda_check(c, "apply_h");
+}
+
+// ---- the Alg. 2 step -----------------------------------------------------------------------------------------
+struct F3Step {
+  cplx* phi; HistPtrs h; cplx* cpart; AbmCoef k; double c0dt;
+  cudaStream_t user;
+};
+
+static inline cudaStream_t f3_stream(wslda_ctx* c, const F3Step& s, int q) { return c->P.ns > 1 ? c->aux[q] : s.user; }
+static void f3_fork(wslda_ctx* c, const F3Step& s) {
+  if (c->P.ns == 1) return;
+  cudaEventRecord(c->ev_fork, s.user);
+  for (int q = 0; q < c->P.ns; ++q) cudaStreamWaitEvent(c->aux[q], c->ev_fork, 0);
+}
+static void f3_join(wslda_ctx* c, const F3Step& s) {
+  if (c->P.ns == 1) return;
+  for (int q = 0; q < c->P.ns; ++q) { cudaEventRecord(c->ev_join[q], c->aux[q]); cudaStreamWaitEvent(s.user, c->ev_join[q], 0); }
+}
+
+static F3Dens f3_dens_args(wslda_ctx* c, int q, int64_t n0, int first) {
+  F3Dens d; d.cpref = c->cpref + n0; d.w_a = c->w_a + n0; d.w_b = c->w_b + n0; d.acc = c->f_acc[q]; d.first = first;
+  return d;
+}
+
+// Alg. 2 step 1-2: predictor P -> phi buffer, C_part -> oldest history buffer, scale_n = 1/|P|
+static void f3_stage1(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int64_t n0, int cnt) {
+  const Plan& P = c->P;
+  const int64_t off = 2 * n0 * P.M;
+  HistPtrs h = s.h;
+  for (int j = 0; j < 5; ++j) if (h.f[j]) h.f[j] += off;
+  WORK(c, 32.0 * P.M * cnt * (1 + c->m + 2), 0);
+  LAUNCH(c, k_abm_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, s.phi + off, h, s.cpart + off, s.k, P.M,
+         c->f.normalize ? c->f_partn[q] : (double*)nullptr, P.nblk);
+  if (c->f.normalize)
+    LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->f_partn[q], P.nblk, (int64_t)cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
+}
+// Alg. 2 steps 3-4, 8: phi_new = C_part + c0 dt f(P), normalised, written over P (+ its densities)
+static void f3_stage2(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int64_t n0, int cnt, int do_dens, int first) {
+  const Plan& P = c->P;
+  const int64_t off = 2 * n0 * P.M;
+  const double* sc = c->f.normalize ? c->scale + n0 : nullptr;
+  f3_hpsi(c, q, st, s.phi + off, sc, n0, cnt, F3_CORR, c->f_X[q], s.cpart + off, s.c0dt);
+  f3_scal(c, q, st, n0, cnt, F3_CORR, c->f.subtract_mean_energy, s.c0dt, nullptr);
+  F3Fin2 f;
+  f.X = c->f_X[q]; f.phi = s.phi + off; f.scaleP = sc; f.eps = c->eps + n0; f.scale_new = c->scale2 + n0; f.kappa = s.c0dt;
+  f.cnt = cnt; f.M = P.M; f.do_dens = do_dens; f.d = f3_dens_args(c, q, n0, first);
+  WORK(c, 32.0 * P.M * cnt, 0);                            // writes phi_new
+  LAUNCH(c, k_f3_fin2, nb(P.M, 128), 128, 0, st, f);
+}
+// Alg. 2 step 9: f(phi_new) -> the recycled oldest history buffer
+static void f3_stage3(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int64_t n0, int cnt) {
+  const Plan& P = c->P;
+  const int64_t off = 2 * n0 * P.M;
+  f3_hpsi(c, q, st, s.phi + off, nullptr, n0, cnt, F3_RHS, c->f_X[q], nullptr, 0.0);
+  f3_scal(c, q, st, n0, cnt, F3_RHS, c->f.subtract_mean_energy, 0.0, nullptr);
+  WORK(c, 32.0 * P.M * cnt, 0);                            // writes f_new
+  LAUNCH(c, k_f3_fin3, dim3(nb(2 * P.M, 256), (unsigned)cnt), 256, 0, st, c->f_X[q], s.phi + off, c->eps + n0, s.cpart + off, 2 * P.M);
+}
+
+static void potentials(wslda_ctx* c, cudaStream_t st);
+static unsigned step_mask(const wslda_ctx* c);
+
+static void f3_dens_final(wslda_ctx* c, int used, cudaStream_t st) {
+  const int64_t M = c->P.M;
+  LAUNCH(c, k_f3_dens_final, nb(4 * M, 256), 256, 0, st, c->f_acc[0], used, (int64_t)(c->P.fast_stream_bytes / 8), M, c->raw);
+}
+
+static bool f3_step_ok(const wslda_ctx* c) {
+  return c->P.fast && (c->f.func_id == WSLDA_FUNC_FIXED || step_mask(c) == (WSLDA_D_RHO | WSLDA_D_NU));
+}
+
+static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
+  const Plan& P = c->P;
+  const int64_t n_wf = P.n_wf;
+  const int fc = P.fc, ns = P.ns;
+  const int64_t n_chunks = (n_wf + fc - 1) / fc;
+  const int used = (int)(n_chunks < ns ? n_chunks : ns);
+  auto cnt_of = [&](int64_t k) { return (int)((n_wf - k * fc < fc) ? n_wf - k * fc : fc); };
+  const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
+  f3_fork(c, s);
+  if (fixed) {
+    for (int64_t k = 0; k < n_chunks; ++k) {
+      const int q = (int)(k % ns); cudaStream_t st = f3_stream(c, s, q);
+      f3_stage1(c, s, q, st, k * fc, cnt_of(k));
+      f3_stage2(c, s, q, st, k * fc, cnt_of(k), 0, 0);
+      f3_stage3(c, s, q, st, k * fc, cnt_of(k));
+    }
+    f3_join(c, s);
+    return;
+  }
+  for (int64_t k = 0; k < n_chunks; ++k) {
+    const int q = (int)(k % ns); cudaStream_t st = f3_stream(c, s, q);
+    const int64_t n0 = k * fc; const int cnt = cnt_of(k);
+    f3_stage1(c, s, q, st, n0, cnt);
+    F3DensOnly d;
+    d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
+    d.d = f3_dens_args(c, q, n0, k < ns);
+    LAUNCH(c, k_f3_dens, nb(P.M, 128), 128, 0, st, d);
+  }
+  f3_join(c, s);
+  f3_dens_final(c, used, s.user);
+  potentials(c, s.user);
+  f3_fork(c, s);
+  for (int64_t k = 0; k < n_chunks; ++k) {
+    const int q = (int)(k % ns);
+    f3_stage2(c, s, q, f3_stream(c, s, q), k * fc, cnt_of(k), 1, k < ns);
+  }
+  f3_join(c, s);
+  f3_dens_final(c, used, s.user);
+  potentials(c, s.user);
+  f3_fork(c, s);
+  for (int64_t k = 0; k < n_chunks; ++k) {
+    const int q = (int)(k % ns);
+    f3_stage3(c, s, q, f3_stream(c, s, q), k * fc, cnt_of(k));
+  }
+  f3_join(c, s);
+}

@@ -139,6 +139,9 @@ extern "C" wslda_status wslda_set_field(wslda_ctx* c, int id, const void* src, v
   return cuda_check(c, "set_field");
 }
 
+static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
+                               cudaStream_t st);
+
 static Fields fields_of(const wslda_ctx* c) {
   Fields F;
   F.alpha_a = c->alpha_a; F.alpha_b = c->alpha_b; F.lap_a = c->lap_a; F.lap_b = c->lap_b; F.U_a = c->U_a; F.U_b = c->U_b;
@@ -186,6 +189,7 @@ extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi
   const cplx* psi = (const cplx*)psi_; cplx* hpsi = (cplx*)hpsi_;
   const int64_t M = c->P.M;
   cudaStream_t st = S(stream);
+  if (c->P.fast) return f3_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
     const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
     h_chunk(c, psi + 2 * n0 * M, nullptr, n0, cnt, hpsi + 2 * n0 * M, true, st);

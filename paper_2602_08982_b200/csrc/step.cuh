@@ -2,7 +2,7 @@
 // Adams-Bashforth-Moulton predictor-corrector following Alg. 2.  General chunked path:
 // spinors are processed in chunks whose intermediates (spectral terms, H psi) stay in L2-sized scratch.
 #pragma once
-#include "ops.cuh"
+#include "fast_step.cuh"
 
 // Eqs. 46-50
 static const double AB3[5] = {23.0 / 12, -16.0 / 12, 5.0 / 12, 0, 0};
@@ -180,7 +180,10 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
   b.c0dt = C[0] * dt;
   const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
   const unsigned mask = step_mask(c);
-  if (fixed) {                                           // no global barrier: run the three stages chunk by chunk
+  if (f3_step_ok(c)) {                                   // fused 3-D path (fast_step.cuh)
+    F3Step s; s.phi = b.phi; s.h = b.h; s.cpart = b.cpart; s.k = b.k; s.c0dt = b.c0dt; s.user = st;
+    f3_abm_step(c, s);
+  } else if (fixed) {                                    // no global barrier: run the three stages chunk by chunk
     for (int64_t n0 = 0; n0 < n_wf; n0 += P.chunk_n) {
       const int64_t cnt = chunk_len(c, n0);
       stage1(c, b, n0, cnt, st); stage2(c, b, n0, cnt, st); stage3(c, b, n0, cnt, st);

@@ -52,7 +52,9 @@ def spinors(w, seed=9):
 
 SHAPES = [((8, 4, 8), (1.0, 0.9, 1.1)), ((16, 8), (1.0, 1.2)), ((32,), (0.8,)), ((2, 2, 4), (1.0, 1.0, 1.0)),
           ((32, 16, 16), (1.0, 1.0, 0.9)),      # 8192 points: the multi-pass (large lattice) regime
-          ((128, 64), (1.0, 1.1))]              # 2-D lattice in the large regime
+          ((128, 64), (1.0, 1.1)),              # 2-D lattice in the large regime
+          ((8, 32, 32), (1.0, 1.1, 0.9)),       # Ny = Nz = 32: the fused register-FFT path (fast3d.cuh)
+          ((16, 32, 32), (0.9, 1.0, 1.0))]
 
 
 @pytest.mark.parametrize("kin_form", [0, 1, 2])
@@ -188,3 +190,55 @@ def test_run_to_run_bit_reproducible():
     a = run_both(w, psi0, 5)[0]
     b = run_both(w, psi0, 5)[0]
     assert np.array_equal(a, b)
+
+
+# ---- the fused 3-D path (Ny = Nz = 32): ragged chunks over several concurrent streams ---------------------------
+@pytest.fixture
+def small_fast_chunks(monkeypatch):
+    monkeypatch.setenv("WSLDA_FAST_CHUNK", "3")
+    monkeypatch.setenv("WSLDA_FAST_STREAMS", "3")
+
+
+@pytest.mark.parametrize("kin_form", [0, 1])
+@pytest.mark.parametrize("nx", [8, 32])
+def test_fast3d_apply_h_ragged_chunks(small_fast_chunks, nx, kin_form):
+    w = generic((nx, 32, 32), (1.0, 0.95, 1.05), 11, kin_form, n_modes=2)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi)
+    h, e = g.apply_h(to_gpu(psi))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    assert any(k.startswith("k_f3") for k in _kernels_of(g, lambda: g.apply_h(to_gpu(psi))))
+
+
+def _kernels_of(g, fn):
+    g.profile(True)
+    fn()
+    rep = g.profile_report()
+    g.profile(False)
+    return list(rep)
+
+
+@pytest.mark.parametrize("case", ["fixed_sym40", "fixed_laplace_noshift", "bdg", "slda_trap_32", "fixed_ab5am5_nonorm"])
+def test_fast3d_abm_matches_oracle(small_fast_chunks, case):
+    if case == "fixed_sym40":
+        w = generic((8, 32, 32), (1.0, 1.0, 1.1), 10, 1, dt=0.004); n = 8
+    elif case == "fixed_laplace_noshift":
+        w = generic((16, 32, 32), (1.0, 1.0, 1.0), 7, 0, dt=0.004, subtract_mean_energy=0); n = 6
+    elif case == "fixed_ab5am5_nonorm":
+        w = generic((8, 32, 32), (1.0, 1.0, 1.0), 8, 1, dt=0.004, ab_order=5, am_order=5, normalize=0); n = 6
+    elif case == "bdg":
+        w = generic((8, 32, 32), (1.0, 1.0, 1.0), 20, 0, func_id=1, four_pi_as=-2.0, dt=0.005); n = 6
+    else:
+        w = wl.cfg4(n_side=32, n_wf=20, kin_form=1, n_steps=5); n = 5      # configs[3] recipe, full lattice, 20 spinors
+    psi0 = w.spinors() if w.kidx is not None else spinors(w)
+    pg, po, fg, fo, o, g = run_both(w, psi0, n)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    if w.func_id:
+        for f in ("delta", "U_a", "rho_a", "nu"):
+            assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    assert any(k.startswith("k_f3") for k in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt)))
