@@ -39,38 +39,48 @@ struct F3PassA {
   int NX;
 };
 
+// forward 2-D transform of the plane held one line per lane (x[j] = (j, lane)): FFT along j, transpose through
+// the padded tile, FFT along the other axis; returns x[j] = (k_other = j, k_first = lane).  The loop is NOT
+// unrolled so that the 32-point butterfly code exists once (instruction-cache footprint).
+__device__ __forceinline__ void f3_plane_forward(cplx* x, cplx* S, int lane) {
+#pragma unroll 1
+  for (int pass = 0; pass < 2; ++pass) {
+    fft_reg<F3_N, false>(x);
+    if (pass == 0) {
+#pragma unroll
+      for (int j = 0; j < F3_N; ++j) S[j * F3_PITCH + lane] = x[j];
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < F3_N; ++j) x[j] = S[lane * F3_PITCH + j];
+      __syncwarp();
+    }
+  }
+}
+
 template <bool SYM>
 __global__ void __launch_bounds__(128, 3) k_f3_pass_a(F3PassA a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int item = blockIdx.x * 4 + warp;
-  if (item >= a.n_items) return;
   cplx* S = reinterpret_cast<cplx*>(smem_raw) + warp * (F3_N * F3_PITCH);
-  const int ix = item % a.NX, cc = item / a.NX, c = cc & 1;
-  const double s = a.scale ? a.scale[cc >> 1] : 1.0;
-  const cplx* src = a.psi + (size_t)item * F3_PLANE;
   cplx x[F3_N];
+  for (int item = blockIdx.x * 4 + warp; item < a.n_items; item += gridDim.x * 4) {
+    const int ix = item % a.NX, cc = item / a.NX, c = cc & 1;
+    const double s = a.scale ? a.scale[cc >> 1] : 1.0;
+    const cplx* src = a.psi + (size_t)item * F3_PLANE;
+    const double* al = a.alpha[c] + (size_t)ix * F3_PLANE;
+#pragma unroll 1
+    for (int t = 0; t < (SYM ? 2 : 1); ++t) {
 #pragma unroll
-  for (int t = 0; t < (SYM ? 2 : 1); ++t) {
-    if (t == 0) {
+      for (int j = 0; j < F3_N; ++j) {
+        double f = s;
+        if (SYM && t) f *= al[j * F3_N + lane];
+        x[j] = cscale(src[j * F3_N + lane], f);                  // (y = j, z = lane)
+      }
+      f3_plane_forward(x, S, lane);                              // (kz = j, ky = lane)
+      cplx* dst = (t == 0 ? a.spec0 : a.spec1) + (size_t)item * F3_PLANE;
 #pragma unroll
-      for (int j = 0; j < F3_N; ++j) x[j] = cscale(src[j * F3_N + lane], s);
-    } else {
-      const double* al = a.alpha[c] + (size_t)ix * F3_PLANE;
-#pragma unroll
-      for (int j = 0; j < F3_N; ++j) x[j] = cscale(src[j * F3_N + lane], s * al[j * F3_N + lane]);
+      for (int j = 0; j < F3_N; ++j) dst[j * F3_N + lane] = x[j];
     }
-    fft_reg<F3_N, false>(x);                                   // along y; lane = z
-#pragma unroll
-    for (int j = 0; j < F3_N; ++j) S[j * F3_PITCH + lane] = x[j];
-    __syncwarp();
-#pragma unroll
-    for (int j = 0; j < F3_N; ++j) x[j] = S[lane * F3_PITCH + j];   // lane = ky, j = z
-    __syncwarp();
-    fft_reg<F3_N, false>(x);                                   // along z
-    cplx* dst = (t == 0 ? a.spec0 : a.spec1) + (size_t)item * F3_PLANE;
-#pragma unroll
-    for (int j = 0; j < F3_N; ++j) dst[j * F3_N + lane] = x[j];    // [kz = j][ky = lane]
   }
 }
 
@@ -85,24 +95,32 @@ struct F3PassB {
   double invM;
 };
 
+// The inverse transform is conj(FFT(conj(x))) (exact: conjugation only flips signs), so only the forward
+// butterfly code is instantiated and the two directions share one loop body.
 template <int NX>
 __global__ void __launch_bounds__(128, 3) k_f3_pass_b(F3PassB a) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int item = blockIdx.x * 4 + warp;
-  if (item >= a.n_items) return;
-  const int kz = item & (F3_N - 1), cc = item >> 5;
-  const double kyz2 = a.ky2[lane] + a.kz2[kz];
   cplx x[NX];
-  for (int t = 0; t < a.n_spec; ++t) {
-    cplx* p = a.spec[t] + (size_t)cc * NX * F3_PLANE + kz * F3_N + lane;
+  for (int item = blockIdx.x * 4 + warp; item < a.n_items; item += gridDim.x * 4) {
+    const int kz = item & (F3_N - 1), cc = item >> 5;
+    const double kyz2 = a.ky2[lane] + a.kz2[kz];
+#pragma unroll 1
+    for (int t = 0; t < a.n_spec; ++t) {
+      cplx* p = a.spec[t] + (size_t)cc * NX * F3_PLANE + kz * F3_N + lane;
 #pragma unroll
-    for (int j = 0; j < NX; ++j) x[j] = p[(size_t)j * F3_PLANE];
-    fft_reg<NX, false>(x);
+      for (int j = 0; j < NX; ++j) x[j] = p[(size_t)j * F3_PLANE];
+#pragma unroll 1
+      for (int dir = 0; dir < 2; ++dir) {
+        fft_reg<NX, false>(x);
 #pragma unroll
-    for (int j = 0; j < NX; ++j) x[j] = cscale(x[j], -(a.kx2[j] + kyz2) * a.invM);   // even derivative: Nyquist kept
-    fft_reg<NX, true>(x);
+        for (int j = 0; j < NX; ++j) {
+          const double f = dir ? 1.0 : -(a.kx2[j] + kyz2) * a.invM;     // even derivative: Nyquist kept
+          x[j] = make_double2(x[j].x * f, -x[j].y * f);                 // conj(x) * f
+        }
+      }
 #pragma unroll
-    for (int j = 0; j < NX; ++j) p[(size_t)j * F3_PLANE] = x[j];
+      for (int j = 0; j < NX; ++j) p[(size_t)j * F3_PLANE] = x[j];
+    }
   }
 }
 
@@ -125,95 +143,84 @@ struct F3PassC {
   int NX;
 };
 
-// inverse 2-D transform of one plane: in x[j] = spectrum (kz = j, ky = lane), out x[j] = value (y = j, z = lane)
-__device__ __forceinline__ void f3_plane_inverse(cplx* x, cplx* S, int lane) {
-  fft_reg<F3_N, true>(x);                                      // along z: x[j] = (z = j, ky = lane)
-#pragma unroll
-  for (int j = 0; j < F3_N; ++j) S[j * F3_PITCH + lane] = x[j];
-  __syncwarp();
-#pragma unroll
-  for (int j = 0; j < F3_N; ++j) x[j] = S[lane * F3_PITCH + j];     // lane = z, j = ky
-  __syncwarp();
-  fft_reg<F3_N, true>(x);                                      // along y
-}
-
 template <bool SYM, int MODE>
 __global__ void __launch_bounds__(64, SYM ? 3 : 6) k_f3_pass_c(F3PassC a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int item = blockIdx.x * 2 + warp;
-  if (item >= a.n_items) return;
   constexpr int PER_WARP = F3_N * F3_PITCH + (SYM ? F3_PLANE : 0);
   cplx* S = reinterpret_cast<cplx*>(smem_raw) + warp * PER_WARP;
   cplx* T = S + F3_N * F3_PITCH;                               // SYM: alpha * lap w, thread-private slots
-  const int ix = item % a.NX, n = item / a.NX;
   const size_t M = (size_t)a.NX * F3_PLANE;
-  const double s = a.scale ? a.scale[n] : 1.0, kp2 = a.kperp2[n];
-  const size_t pl = (size_t)ix * F3_PLANE;                      // plane offset inside a field / component
-  const cplx* pu = a.psi + (size_t)(2 * n) * M + pl;
-  const cplx* pv = pu + M;
-  double e = 0.0, xx = 0.0, xpr = 0.0, xpi = 0.0, pp = 0.0;
-  cplx x[F3_N];
-#pragma unroll
-  for (int c = 0; c < 2; ++c) {
-    const size_t cplane = ((size_t)(2 * n + c) * a.NX + ix) * F3_PLANE;
-    const double* al = a.F.alpha[c] + pl;
-    {
-      const cplx* sp = a.spec0 + cplane;
-#pragma unroll
-      for (int j = 0; j < F3_N; ++j) x[j] = sp[j * F3_N + lane];
-      f3_plane_inverse(x, S, lane);
-    }
-    if (SYM) {
-#pragma unroll
-      for (int j = 0; j < F3_N; ++j) T[j * F3_N + lane] = cscale(x[j], al[j * F3_N + lane]);
-      const cplx* sp = a.spec1 + cplane;
-#pragma unroll
-      for (int j = 0; j < F3_N; ++j) x[j] = sp[j * F3_N + lane];
-      f3_plane_inverse(x, S, lane);
-    }
-    const double* lp = a.F.lap[c] + pl;
-    const double* Uc = a.F.U[c] + pl;
-    const double mu = a.F.mu[c];
-#pragma unroll
-    for (int j = 0; j < F3_N; ++j) {
-      const int i = j * F3_N + lane;
-      const cplx u = cscale(pu[i], s), v = cscale(pv[i], s);
-      const cplx w = c ? v : u;
-      cplx K;
-      if (SYM) {
-        const cplx t = T[i];
-        const double a_ = al[i], l_ = lp[i], h = 0.5 * a_ * kp2;
-        K.x = -0.25 * (x[j].x + t.x - l_ * w.x) + h * w.x;     // Eq. 40 + transverse shift
-        K.y = -0.25 * (x[j].y + t.y - l_ * w.y) + h * w.y;
-      } else {
-        K.x = -0.5 * x[j].x + 0.5 * kp2 * w.x;                 // Eq. 14
-        K.y = -0.5 * x[j].y + 0.5 * kp2 * w.y;
-      }
-      const cplx D = cadd(a.F.delta[pl + i], a.F.dext[pl + i]);
-      const double pot = Uc[i] - mu;
-      cplx H;
-      if (c == 0) H = cadd(K, cadd(cscale(u, pot), cmul(D, v)));                  // Eqs. 5, 15
-      else H = csub(cmul(cconj(D), u), cadd(K, cscale(v, pot)));
-      e += w.x * H.x + w.y * H.y;
-      cplx o;
-      if (MODE == F3_APPLY) o = H;
-      else if (MODE == F3_RHS) o = make_double2(H.y, -H.x);                        // -i H
-      else {
-        const cplx cp = a.cpart[(size_t)(2 * n + c) * M + pl + i];
-        o = make_double2(cp.x + a.kappa * H.y, cp.y - a.kappa * H.x);             // C_part - i kappa H
-        xx += cabs2(o); xpr += o.x * w.x + o.y * w.y; xpi += o.x * w.y - o.y * w.x; pp += cabs2(w);
-      }
-      a.out[(size_t)(2 * n + c) * M + pl + i] = o;
-    }
-    if (SYM) __syncwarp();
-  }
   const int np = a.n_items;
-  e = warp_sum(e);
-  if (MODE == F3_CORR) { xx = warp_sum(xx); xpr = warp_sum(xpr); xpi = warp_sum(xpi); pp = warp_sum(pp); }
-  if (lane == 0) {
-    a.part[item] = e;
-    if (MODE == F3_CORR) { a.part[np + item] = xx; a.part[2 * np + item] = xpr; a.part[3 * np + item] = xpi; a.part[4 * np + item] = pp; }
+  cplx x[F3_N];
+  for (int item = blockIdx.x * 2 + warp; item < a.n_items; item += gridDim.x * 2) {
+    const int ix = item % a.NX, n = item / a.NX;
+    const double s = a.scale ? a.scale[n] : 1.0, kp2 = a.kperp2[n];
+    const size_t pl = (size_t)ix * F3_PLANE;                    // plane offset inside a field / component
+    const cplx* pu = a.psi + (size_t)(2 * n) * M + pl;
+    const cplx* pv = pu + M;
+    double e = 0.0, xx = 0.0, xpr = 0.0, xpi = 0.0, pp = 0.0;
+#pragma unroll 1
+    for (int c = 0; c < 2; ++c) {
+      const size_t cplane = ((size_t)(2 * n + c) * a.NX + ix) * F3_PLANE;
+      const double* al = a.F.alpha[c] + pl;
+#pragma unroll 1
+      for (int t = 0; t < (SYM ? 2 : 1); ++t) {
+        const cplx* sp = (t ? a.spec1 : a.spec0) + cplane;
+#pragma unroll
+        for (int j = 0; j < F3_N; ++j) x[j] = cconj(sp[j * F3_N + lane]);        // (kz = j, ky = lane), conjugated
+        f3_plane_forward(x, S, lane);                                             // conj of value at (y = j, z = lane)
+        if (SYM && t == 0) {
+#pragma unroll
+          for (int j = 0; j < F3_N; ++j) T[j * F3_N + lane] = cscale(cconj(x[j]), al[j * F3_N + lane]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < F3_N; ++j) S[j * F3_PITCH + lane] = cconj(x[j]);   // own column: thread-private
+        }
+      }
+      const double* lp = a.F.lap[c] + pl;
+      const double* Uc = a.F.U[c] + pl;
+      const double mu = a.F.mu[c];
+      const size_t ob = (size_t)(2 * n + c) * M + pl;
+#pragma unroll 4
+      for (int j = 0; j < F3_N; ++j) {
+        const int i = j * F3_N + lane;
+        const cplx u = cscale(pu[i], s), v = cscale(pv[i], s);
+        const cplx w = c ? v : u;
+        const cplx L = S[j * F3_PITCH + lane];
+        cplx K;
+        if (SYM) {
+          const cplx t = T[i];
+          const double a_ = al[i], l_ = lp[i], h = 0.5 * a_ * kp2;
+          K.x = -0.25 * (L.x + t.x - l_ * w.x) + h * w.x;        // Eq. 40 + transverse shift
+          K.y = -0.25 * (L.y + t.y - l_ * w.y) + h * w.y;
+        } else {
+          K.x = -0.5 * L.x + 0.5 * kp2 * w.x;                    // Eq. 14
+          K.y = -0.5 * L.y + 0.5 * kp2 * w.y;
+        }
+        const cplx D = cadd(a.F.delta[pl + i], a.F.dext[pl + i]);
+        const double pot = Uc[i] - mu;
+        cplx H;
+        if (c == 0) H = cadd(K, cadd(cscale(u, pot), cmul(D, v)));                // Eqs. 5, 15
+        else H = csub(cmul(cconj(D), u), cadd(K, cscale(v, pot)));
+        e += w.x * H.x + w.y * H.y;
+        cplx o;
+        if (MODE == F3_APPLY) o = H;
+        else if (MODE == F3_RHS) o = make_double2(H.y, -H.x);                      // -i H
+        else {
+          const cplx cp = a.cpart[ob + i];
+          o = make_double2(cp.x + a.kappa * H.y, cp.y - a.kappa * H.x);           // C_part - i kappa H
+          xx += cabs2(o); xpr += o.x * w.x + o.y * w.y; xpi += o.x * w.y - o.y * w.x; pp += cabs2(w);
+        }
+        a.out[ob + i] = o;
+      }
+    }
+    e = warp_sum(e);
+    if (MODE == F3_CORR) { xx = warp_sum(xx); xpr = warp_sum(xpr); xpi = warp_sum(xpi); pp = warp_sum(pp); }
+    if (lane == 0) {
+      a.part[item] = e;
+      if (MODE == F3_CORR) { a.part[np + item] = xx; a.part[2 * np + item] = xpr; a.part[3 * np + item] = xpi; a.part[4 * np + item] = pp; }
+    }
   }
 }
 

@@ -11,6 +11,9 @@ static F3Fields f3_fields(const wslda_ctx* c) {
   return F;
 }
 
+// persistent grids: at most (CTAs per SM) x 148 SMs, warps stride over the items
+static inline int f3_grid(int want, int per_sm) { const int cap = per_sm * 148; return want < cap ? want : cap; }
+
 // out = APPLY: H psi | CORR: C_part - i kappa H psi | RHS: -i H psi  for the cnt spinors of a chunk (psi_chunk,
 // scale_chunk, out, cpart already offset to the chunk; n0 = global index of its first spinor); pass-C partial
 // sums go to f_part[q].  q = scratch slot, st = the stream that owns it.
@@ -27,18 +30,18 @@ static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk,
   a.spec0 = c->f_spec0[q]; a.spec1 = c->f_spec1[q]; a.n_items = cnt * 2 * NX; a.NX = NX;
   WORK(c, 32.0 * M * cnt, fl_plane);                       // reads psi once
   auto ka = sym ? k_f3_pass_a<true> : k_f3_pass_a<false>;
-  LAUNCHN(c, "k_f3_pass_a", ka, (a.n_items + 3) / 4, 128, 4 * F3_TILE_BYTES, st, a);
+  LAUNCHN(c, "k_f3_pass_a", ka, f3_grid((a.n_items + 3) / 4, 3), 128, 4 * F3_TILE_BYTES, st, a);
   F3PassB b;
   b.spec[0] = c->f_spec0[q]; b.spec[1] = c->f_spec1[q]; b.n_spec = nspec; b.n_items = cnt * 2 * F3_N;
   b.ky2 = c->k2n[1]; b.kz2 = c->k2n[2]; b.invM = c->L.invM;
   for (int j = 0; j < 32; ++j) b.kx2[j] = j < NX ? c->hk2[0][j] : 0.0;
   WORK(c, 0, fl_x);
   auto kb = NX == 32 ? k_f3_pass_b<32> : NX == 16 ? k_f3_pass_b<16> : k_f3_pass_b<8>;
-  LAUNCHN(c, "k_f3_pass_b", kb, (b.n_items + 3) / 4, 128, 0, st, b);
+  LAUNCHN(c, "k_f3_pass_b", kb, f3_grid((b.n_items + 3) / 4, 3), 128, 0, st, b);
   F3PassC k;
   k.spec0 = c->f_spec0[q]; k.spec1 = c->f_spec1[q]; k.psi = psi_chunk; k.scale = scale_chunk; k.kperp2 = c->kperp2 + n0;
   k.F = f3_fields(c); k.out = out; k.cpart = cpart; k.kappa = kappa; k.part = c->f_part[q]; k.n_items = cnt * NX; k.NX = NX;
-  const int grid = (k.n_items + 1) / 2;
+  const int grid = f3_grid((k.n_items + 1) / 2, sym ? 3 : 6);
   const size_t sm_sym = 2 * (F3_TILE_BYTES + F3_PLANE * 16), sm_lap = 2 * F3_TILE_BYTES;
   WORK(c, mode == F3_CORR ? 32.0 * M * cnt : (mode == F3_APPLY ? 32.0 * M * cnt : 0.0), fl_plane);
   void (*kc)(F3PassC);
