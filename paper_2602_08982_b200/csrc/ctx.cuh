@@ -8,6 +8,7 @@
 #include "density.cuh"
 #include "fft_large.cuh"
 #include "fast3d.cuh"
+#include "mega3d.cuh"
 #include "kernels.cuh"
 
 struct Plan {
@@ -21,6 +22,9 @@ struct Plan {
   // fused 3-D path (fast3d.cuh): enabled flag, spinors per chunk, concurrent streams, per-stream scratch
   int fast, fc, ns;
   size_t off_fast, fast_spec_bytes, fast_part_bytes, fast_stream_bytes;
+  // persistent dataflow kernels (mega3d.cuh): enabled flag, spinors per group, number of groups, ring buffers
+  int mega, gs, mG;
+  size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -90,6 +94,19 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
+  P.mega = P.fast; P.gs = 8;
+  if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
+  if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
+  if (P.gs > n_wf) P.gs = (int)n_wf;
+  P.mG = (int)((n_wf + P.gs - 1) / P.gs);
+  P.off_mega = o; P.mega_ring_bytes = P.mega_part_bytes = P.mega_acc_bytes = P.mega_sync_bytes = 0;
+  if (P.mega) {
+    P.mega_ring_bytes = align_up((size_t)F3_RING * P.gs * 2 * M * 16);
+    P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * P.N[0] * 8);
+    P.mega_acc_bytes = align_up((size_t)F3_RING * 4 * M * 8);
+    P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * P.mG * sizeof(int));
+    o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes;
+  }
   P.total = o;
   return 0;
 }
@@ -108,6 +125,10 @@ struct wslda_ctx {
   cudaStream_t aux[4];             // fused path: concurrent chunk streams (created by the library)
   cudaEvent_t ev_fork, ev_join[4];
   cplx *f_spec0[4], *f_spec1[4], *f_X[4];
+  cplx *m_spec0, *m_spec1, *m_X;   // persistent-kernel rings
+  double *m_part, *m_acc;
+  F3Sync* m_sync;
+  int mega_grid;
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
@@ -260,6 +281,24 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
+  }
+  if (P.mega) {
+    char* b = base + P.off_mega;
+    c->m_spec0 = (cplx*)b; c->m_spec1 = (cplx*)(b + P.mega_ring_bytes); c->m_X = (cplx*)(b + 2 * P.mega_ring_bytes);
+    b += 3 * P.mega_ring_bytes;
+    c->m_part = (double*)b; b += P.mega_part_bytes;
+    c->m_acc = (double*)b; b += P.mega_acc_bytes;
+    c->m_sync = (F3Sync*)b;
+    int occ = 0, best = 3;
+#define WS_MEGA_ATTR(K) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES); \
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, K, 128, 4 * F3_TILE_BYTES); if (occ > 0 && occ < best) best = occ; } while (0)
+    WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
+    WS_MEGA_ATTR((k_f3_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<false, F3_RHS>));
+#undef WS_MEGA_ATTR
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+    c->mega_grid = best * sms;
+    if (const char* e = getenv("WSLDA_MEGA_CTAS")) { int v = atoi(e); if (v > 0) c->mega_grid = v; }
   }
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
   cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);

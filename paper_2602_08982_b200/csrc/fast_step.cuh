@@ -50,6 +50,36 @@ static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk,
   LAUNCHN(c, "k_f3_pass_c", kc, grid, 64, sym ? sm_sym : sm_lap, st, k);
 }
 
+// One persistent dataflow launch (mega3d.cuh) over spinors [n0, n0 + n) of the caller's buffers:
+// APPLY: out = H psi (+ eps via k_f3_scal); CORR: psi buffer <- phi_new (normalised) + densities; RHS: out = f(psi).
+static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, const double* scale, int64_t n0, int64_t n,
+                    cplx* out, const cplx* cpart, double kappa, int do_dens) {
+  const Plan& P = c->P;
+  const bool sym = c->f.kin_form == WSLDA_KIN_SYM40;
+  F3Mega a;
+  a.psi = psi; a.scale = scale; a.kperp2 = c->kperp2 + n0; a.F = f3_fields(c);
+  a.ky2 = c->k2n[1]; a.kz2 = c->k2n[2];
+  for (int j = 0; j < 32; ++j) a.kx2[j] = j < P.N[0] ? c->hk2[0][j] : 0.0;
+  a.invM = c->L.invM; a.dV = c->dV; a.kappa = kappa;
+  a.spec0 = c->m_spec0; a.spec1 = c->m_spec1; a.X = c->m_X; a.out = out; a.cpart = cpart; a.part = c->m_part;
+  a.eps_out = mode == F3_APPLY ? nullptr : c->eps + n0;
+  a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.do_dens = do_dens;
+  a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.acc = c->m_acc; a.sync = c->m_sync;
+  a.n = (int)n; a.gs = P.gs; a.G = (int)((n + P.gs - 1) / P.gs); a.NX = P.N[0];
+  cudaMemsetAsync(c->m_sync, 0, sizeof(F3Sync) + (size_t)4 * a.G * sizeof(int), st);
+  const int NX = P.N[0], nspec = sym ? 2 : 1;
+  const int IT = a.gs * 2 * NX / 4 + a.gs * 16 + (sym ? a.gs * NX : a.gs * NX / 2) + (mode == F3_APPLY ? 0 : NX * F3_DSPLIT);
+  const long total = (long)(a.G + 3) * IT;
+  const int grid = (int)(total < c->mega_grid ? total : c->mega_grid);
+  const double M = (double)P.M;
+  WORK(c, M * n * (mode == F3_CORR ? 96.0 : 64.0), 5.0 * M * (P.lg[0] + 10.0) * 2.0 * 2 * nspec * n);
+  void (*k)(F3Mega);
+  if (sym) k = mode == F3_APPLY ? k_f3_mega<true, F3_APPLY> : mode == F3_CORR ? k_f3_mega<true, F3_CORR> : k_f3_mega<true, F3_RHS>;
+  else k = mode == F3_APPLY ? k_f3_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3_mega<false, F3_CORR> : k_f3_mega<false, F3_RHS>;
+  LAUNCHN(c, mode == F3_APPLY ? "k_f3_mega_apply" : mode == F3_CORR ? "k_f3_mega_corr" : "k_f3_mega_rhs", k, grid, 128,
+          4 * F3_TILE_BYTES, st, a);
+}
+
 static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, int mode, int use_shift, double kappa,
                     double* eps_user) {
   F3Scal s;
@@ -61,6 +91,14 @@ static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, i
 static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
                                cudaStream_t st) {
   const int64_t M = c->P.M;
+  if (c->P.mega && n_count > 0) {
+    f3_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0);
+    F3Scal s;
+    s.part = c->m_part; s.cnt = (int)n_count; s.NX = c->P.N[0]; s.mode = F3_APPLY; s.use_shift = 1; s.normalize = 0;
+    s.dV = c->dV; s.kappa = 0.0; s.eps = c->eps + n_first; s.eps_user = eps_dev ? eps_dev + n_first : nullptr; s.scale_new = nullptr;
+    LAUNCH(c, k_f3_scal, (unsigned)((n_count + 3) / 4), 128, 0, st, s);
+    return cuda_check(c, "apply_h");
+  }
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.fc) {
     const int cnt = (int)((n_first + n_count - n0 < c->P.fc) ? n_first + n_count - n0 : c->P.fc);
     f3_hpsi(c, 0, st, psi + 2 * n0 * M, nullptr, n0, cnt, F3_APPLY, hpsi + 2 * n0 * M, nullptr, 0.0);
@@ -146,6 +184,31 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
   const int used = (int)(n_chunks < ns ? n_chunks : ns);
   auto cnt_of = [&](int64_t k) { return (int)((n_wf - k * fc < fc) ? n_wf - k * fc : fc); };
   const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
+  if (P.mega) {                                          // stage 1 in chunks, stages 2 and 3 as persistent dataflow kernels
+    f3_fork(c, s);
+    for (int64_t k = 0; k < n_chunks; ++k) {
+      const int q = (int)(k % ns); cudaStream_t st = f3_stream(c, s, q);
+      const int64_t n0 = k * fc; const int cnt = cnt_of(k);
+      f3_stage1(c, s, q, st, n0, cnt);
+      if (!fixed) {
+        F3DensOnly d;
+        d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
+        d.d = f3_dens_args(c, q, n0, k < ns);
+        WORK(c, 0, 0);
+        LAUNCH(c, k_f3_dens, nb(P.M, 128), 128, 0, st, d);
+      }
+    }
+    f3_join(c, s);
+    if (!fixed) { f3_dens_final(c, used, s.user); potentials(c, s.user); }
+    f3_mega(c, s.user, F3_CORR, s.phi, c->f.normalize ? c->scale : nullptr, 0, n_wf, s.phi, s.cpart, s.c0dt, !fixed);
+    if (!fixed) {
+      const int slots = (int)(c->P.mG < F3_RING ? c->P.mG : F3_RING);
+      LAUNCH(c, k_f3_dens_final, nb(4 * P.M, 256), 256, 0, s.user, c->m_acc, slots, (int64_t)(4 * P.M), P.M, c->raw);
+      potentials(c, s.user);
+    }
+    f3_mega(c, s.user, F3_RHS, s.phi, nullptr, 0, n_wf, s.cpart, nullptr, 0.0, 0);
+    return;
+  }
   f3_fork(c, s);
   if (fixed) {
     for (int64_t k = 0; k < n_chunks; ++k) {

@@ -197,6 +197,7 @@ def test_run_to_run_bit_reproducible():
 def small_fast_chunks(monkeypatch):
     monkeypatch.setenv("WSLDA_FAST_CHUNK", "3")
     monkeypatch.setenv("WSLDA_FAST_STREAMS", "3")
+    monkeypatch.setenv("WSLDA_MEGA_GROUP", "3")          # ragged last group, more groups than ring slots
 
 
 @pytest.mark.parametrize("kin_form", [0, 1])
