@@ -94,7 +94,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
-  P.mega = P.fast; P.gs = 8;
+  P.mega = P.fast; P.gs = 4;
   if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
   if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
   if (P.gs > n_wf) P.gs = (int)n_wf;
@@ -289,7 +289,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->m_part = (double*)b; b += P.mega_part_bytes;
     c->m_acc = (double*)b; b += P.mega_acc_bytes;
     c->m_sync = (F3Sync*)b;
-    int occ = 0, best = 3;
+    int occ = 0, best = F3_MEGA_OCC;
 #define WS_MEGA_ATTR(K) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES); \
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, K, 128, 4 * F3_TILE_BYTES); if (occ > 0 && occ < best) best = occ; } while (0)
     WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
@@ -351,6 +351,14 @@ extern "C" int wslda_profile_report(wslda_ctx* c, char* buf, size_t buf_bytes) {
   }
   return (int)names.size();
 }
+
+#ifdef F3_TIMING
+extern "C" void wslda_debug_cycles(unsigned long long* out, int reset) {
+  cudaDeviceSynchronize();
+  if (out) cudaMemcpyFromSymbol(out, g_f3_cycles, sizeof(unsigned long long) * 64);
+  if (reset) { unsigned long long z[64] = {0}; cudaMemcpyToSymbol(g_f3_cycles, z, sizeof z); }
+}
+#endif
 
 extern "C" wslda_status wslda_ctx_destroy(wslda_ctx* c) {
   if (!c) return WSLDA_EINVAL;

@@ -15,6 +15,16 @@
 #include "fast3d.cuh"
 
 #define F3_RING 4
+// optional phase timing (build with -DF3_TIMING): per-kind cycle sums in g_f3_cycles[kind][phase]
+#ifdef F3_TIMING
+__device__ unsigned long long g_f3_cycles[8][8];
+#define F3_T0() long long t_ = clock64()
+#define F3_T(kind, phase) do { long long n_ = clock64(); if ((threadIdx.x & 31) == 0) atomicAdd(&g_f3_cycles[kind][phase], (unsigned long long)(n_ - t_)); t_ = n_; } while (0)
+#else
+#define F3_T0() do {} while (0)
+#define F3_T(kind, phase) do {} while (0)
+#endif
+#define F3_MEGA_OCC 2
 #define F3_DSPLIT 2            // D items per x-plane
 
 struct F3Sync {                // device counters, zeroed before every launch
@@ -47,6 +57,29 @@ struct F3Mega {
 
 __device__ __forceinline__ cplx ldcg2(const cplx* p) { return __ldcg(p); }
 
+// L2 eviction priorities (createpolicy, PTX ISA 7.4+): the spectrum / X rings and psi are re-read by later items
+// and must survive in L2 (evict_last); data touched for the last time is marked evict_first so that it leaves
+// first.  KEEP / DROP are per-thread 64-bit policy words.
+struct F3Pol { uint64_t keep, drop; };
+__device__ __forceinline__ F3Pol f3_policies() {
+  F3Pol p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p.keep));
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p.drop));
+  return p;
+}
+__device__ __forceinline__ cplx ld_pol(const cplx* p, uint64_t pol) {        // L1-bypassing load with an L2 policy
+  cplx v;
+  asm volatile("ld.global.cg.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ void st_pol(cplx* p, cplx v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
+__device__ __forceinline__ void f3_pf1(const void* p) { asm volatile("prefetch.global.L1 [%0];" :: "l"(p)); }
+__device__ __forceinline__ void f3_pf(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
+
 // one thread waits until *ctr >= target (bounded), then the whole CTA proceeds
 __device__ __forceinline__ void f3_wait(int* ctr, int target, F3Sync* sy) {
   if (threadIdx.x == 0) {
@@ -59,14 +92,15 @@ __device__ __forceinline__ void f3_wait(int* ctr, int target, F3Sync* sy) {
   }
   __syncthreads();
 }
-__device__ __forceinline__ void f3_signal(int* ctr) {
+__device__ __forceinline__ void f3_signal(int* ctr, int* next, int& ticket) {
+  if (threadIdx.x == 0) ticket = atomicAdd(next, 1);       // the next ticket travels while the barrier and the fence complete
   __syncthreads();
   if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1); }
 }
 
 // ---- A: forward plane transforms of 4 component planes (one per warp) ----------------------------------------
 template <bool SYM>
-__device__ __forceinline__ void f3_body_a(const F3Mega& a, int g, int ia, cplx* tiles, cplx* x) {
+__device__ __forceinline__ void f3_body_a(const F3Mega& a, const F3Pol& pol, int g, int ia, cplx* tiles, cplx* x) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int p = 4 * ia + warp, nl = p / (2 * a.NX), rem = p - nl * 2 * a.NX, c = rem / a.NX, ix = rem - c * a.NX;
   const int n = g * a.gs + nl;
@@ -78,34 +112,40 @@ __device__ __forceinline__ void f3_body_a(const F3Mega& a, int g, int ia, cplx* 
   const double* al = a.F.alpha[c] + (size_t)ix * F3_PLANE;
   const size_t sb = (((size_t)(g % F3_RING) * a.gs + nl) * 2 + c) * M + (size_t)ix * F3_PLANE;
 #pragma unroll 1
+  F3_T0();
   for (int t = 0; t < (SYM ? 2 : 1); ++t) {
 #pragma unroll
     for (int j = 0; j < F3_N; ++j) {
       double f = s;
       if (SYM && t) f *= al[j * F3_N + lane];
-      x[j] = cscale(src[j * F3_N + lane], f);
+      x[j] = cscale(ld_pol(src + j * F3_N + lane, pol.keep), f);      // psi is read again by C (and D)
     }
+    F3_T(0, 0);
     f3_plane_forward(x, S, lane);
+    F3_T(0, 1);
     cplx* dst = (t == 0 ? a.spec0 : a.spec1) + sb;
 #pragma unroll
-    for (int j = 0; j < F3_N; ++j) dst[j * F3_N + lane] = x[j];
+    for (int j = 0; j < F3_N; ++j) st_pol(dst + j * F3_N + lane, x[j], pol.keep);
+    F3_T(0, 2);
   }
 }
 
 // ---- B: x-lines of 4 (component, kz) rows: FFT x, -k^2/M, inverse FFT x, in place ------------------------------
 template <int NX, bool SYM>
-__device__ __forceinline__ void f3_body_b(const F3Mega& a, int g, int ib, cplx* x) {
+__device__ __forceinline__ void f3_body_b(const F3Mega& a, const F3Pol& pol, int g, int ib, cplx* x) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int q = 4 * ib + warp, kz = q & (F3_N - 1), ccl = q >> 5;
   if (g * a.gs + (ccl >> 1) >= a.n) return;
   const size_t M = (size_t)NX * F3_PLANE;
   const double kyz2 = a.ky2[lane] + a.kz2[kz];
   const size_t sb = ((size_t)(g % F3_RING) * a.gs * 2 + ccl) * M + kz * F3_N + lane;
+  F3_T0();
 #pragma unroll 1
   for (int t = 0; t < (SYM ? 2 : 1); ++t) {
     cplx* p = (t ? a.spec1 : a.spec0) + sb;
 #pragma unroll
-    for (int j = 0; j < NX; ++j) x[j] = ldcg2(p + (size_t)j * F3_PLANE);
+    for (int j = 0; j < NX; ++j) x[j] = ld_pol(p + (size_t)j * F3_PLANE, pol.keep);
+    F3_T(1, 0);
 #pragma unroll 1
     for (int dir = 0; dir < 2; ++dir) {
       fft_reg<NX, false>(x);
@@ -116,7 +156,10 @@ __device__ __forceinline__ void f3_body_b(const F3Mega& a, int g, int ib, cplx* 
       }
     }
 #pragma unroll
-    for (int j = 0; j < NX; ++j) p[(size_t)j * F3_PLANE] = x[j];
+    F3_T(1, 1);
+#pragma unroll
+    for (int j = 0; j < NX; ++j) st_pol(p + (size_t)j * F3_PLANE, x[j], pol.keep);
+    F3_T(1, 2);
   }
 }
 
@@ -125,7 +168,7 @@ __device__ __forceinline__ void f3_body_b(const F3Mega& a, int g, int ib, cplx* 
 // Eq. 14: lap u | lap v of TWO x-planes.  Each warp leaves its plane in its own tile; after the barrier every
 // thread finishes 32 / WPI rows of both components (psi, C_part and the fields are read once per point).
 template <bool SYM, int MODE>
-__device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* tiles, double* red, cplx* x) {
+__device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int g, int ic, cplx* tiles, double* red, cplx* x) {
   constexpr int NS = SYM ? 2 : 1, WPI = 2 * NS, IPC = 4 / WPI, ROWS = F3_N / WPI, TILE = F3_N * F3_PITCH;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int pI = warp / WPI, wl = warp % WPI, c = wl / NS, t = wl % NS;
@@ -134,11 +177,33 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* 
   const size_t M = (size_t)a.NX * F3_PLANE, pl = (size_t)ix * F3_PLANE;
   const size_t ring = ((size_t)(g % F3_RING) * a.gs + nl) * 2;        // ring index of component 0 of this spinor
   cplx* S = tiles + warp * TILE;
+  F3_T0();
   if (valid) {
+    // this thread's epilogue rows: pull psi, C_part and the fields towards L1 now, they are used after the transform
+    {
+      const size_t r0 = pl + (size_t)(wl * ROWS) * F3_N;             // first point of the warp's rows
+      const char* pu8 = (const char*)(a.psi + (size_t)(2 * n) * M + r0);
+      const char* cu8 = (const char*)(a.cpart + (size_t)(2 * n) * M + r0);
+      constexpr int LW = ROWS * F3_N * 16 / 128;                     // 128-byte lines of complex rows per warp
+      for (int q = lane; q < LW; q += 32) {
+        f3_pf1(pu8 + q * 128); f3_pf1(pu8 + M * 16 + q * 128);
+        if (MODE == F3_CORR) { f3_pf1(cu8 + q * 128); f3_pf1(cu8 + M * 16 + q * 128); }
+        f3_pf1((const char*)(a.F.delta + r0) + q * 128); f3_pf1((const char*)(a.F.dext + r0) + q * 128);
+      }
+      for (int q = lane; q < LW / 2; q += 32) {
+        f3_pf1((const char*)(a.F.U[0] + r0) + q * 128); f3_pf1((const char*)(a.F.U[1] + r0) + q * 128);
+        if (SYM) {
+          f3_pf1((const char*)(a.F.alpha[0] + r0) + q * 128); f3_pf1((const char*)(a.F.alpha[1] + r0) + q * 128);
+          f3_pf1((const char*)(a.F.lap[0] + r0) + q * 128); f3_pf1((const char*)(a.F.lap[1] + r0) + q * 128);
+        }
+      }
+    }
     const cplx* sp = (t ? a.spec1 : a.spec0) + (ring + c) * M + pl;
 #pragma unroll
-    for (int j = 0; j < F3_N; ++j) x[j] = cconj(ldcg2(sp + j * F3_N + lane));
+    for (int j = 0; j < F3_N; ++j) x[j] = cconj(ld_pol(sp + j * F3_N + lane, pol.drop));        // last use of the spectrum
+    F3_T(2, 0);
     f3_plane_forward(x, S, lane);                                    // conj of the value at (y = j, z = lane)
+    F3_T(2, 1);
     const double* al = a.F.alpha[c] + pl;
 #pragma unroll
     for (int j = 0; j < F3_N; ++j) {
@@ -146,7 +211,9 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* 
       S[j * F3_PITCH + lane] = make_double2(x[j].x * f, -x[j].y * f);
     }
   }
+  F3_T(2, 2);
   __syncthreads();
+  F3_T(2, 3);
   double e = 0.0, xx = 0.0, xpr = 0.0, xpi = 0.0, pp = 0.0;
   if (valid) {
     const cplx* tb = tiles + pI * WPI * TILE;
@@ -179,13 +246,13 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* 
       const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                // Eqs. 5, 15
       const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, pb)));
       e += u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
-      if (MODE == F3_APPLY) { ou[i] = Hu; ov[i] = Hv; }
-      else if (MODE == F3_RHS) { ou[i] = make_double2(Hu.y, -Hu.x); ov[i] = make_double2(Hv.y, -Hv.x); }   // -i H
+      if (MODE == F3_APPLY) { st_pol(ou + i, Hu, pol.drop); st_pol(ov + i, Hv, pol.drop); }
+      else if (MODE == F3_RHS) { st_pol(ou + i, make_double2(Hu.y, -Hu.x), pol.keep); st_pol(ov + i, make_double2(Hv.y, -Hv.x), pol.keep); }   // -i H
       else {
         const cplx c0 = cu[i], c1 = cu[M + i];
         const cplx xu = make_double2(c0.x + a.kappa * Hu.y, c0.y - a.kappa * Hu.x);             // C_part - i kappa H
         const cplx xv = make_double2(c1.x + a.kappa * Hv.y, c1.y - a.kappa * Hv.x);
-        ou[i] = xu; ov[i] = xv;
+        st_pol(ou + i, xu, pol.keep); st_pol(ov + i, xv, pol.keep);
         xx += cabs2(xu) + cabs2(xv);
         xpr += xu.x * u.x + xu.y * u.y + xv.x * v.x + xv.y * v.y;
         xpi += xu.x * u.y - xu.y * u.x + xv.x * v.y - xv.y * v.x;
@@ -193,6 +260,7 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* 
       }
     }
   }
+  F3_T(2, 4);
   e = warp_sum(e);
   if (MODE == F3_CORR) { xx = warp_sum(xx); xpr = warp_sum(xpr); xpi = warp_sum(xpi); pp = warp_sum(pp); }
   if (lane == 0) {
@@ -214,12 +282,13 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, int g, int ic, cplx* 
 // CORR: phi_new = (X + i kappa eps w) * scale_new over P (Alg. 2 steps 4, 8) + densities of phi_new;
 // RHS : f_new = Y + i eps phi (Alg. 2 step 9, Eq. 45b).
 template <int MODE>
-__device__ __forceinline__ void f3_body_d(const F3Mega& a, int g, int id, double* s_eps, double* s_sn) {
+__device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int g, int id, double* s_eps, double* s_sn) {
   constexpr int PTS = F3_PLANE / F3_DSPLIT / 128;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ix = id / F3_DSPLIT, half = id - ix * F3_DSPLIT;
   const int cnt = (a.n - g * a.gs < a.gs) ? a.n - g * a.gs : a.gs;
   const size_t M = (size_t)a.NX * F3_PLANE, np = (size_t)a.n * a.NX;
+  F3_T0();
   for (int nl = warp; nl < cnt; nl += 4) {
     const int n = g * a.gs + nl;
     double v[F3_NPART];
@@ -240,40 +309,48 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, int g, int id, double
     }
   }
   __syncthreads();
+  F3_T(3, 0);
   const size_t p0 = (size_t)ix * F3_PLANE + half * (F3_PLANE / F3_DSPLIT) + threadIdx.x;
   const size_t ring = (size_t)(g % F3_RING) * a.gs * 2;
   double acc[PTS][4];
 #pragma unroll
   for (int r = 0; r < PTS; ++r) { acc[r][0] = acc[r][1] = acc[r][2] = acc[r][3] = 0.0; }
-#pragma unroll 1
+#pragma unroll 2
   for (int nl = 0; nl < cnt; ++nl) {
     const int n = g * a.gs + nl;
     const double e = s_eps[nl];
     const cplx* Xu = a.X + (ring + 2 * nl) * M + p0;
     const cplx* pu = a.psi + (size_t)(2 * n) * M + p0;
     cplx* ou = a.out + (size_t)(2 * n) * M + p0;
+    if (nl + 1 < cnt && (threadIdx.x & 7) == 0) {                 // one request per 128-byte line
+#pragma unroll
+      for (int r = 0; r < PTS; ++r) {
+        f3_pf1(pu + 2 * M + r * 128); f3_pf1(pu + 3 * M + r * 128);
+      }
+    }
     if (MODE == F3_CORR) {
       const double sP = a.scale ? a.scale[n] : 1.0, ke = a.kappa * e, sn = s_sn[nl];
       const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n];
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        const cplx xu = ldcg2(Xu + r * 128), xv = ldcg2(Xu + M + r * 128);
+        const cplx xu = ld_pol(Xu + r * 128, pol.drop), xv = ld_pol(Xu + M + r * 128, pol.drop);
         const cplx wu = cscale(pu[r * 128], sP), wv = cscale(pu[M + r * 128], sP);
         const cplx u = make_double2((xu.x - ke * wu.y) * sn, (xu.y + ke * wu.x) * sn);
         const cplx v = make_double2((xv.x - ke * wv.y) * sn, (xv.y + ke * wv.x) * sn);
-        ou[r * 128] = u; ou[M + r * 128] = v;
+        st_pol(ou + r * 128, u, pol.drop); st_pol(ou + M + r * 128, v, pol.drop);
         if (a.do_dens) f3_dens_add(acc[r], u, v, cp, wa, wb);
       }
     } else {
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        const cplx yu = ldcg2(Xu + r * 128), yv = ldcg2(Xu + M + r * 128);
+        const cplx yu = ld_pol(Xu + r * 128, pol.drop), yv = ld_pol(Xu + M + r * 128, pol.drop);
         const cplx u = pu[r * 128], v = pu[M + r * 128];
-        ou[r * 128] = make_double2(yu.x - e * u.y, yu.y + e * u.x);
-        ou[M + r * 128] = make_double2(yv.x - e * v.y, yv.y + e * v.x);
+        st_pol(ou + r * 128, make_double2(yu.x - e * u.y, yu.y + e * u.x), pol.drop);
+        st_pol(ou + M + r * 128, make_double2(yv.x - e * v.y, yv.y + e * v.x), pol.drop);
       }
     }
   }
+  F3_T(3, 1);
   if (MODE == F3_CORR && a.do_dens) {
     double* ac = a.acc + (size_t)(g % F3_RING) * 4 * M + p0;
 #pragma unroll
@@ -286,59 +363,101 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, int g, int id, double
   }
 }
 
+// Cooperative L2 prefetch: every item of tick t fetches its 1/IT share of the read-only inputs the NEXT tick
+// will read from HBM -- psi of group t+1 (A items) and C_part of group t-1 (C items of tick t+1) -- so that those
+// loads find their lines in L2.  Needs no ticket look-ahead, hence adds no dependency latency.
+template <int MODE>
+__device__ __forceinline__ void f3_prefetch_tick(const F3Mega& a, int tick, int r, int IT) {
+  const size_t M = (size_t)a.NX * F3_PLANE;
+  const long lines = (long)a.gs * 2 * M * 16 / 128;              // 128-byte lines of one group of one buffer
+  const long chunk = (lines + IT - 1) / IT, q0 = (long)r * chunk;
+  long q1 = q0 + chunk; if (q1 > lines) q1 = lines;
+  const int ga = tick + 1, gc = tick - 1;
+  if (ga < a.G) {
+    const long lim = (long)((a.n - ga * a.gs < a.gs) ? a.n - ga * a.gs : a.gs) * 2 * M * 16 / 128;
+    const char* base = (const char*)(a.psi + (size_t)ga * a.gs * 2 * M);
+    for (long q = q0 + threadIdx.x; q < q1 && q < lim; q += 128) f3_pf(base + q * 128);
+  }
+  if (MODE == F3_CORR && gc >= 0 && gc < a.G) {
+    const long lim = (long)((a.n - gc * a.gs < a.gs) ? a.n - gc * a.gs : a.gs) * 2 * M * 16 / 128;
+    const char* base = (const char*)(a.cpart + (size_t)gc * a.gs * 2 * M);
+    for (long q = q0 + threadIdx.x; q < q1 && q < lim; q += 128) f3_pf(base + q * 128);
+  }
+}
+
 // ---- the persistent kernel ----------------------------------------------------------------------------------
 template <bool SYM, int MODE>
-__global__ void __launch_bounds__(128, 3) k_f3_mega(F3Mega a) {
+__global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3_mega(F3Mega a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* tiles = reinterpret_cast<cplx*>(smem_raw);
-  __shared__ int s_item;
+  __shared__ int s_item[2];
   __shared__ double red[4 * F3_NPART];
   __shared__ double s_eps[32], s_sn[32];
   cplx x[F3_N];
+  const F3Pol pol = f3_policies();
   const int G = a.G, NX = a.NX;
   int* done = reinterpret_cast<int*>(a.sync + 1);
   const int nA = a.gs * 2 * NX / 4, nB = a.gs * 16, nC = SYM ? a.gs * NX : a.gs * NX / 2;
   const int nD = MODE == F3_APPLY ? 0 : NX * F3_DSPLIT;
   const int IT = nA + nB + nC + nD, total = (G + 3) * IT;
+  int t1 = 0;
+  if (threadIdx.x == 0) t1 = atomicAdd(&a.sync->next, 1);
   for (;;) {
-    if (threadIdx.x == 0) s_item = atomicAdd(&a.sync->next, 1);
+    F3_T0();
+    if (threadIdx.x == 0) s_item[0] = t1;
     __syncthreads();
-    const int item = s_item;
+    const int item = s_item[0];
     __syncthreads();
     if (item >= total) break;
     const int tick = item / IT, r = item - tick * IT;
+    bool drew = false;
+    f3_prefetch_tick<MODE>(a, tick, r, IT);
+    F3_T(4, 0);
     if (r < nA) {
       const int g = tick;
       if (g < G) {
         if (g >= F3_RING) f3_wait(&done[2 * G + g - F3_RING], nC, a.sync);
-        f3_body_a<SYM>(a, g, r, tiles, x);
-        f3_signal(&done[g]);
+        F3_T(4, 1);
+        f3_body_a<SYM>(a, pol, g, r, tiles, x);
+        F3_T0();
+        f3_signal(&done[g], &a.sync->next, t1); drew = true;
+        F3_T(4, 5);
       }
     } else if (r < nA + nB) {
       const int g = tick - 1;
       if (g >= 0 && g < G) {
         f3_wait(&done[g], nA, a.sync);
-        if (NX == 32) f3_body_b<32, SYM>(a, g, r - nA, x);
-        else if (NX == 16) f3_body_b<16, SYM>(a, g, r - nA, x);
-        else f3_body_b<8, SYM>(a, g, r - nA, x);
-        f3_signal(&done[G + g]);
+        F3_T(4, 2);
+        if (NX == 32) f3_body_b<32, SYM>(a, pol, g, r - nA, x);
+        else if (NX == 16) f3_body_b<16, SYM>(a, pol, g, r - nA, x);
+        else f3_body_b<8, SYM>(a, pol, g, r - nA, x);
+        F3_T0();
+        f3_signal(&done[G + g], &a.sync->next, t1); drew = true;
+        F3_T(4, 5);
       }
     } else if (r < nA + nB + nC) {
       const int g = tick - 2;
       if (g >= 0 && g < G) {
         f3_wait(&done[G + g], nB, a.sync);
         if (MODE != F3_APPLY && g >= F3_RING) f3_wait(&done[3 * G + g - F3_RING], nD, a.sync);
-        f3_body_c<SYM, MODE>(a, g, r - nA - nB, tiles, red, x);
-        f3_signal(&done[2 * G + g]);
+        F3_T(4, 3);
+        f3_body_c<SYM, MODE>(a, pol, g, r - nA - nB, tiles, red, x);
+        F3_T0();
+        f3_signal(&done[2 * G + g], &a.sync->next, t1); drew = true;
+        F3_T(4, 5);
       }
     } else {
       const int g = tick - 3;
       if (g >= 0 && g < G) {
         f3_wait(&done[2 * G + g], nC, a.sync);
         if (g >= F3_RING) f3_wait(&done[3 * G + g - F3_RING], nD, a.sync);
-        if (MODE != F3_APPLY) f3_body_d<MODE>(a, g, r - nA - nB - nC, s_eps, s_sn);
-        f3_signal(&done[3 * G + g]);
+        F3_T(4, 4);
+        if (MODE != F3_APPLY) f3_body_d<MODE>(a, pol, g, r - nA - nB - nC, s_eps, s_sn);
+        F3_T0();
+        f3_signal(&done[3 * G + g], &a.sync->next, t1); drew = true;
+        F3_T(4, 5);
       }
     }
+    if (!drew && threadIdx.x == 0) t1 = atomicAdd(&a.sync->next, 1);
   }
 }
