@@ -3,6 +3,8 @@
 Every check compares the oracle with something that is NOT the oracle: closed forms typed out here, dense
 matrices built with numpy from Eqs. 28a/b, numpy's eigh / FFT as independent third parties, conservation laws.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -548,6 +550,15 @@ def test_p13_uniform_unitary_gas_values():
     n, t, a = moments(mu - U, D)
     r = o.functional_point(n, n, t, t, a)
     assert abs(2 * n - rho) < 1e-9
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "eq12d_unitary_gas.txt")):
+        if line.strip() and not line.startswith("#"):
+            name, val, unc = line.split()
+            gold[name] = (float(val), float(unc))
+    assert alpha == gold["A_at_p0"][0]
+    # the paper's printed values with their printed uncertainty (+ the finite-cutoff shift of the gap, < 0.01)
+    assert abs(D / eF - gold["Delta_over_eF"][0]) <= gold["Delta_over_eF"][1] + 0.01, D / eF
+    assert abs(r["edens"] / (0.6 * rho * eF) - gold["E_over_EFG"][0]) <= gold["E_over_EFG"][1] + 0.01
     assert 0.49 <= D / eF <= 0.52, D / eF
     assert 0.38 <= r["edens"] / (0.6 * rho * eF) <= 0.41, r["edens"] / (0.6 * rho * eF)
     assert abs(mu / eF - r["edens"] / (0.6 * rho * eF)) < 0.02      # mu = xi eF at unitarity (thermodynamics)
