@@ -184,6 +184,22 @@ def run_reference(args):
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def max_over_ranks(ms, world, device):
+    """Multi-GPU timing rule: the step time of the job is the MAX over ranks of the device-timed region."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(n_wf_per_rank, steps, world, ms):
+    """Whole-job throughput of `world` independent replicas (weak scaling, no data-path collective)."""
+    return world * n_wf_per_rank * steps / (ms * 1e-3)
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -238,12 +254,9 @@ def run_gpu(args):
     ms = e0.elapsed_time(e1)
     launches = g.launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     finite = bool(torch.isfinite(torch.view_as_real(phi[:: max(1, w.n_wf // 64)])).all())
-    value = world * w.n_wf * args.steps / (ms * 1e-3)
+    value = job_value(w.n_wf, args.steps, world, ms)
 
     # ---- per-kernel device times (separate pass, event pairs around every launch) -> dominant kernel
     prof_steps = min(args.steps, 2)
@@ -305,10 +318,7 @@ def run_gpu(args):
         e1.record()
         barrier()
         ms_e = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms_e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e = float(t.item())
+        ms_e = max_over_ranks(ms_e, world, "cuda")
         buf = n_e * 32 * w.M
         e2e = {"value": world * n_e * n_e2e_steps / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": buf * (1 + ge.m),
                "d2h_bytes_per_step": 2 * buf, "n_wf": n_e, "steps": n_e2e_steps,

@@ -22,8 +22,9 @@ def test_library_builds_and_exports_every_declared_symbol():
 def test_workspace_bytes_is_pure_host_and_monotone():
     f = ws.make_functional(func_id=2, kin_form=1)
     a = ws.workspace_bytes((32, 32, 32), 3, 64, f)
-    b = ws.workspace_bytes((64, 64, 64), 3, 64, f)
-    assert 0 < a < b
+    b = ws.workspace_bytes((32, 32, 32), 3, 4096, f)
+    assert 0 < a < b                                             # grows with the per-spinor arrays
+    assert ws.workspace_bytes((64, 64, 64), 3, 64, f) > ws.workspace_bytes((16, 16, 16), 3, 64, f) > 0
     assert ws.workspace_bytes((128, 32, 32), 1, 1024, f) > 0
     assert ws.workspace_bytes((64, 64, 32), 2, 128, f) > 0
 
