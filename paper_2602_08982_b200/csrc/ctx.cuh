@@ -24,7 +24,7 @@ struct Plan {
   size_t off_fast, fast_spec_bytes, fast_part_bytes, fast_stream_bytes;
   // persistent dataflow kernels (mega3d.cuh): enabled flag, spinors per group, number of groups, ring buffers
   int mega, gs, mG;
-  size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes;
+  size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -99,13 +99,14 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
   if (P.gs > n_wf) P.gs = (int)n_wf;
   P.mG = (int)((n_wf + P.gs - 1) / P.gs);
-  P.off_mega = o; P.mega_ring_bytes = P.mega_part_bytes = P.mega_acc_bytes = P.mega_sync_bytes = 0;
+  P.off_mega = o; P.mega_ring_bytes = P.mega_part_bytes = P.mega_acc_bytes = P.mega_sync_bytes = P.mega_pack_bytes = 0;
   if (P.mega) {
     P.mega_ring_bytes = align_up((size_t)F3_RING * P.gs * 2 * M * 16);
     P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * P.N[0] * 8);
     P.mega_acc_bytes = align_up((size_t)F3_RING * 4 * M * 8);
     P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * P.mG * sizeof(int));
-    o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes;
+    P.mega_pack_bytes = align_up((size_t)M * 48);
+    o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
   P.total = o;
   return 0;
@@ -128,6 +129,7 @@ struct wslda_ctx {
   cplx *m_spec0, *m_spec1, *m_X;   // persistent-kernel rings
   double *m_part, *m_acc;
   F3Sync* m_sync;
+  cplx* m_pack;
   int mega_grid;
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -288,7 +290,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     b += 3 * P.mega_ring_bytes;
     c->m_part = (double*)b; b += P.mega_part_bytes;
     c->m_acc = (double*)b; b += P.mega_acc_bytes;
-    c->m_sync = (F3Sync*)b;
+    c->m_sync = (F3Sync*)b; b += P.mega_sync_bytes;
+    c->m_pack = (cplx*)b;
     int occ = 0, best = F3_MEGA_OCC;
 #define WS_MEGA_ATTR(K) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES); \
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, K, 128, 4 * F3_TILE_BYTES); if (occ > 0 && occ < best) best = occ; } while (0)

@@ -67,6 +67,8 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.acc = c->m_acc; a.sync = c->m_sync;
   a.n = (int)n; a.gs = P.gs; a.G = (int)((n + P.gs - 1) / P.gs); a.NX = P.N[0];
   cudaMemsetAsync(c->m_sync, 0, sizeof(F3Sync) + (size_t)4 * a.G * sizeof(int), st);
+  a.pack = c->m_pack;
+  LAUNCH(c, k_f3_pack, nb(P.M, 256), 256, 0, st, a.F, sym ? 1 : 0, P.M, c->m_pack);
   const int NX = P.N[0], nspec = sym ? 2 : 1;
   const int IT = a.gs * 2 * NX / 4 + a.gs * 16 + (sym ? a.gs * NX : a.gs * NX / 2) + (mode == F3_APPLY ? 0 : NX * F3_DSPLIT);
   const long total = (long)(a.G + 3) * IT;

@@ -39,6 +39,7 @@ struct F3Mega {
   const double* scale;         // per spinor (nullable)
   const double* kperp2;        // per spinor
   F3Fields F;
+  const cplx* pack;            // [M][3]: (q_a, q_b), Delta + Delta_ext, (alpha_a, alpha_b)  -- see k_f3_pack
   const double *ky2, *kz2;
   double kx2[32];
   double invM, dV, kappa;
@@ -54,6 +55,19 @@ struct F3Mega {
   F3Sync* sync;
   int n, gs, G, NX;
 };
+
+// Pointwise fields of H gathered per lattice point so that the C epilogue reads 2-3 16-byte words instead of
+// ten scattered ones: q_sigma = U_sigma - mu_sigma (+ lap(alpha_sigma) / 4 for the Eq. 40 form, whose
+// -(lap alpha) w / 4... term enters H with +1/4), D = Delta + Delta_ext, and alpha_sigma for the transverse shift.
+__global__ void k_f3_pack(F3Fields F, int sym, int64_t M, cplx* pack) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const double qa = F.U[0][i] - F.mu[0] + (sym ? 0.25 * F.lap[0][i] : 0.0);
+  const double qb = F.U[1][i] - F.mu[1] + (sym ? 0.25 * F.lap[1][i] : 0.0);
+  pack[3 * i] = make_double2(qa, qb);
+  pack[3 * i + 1] = cadd(F.delta[i], F.dext[i]);
+  pack[3 * i + 2] = make_double2(F.alpha[0][i], F.alpha[1][i]);
+}
 
 __device__ __forceinline__ cplx ldcg2(const cplx* p) { return __ldcg(p); }
 
@@ -111,8 +125,8 @@ __device__ __forceinline__ void f3_body_a(const F3Mega& a, const F3Pol& pol, int
   const double s = a.scale ? a.scale[n] : 1.0;
   const double* al = a.F.alpha[c] + (size_t)ix * F3_PLANE;
   const size_t sb = (((size_t)(g % F3_RING) * a.gs + nl) * 2 + c) * M + (size_t)ix * F3_PLANE;
-#pragma unroll 1
   F3_T0();
+#pragma unroll 1
   for (int t = 0; t < (SYM ? 2 : 1); ++t) {
 #pragma unroll
     for (int j = 0; j < F3_N; ++j) {
@@ -155,7 +169,6 @@ __device__ __forceinline__ void f3_body_b(const F3Mega& a, const F3Pol& pol, int
         x[j] = make_double2(x[j].x * f, -x[j].y * f);
       }
     }
-#pragma unroll
     F3_T(1, 1);
 #pragma unroll
     for (int j = 0; j < NX; ++j) st_pol(p + (size_t)j * F3_PLANE, x[j], pol.keep);
@@ -188,15 +201,8 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
       for (int q = lane; q < LW; q += 32) {
         f3_pf1(pu8 + q * 128); f3_pf1(pu8 + M * 16 + q * 128);
         if (MODE == F3_CORR) { f3_pf1(cu8 + q * 128); f3_pf1(cu8 + M * 16 + q * 128); }
-        f3_pf1((const char*)(a.F.delta + r0) + q * 128); f3_pf1((const char*)(a.F.dext + r0) + q * 128);
       }
-      for (int q = lane; q < LW / 2; q += 32) {
-        f3_pf1((const char*)(a.F.U[0] + r0) + q * 128); f3_pf1((const char*)(a.F.U[1] + r0) + q * 128);
-        if (SYM) {
-          f3_pf1((const char*)(a.F.alpha[0] + r0) + q * 128); f3_pf1((const char*)(a.F.alpha[1] + r0) + q * 128);
-          f3_pf1((const char*)(a.F.lap[0] + r0) + q * 128); f3_pf1((const char*)(a.F.lap[1] + r0) + q * 128);
-        }
-      }
+      for (int q = lane; q < 3 * LW; q += 32) f3_pf1((const char*)(a.pack + 3 * r0) + q * 128);
     }
     const cplx* sp = (t ? a.spec1 : a.spec0) + (ring + c) * M + pl;
 #pragma unroll
@@ -223,28 +229,26 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
     cplx* ou = (MODE == F3_APPLY ? a.out + (size_t)(2 * n) * M : a.X + ring * M) + pl;
     cplx* ov = ou + M;
     const cplx* cu = a.cpart + (size_t)(2 * n) * M + pl;
+    const cplx* pk = a.pack + 3 * pl;
 #pragma unroll 4
     for (int jj = 0; jj < ROWS; ++jj) {
       const int j = wl * ROWS + jj, i = j * F3_N + lane, si = j * F3_PITCH + lane;
       const cplx u = cscale(pu[i], s), v = cscale(pv[i], s);
       const cplx Lu = tb[(NS - 1) * TILE + si], Lv = tb[(2 * NS - 1) * TILE + si];
+      const cplx q = pk[3 * i], D = pk[3 * i + 1];
+      double ha = 0.5 * kp2, hb = 0.5 * kp2;
+      if (SYM && kp2 != 0.0) { const cplx al2 = pk[3 * i + 2]; ha *= al2.x; hb *= al2.y; }
       cplx Ku, Kv;
-      if (SYM) {
+      if (SYM) {                                                       // Eq. 40; its +(lap alpha) w / 4 term sits in q
         const cplx Tu = tb[si], Tv = tb[NS * TILE + si];
-        const double aa = a.F.alpha[0][pl + i], ab = a.F.alpha[1][pl + i], la = a.F.lap[0][pl + i], lb = a.F.lap[1][pl + i];
-        const double ha = 0.5 * aa * kp2, hb = 0.5 * ab * kp2;
-        Ku.x = -0.25 * (Lu.x + Tu.x - la * u.x) + ha * u.x;            // Eq. 40 + transverse shift
-        Ku.y = -0.25 * (Lu.y + Tu.y - la * u.y) + ha * u.y;
-        Kv.x = -0.25 * (Lv.x + Tv.x - lb * v.x) + hb * v.x;
-        Kv.y = -0.25 * (Lv.y + Tv.y - lb * v.y) + hb * v.y;
-      } else {
-        Ku = make_double2(-0.5 * Lu.x + 0.5 * kp2 * u.x, -0.5 * Lu.y + 0.5 * kp2 * u.y);     // Eq. 14
-        Kv = make_double2(-0.5 * Lv.x + 0.5 * kp2 * v.x, -0.5 * Lv.y + 0.5 * kp2 * v.y);
+        Ku = make_double2(-0.25 * (Lu.x + Tu.x) + ha * u.x, -0.25 * (Lu.y + Tu.y) + ha * u.y);
+        Kv = make_double2(-0.25 * (Lv.x + Tv.x) + hb * v.x, -0.25 * (Lv.y + Tv.y) + hb * v.y);
+      } else {                                                         // Eq. 14
+        Ku = make_double2(-0.5 * Lu.x + ha * u.x, -0.5 * Lu.y + ha * u.y);
+        Kv = make_double2(-0.5 * Lv.x + hb * v.x, -0.5 * Lv.y + hb * v.y);
       }
-      const cplx D = cadd(a.F.delta[pl + i], a.F.dext[pl + i]);
-      const double pa = a.F.U[0][pl + i] - a.F.mu[0], pb = a.F.U[1][pl + i] - a.F.mu[1];
-      const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                // Eqs. 5, 15
-      const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, pb)));
+      const cplx Hu = cadd(Ku, cadd(cscale(u, q.x), cmul(D, v)));                               // Eqs. 5, 15
+      const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, q.y)));
       e += u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
       if (MODE == F3_APPLY) { st_pol(ou + i, Hu, pol.drop); st_pol(ov + i, Hv, pol.drop); }
       else if (MODE == F3_RHS) { st_pol(ou + i, make_double2(Hu.y, -Hu.x), pol.keep); st_pol(ov + i, make_double2(Hv.y, -Hv.x), pol.keep); }   // -i H
