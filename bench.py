@@ -278,6 +278,13 @@ def run_gpu(args):
         roof = {"kernel": top, "bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                 "frac": ach / (fp64_peak / 1e12), "traffic": None,
                 "peak_source": "measured FP64 DFMA chain on this pool's B200 (DESIGN.md 7)"}
+    try:
+        tr = json.load(open(os.path.join(ROOT, "profiles", "r01_mega_traffic.json.txt")))
+        if top in tr["dram_bytes_per_spinor"]:
+            roof["traffic"] = tr["dram_bytes_per_spinor"][top] * w.n_wf * (top_cnt / prof_steps)
+            roof["traffic_source"] = tr["source"] + ", per-spinor DRAM bytes x n_wf"
+    except (OSError, ValueError, KeyError):
+        pass
     roof.update({"share_of_step": top_ms / tot_ms, "launches_per_step": top_cnt / prof_steps,
                  "avg_launch_ms": top_ms / top_cnt, "alg_bytes_per_launch": top_bytes / top_cnt,
                  "alg_flops_per_launch": top_flops / top_cnt})

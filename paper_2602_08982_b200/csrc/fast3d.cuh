@@ -308,11 +308,11 @@ __global__ void __launch_bounds__(128) k_f3_fin2(F3Fin2 a) {
 
 // densities of scale_n * psi for the spinors of a chunk (stage 1: the normalised predictor)
 struct F3DensOnly { const cplx* psi; const double* scale; int cnt; int64_t M; F3Dens d; };
-__global__ void __launch_bounds__(128) k_f3_dens(F3DensOnly a) {
+__global__ void __launch_bounds__(64) k_f3_dens(F3DensOnly a) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.M) return;
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll 4
+#pragma unroll 8
   for (int n = 0; n < a.cnt; ++n) {
     const double s = a.scale ? a.scale[n] : 1.0;
     const cplx u = cscale(a.psi[(int64_t)(2 * n) * a.M + i], s), v = cscale(a.psi[(int64_t)(2 * n + 1) * a.M + i], s);

@@ -141,7 +141,7 @@ static void f3_stage1(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int
   LAUNCH(c, k_abm_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, s.phi + off, h, s.cpart + off, s.k, P.M,
          c->f.normalize ? c->f_partn[q] : (double*)nullptr, P.nblk);
   if (c->f.normalize)
-    LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->f_partn[q], P.nblk, (int64_t)cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
+    LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->f_partn[q], P.nblk, (int64_t)cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
 }
 // Alg. 2 steps 3-4, 8: phi_new = C_part + c0 dt f(P), normalised, written over P (+ its densities)
 static void f3_stage2(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int64_t n0, int cnt, int do_dens, int first) {
@@ -197,7 +197,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
         d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
         d.d = f3_dens_args(c, q, n0, k < ns);
         WORK(c, 0, 0);
-        LAUNCH(c, k_f3_dens, nb(P.M, 128), 128, 0, st, d);
+        LAUNCH(c, k_f3_dens, nb(P.M, 64), 64, 0, st, d);
       }
     }
     f3_join(c, s);
@@ -229,7 +229,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
     F3DensOnly d;
     d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
     d.d = f3_dens_args(c, q, n0, k < ns);
-    LAUNCH(c, k_f3_dens, nb(P.M, 128), 128, 0, st, d);
+    LAUNCH(c, k_f3_dens, nb(P.M, 64), 64, 0, st, d);
   }
   f3_join(c, s);
   f3_dens_final(c, used, s.user);

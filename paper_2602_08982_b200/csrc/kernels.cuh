@@ -47,10 +47,14 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_norm_partials(const cplx* psi
 // scale_n = 1 / sqrt(dV * sum_blk part) (Eq. 16 with n = m), or eps_n = dV * sum_blk part (Eq. 44b)
 __global__ void k_from_partials(const double* part, int nblk, int64_t n_count, double dV, int as_scale, double* out,
                                 double* out2) {
-  int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  // one warp per spinor: lanes take the partials in stride-32 order, then a fixed shuffle tree (deterministic)
+  const int64_t n = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   if (n >= n_count) return;
   double s = 0.0;
-  for (int b = 0; b < nblk; ++b) s += part[n * nblk + b];
+  for (int b = lane; b < nblk; b += 32) s += part[n * nblk + b];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane) return;
   double r = as_scale ? 1.0 / sqrt(s * dV) : s * dV;
   out[n] = r;
   if (out2) out2[n] = r;

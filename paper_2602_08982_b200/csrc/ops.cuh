@@ -193,7 +193,7 @@ extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
     const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
     h_chunk(c, psi + 2 * n0 * M, nullptr, n0, cnt, hpsi + 2 * n0 * M, true, st);
-    LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->part_e, c->P.nblk, cnt, c->dV, 0, c->eps + n0,
+    LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->part_e, c->P.nblk, cnt, c->dV, 0, c->eps + n0,
            eps_dev ? eps_dev + n0 : nullptr);
   }
   return cuda_check(c, "apply_h");

@@ -35,11 +35,11 @@ static void rebuild(wslda_ctx* c, const cplx* psi, const double* scale, cudaStre
 // eps_n of the chunk from the partials of the last h_chunk (null when the shift of Eq. 44 is off)
 static const double* eps_chunk(wslda_ctx* c, int64_t n0, int64_t cnt, cudaStream_t st) {
   if (!c->f.subtract_mean_energy) return nullptr;
-  LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->part_e, c->P.nblk, cnt, c->dV, 0, c->eps + n0, (double*)nullptr);
+  LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->part_e, c->P.nblk, cnt, c->dV, 0, c->eps + n0, (double*)nullptr);
   return c->eps + n0;
 }
 static void scale_chunk_from_partials(wslda_ctx* c, int64_t n0, int64_t cnt, cudaStream_t st) {
-  LAUNCH(c, k_from_partials, nb(cnt, 128), 128, 0, st, c->part_n, c->P.nblk, cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
+  LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->part_n, c->P.nblk, cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
 }
 
 // f = -i (H - eps) psi for the chunk; psi_chunk in the caller's buffer, scaled on the fly; the scaled state is
