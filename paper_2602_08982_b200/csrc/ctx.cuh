@@ -23,6 +23,9 @@ struct Plan {
   int fast, fc, ns;
   size_t off_fast, fast_spec_bytes, fast_part_bytes, fast_stream_bytes;
   // persistent dataflow kernels (mega3d.cuh): enabled flag, spinors per group, number of groups, ring buffers
+  // fused on-chip stages (onchip_step.cuh): enabled flag, spinors per CTA batch, persistent grid, density partials
+  int oc, ocS, oc_grid;
+  size_t off_oc, oc_dpart_bytes;
   int mega, gs, mG;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
@@ -108,6 +111,13 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_pack_bytes = align_up((size_t)M * 48);
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
+  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
+  if (const char* e = getenv("WSLDA_ONCHIP")) if (atoi(e) == 0) P.oc = 0;
+  { int64_t S = 8192 / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
+  { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS; P.oc_grid = (int)(nb_ < 148 ? nb_ : 148); }
+  if (const char* e = getenv("WSLDA_ONCHIP_CTAS")) { int v = atoi(e); if (v > 0 && v < P.oc_grid) P.oc_grid = v; }
+  P.off_oc = o; P.oc_dpart_bytes = 0;
+  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 256 ? M : 256) * 8); o += P.oc_dpart_bytes; }
   P.total = o;
   return 0;
 }
@@ -130,6 +140,7 @@ struct wslda_ctx {
   double *m_part, *m_acc;
   F3Sync* m_sync;
   cplx* m_pack;
+  double* oc_dpart;
   int mega_grid;
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -303,6 +314,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->mega_grid = best * sms;
     if (const char* e = getenv("WSLDA_MEGA_CTAS")) { int v = atoi(e); if (v > 0) c->mega_grid = v; }
   }
+  if (P.oc) c->oc_dpart = (double*)(base + P.off_oc);
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
   cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);
   const int T = 256;

@@ -149,6 +149,18 @@ __global__ void k_potentials(FuncParams P, const double* raw, const double* vext
   lambda[i] = lam; geff[i] = g; delta[i] = D;
 }
 
+// same sums for many groups (small lattices: G ~ 1000): one warp per (plane, point), lanes stride over the groups and
+// finish with the fixed shuffle tree -- still deterministic, G-fold more parallel.  grid (ceil(M / 8), DP_COUNT) x 256
+__global__ void k_density_reduce_wide(const double* part, int G, double* raw, int64_t M, unsigned mask, int accumulate) {
+  const int64_t i = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int f = blockIdx.y, lane = threadIdx.x & 31;
+  if (i >= M || !(mask & plane_bit(f))) return;
+  double s = 0.0;
+  for (int g = lane; g < G; g += 32) s += part[((int64_t)g * DP_COUNT + f) * M + i];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane == 0) raw[f * M + i] = (accumulate ? raw[f * M + i] : 0.0) + s;
+}
+
 // folded density field for wslda_get_field
 __global__ void k_get_density(const double* raw, int64_t M, int sym, int field_id, double* dst) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

@@ -2,7 +2,7 @@
 // Alg. 2 step as chunk pipelines on up to four concurrent streams so that the passes of
 // different chunks overlap (HBM-bound, L2-bound and FP64-bound phases run side by side on the SMs).
 #pragma once
-#include "ops.cuh"
+#include "onchip_step.cuh"
 
 static F3Fields f3_fields(const wslda_ctx* c) {
   F3Fields F;

@@ -1,0 +1,234 @@
+// onchip_step.cuh -- fused ABM stage kernels for lattices whose spinors fit in shared memory (M <= 4096 points:
+// the quasi-1D / quasi-2D modes and small 3-D boxes; configs[0..2]) with the Eq. 14 kinetic operator.
+// A CTA keeps a batch of S spinors (S * 2 * M <= 8192 complex128 = 128 KB) on chip for the whole stage:
+//   load psi -> forward FFT over the held axes -> -k^2/M (Eq. 26) -> inverse FFT, all in place,
+//   pointwise BdG mix (Eqs. 5, 15) -> eps_n = Re <psi|H psi> reduced inside the CTA (Eq. 44b) ->
+//   RHS : f = -i (H - eps) psi written once                                        (Alg. 2 step 9)
+//   CORR: phi_new = C_part + c0 dt f, its norm reduced inside the CTA, normalised, written once over P,
+//         and the densities of phi_new accumulated per CTA in registers             (Alg. 2 steps 3-4, 8)
+// so a stage is ONE HBM round trip (read psi [+ C_part], write the result) with no scratch traffic at all.
+// Density partials [CTA][4][slots] are summed in a fixed order afterwards: bit-reproducible.
+#pragma once
+#include "ops.cuh"
+
+enum { OC_APPLY = 0, OC_CORR = 1, OC_RHS = 2 };
+#define OC_THREADS 256
+#define OC_MAXS 64
+#define OC_MAXPT 16            // lattice points per thread: max(1, M / 256)
+
+struct OCArgs {
+  Lat L;
+  const cplx* psi;             // [n][2][M], first spinor of the call
+  const double* scale;         // per spinor, nullable
+  const double* kperp2;
+  Fields F;
+  cplx* out;                   // APPLY: H psi; RHS: f; CORR: phi_new (may alias psi)
+  const cplx* cpart;
+  double kappa, dV;
+  int use_shift, normalize;
+  double* eps_out;             // nullable: true eps_n
+  int do_dens;
+  const double *cpref, *w_a, *w_b;
+  double* dpart;               // [gridDim.x][4][slots], slots = max(M, 256)
+  int64_t n;
+  int S;
+};
+
+// per-spinor sums of E[s][i] over the lattice: warp w takes spinors w, w + 8, ...; fixed order
+__device__ __forceinline__ void oc_reduce(const double* E, int cnt, int lgM, double* out_s) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, M = 1 << lgM;
+  for (int s = warp; s < cnt; s += OC_THREADS / 32) {
+    double v = 0.0;
+    for (int i = lane; i < M; i += 32) v += E[(s << lgM) + i];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) out_s[s] = v;
+  }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Lat& L = a.L;
+  const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x;
+  cplx* F = reinterpret_cast<cplx*>(smem_raw);                       // [S][2][M]
+  double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);       // [S][M]
+  __shared__ double s_eps[OC_MAXS], s_sn[OC_MAXS];
+  // slots of this thread: lattice points i(kk) = (tid + 256 kk) & (M - 1), kk < PT; spinors s0, s0 + SSTEP, ...
+  const int PT = M >= OC_THREADS ? M / OC_THREADS : 1;
+  const int SSTEP = M >= OC_THREADS ? 1 : OC_THREADS / M, s0 = M >= OC_THREADS ? 0 : tid >> lgM;
+  double acc[OC_MAXPT][4];
+#pragma unroll
+  for (int kk = 0; kk < OC_MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
+  const int64_t n_batches = (a.n + S - 1) / S;
+  for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
+    const int64_t n0 = b * S;
+    const int cnt = (int)((a.n - n0 < S) ? a.n - n0 : S);
+    const int tot = S * 2 * M, used = cnt * 2 * M;
+    const cplx* src = a.psi + (size_t)n0 * 2 * M;
+    for (int idx = tid; idx < tot; idx += OC_THREADS) {
+      cplx v = make_double2(0.0, 0.0);
+      if (idx < used) { v = src[idx]; if (a.scale) v = cscale(v, a.scale[n0 + (idx >> (lgM + 1))]); }
+      F[idx] = v;
+    }
+    __syncthreads();
+    const int G = 2 * S;
+    if (L.nd > 2) fft_axis<false>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
+    if (L.nd > 1) fft_axis<false>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
+    fft_axis<false>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
+    for (int idx = tid; idx < used; idx += OC_THREADS) {
+      const int i = idx & (M - 1);
+      const int j2 = i & (L.N[2] - 1), j1 = (i >> L.lg[2]) & (L.N[1] - 1), j0 = i >> (L.lg[1] + L.lg[2]);
+      F[idx] = cscale(F[idx], kfactor(L, 0, j0, j1, j2).x);          // -k^2 / M at the stored (digit-reversed) position
+    }
+    __syncthreads();
+    fft_axis<true>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
+    if (L.nd > 1) fft_axis<true>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
+    if (L.nd > 2) fft_axis<true>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
+    // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order)
+    for (int kk = 0; kk < PT; ++kk) {
+      const int i = (tid + OC_THREADS * kk) & (M - 1);
+      const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
+      const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b;
+      for (int s = s0; s < cnt; s += SSTEP) {
+        const int64_t n = n0 + s;
+        const double sc = a.scale ? a.scale[n] : 1.0, kp2 = a.kperp2[n];
+        const cplx u = cscale(src[(size_t)(2 * s) * M + i], sc), v = cscale(src[(size_t)(2 * s + 1) * M + i], sc);
+        const cplx lu = F[(2 * s) * M + i], lv = F[(2 * s + 1) * M + i];
+        const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
+        const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
+        const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                    // Eqs. 5, 15
+        const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, pb)));
+        E[(s << lgM) + i] = u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
+        if (MODE == OC_APPLY) {
+          a.out[(size_t)(2 * n) * M + i] = Hu; a.out[(size_t)(2 * n + 1) * M + i] = Hv;
+        } else {
+          F[(2 * s) * M + i] = Hu; F[(2 * s + 1) * M + i] = Hv;
+        }
+      }
+    }
+    __syncthreads();
+    oc_reduce(E, cnt, lgM, s_eps);
+    __syncthreads();
+    if (tid < cnt) {
+      const double e_true = a.dV * s_eps[tid];
+      if (a.eps_out) a.eps_out[n0 + tid] = e_true;
+      s_eps[tid] = (a.use_shift && MODE != OC_APPLY) ? e_true : 0.0;
+    }
+    __syncthreads();
+    if (MODE != OC_APPLY) {
+      // ---- phase 2: f = -i (H - eps) psi;  RHS writes it, CORR forms phi_new = C_part + kappa f in place
+      for (int kk = 0; kk < PT; ++kk) {
+        const int i = (tid + OC_THREADS * kk) & (M - 1);
+        for (int s = s0; s < cnt; s += SSTEP) {
+          const int64_t n = n0 + s;
+          const double sc = a.scale ? a.scale[n] : 1.0, e = s_eps[s];
+          const cplx u = cscale(src[(size_t)(2 * s) * M + i], sc), v = cscale(src[(size_t)(2 * s + 1) * M + i], sc);
+          const cplx Hu = F[(2 * s) * M + i], Hv = F[(2 * s + 1) * M + i];
+          const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
+          if (MODE == OC_RHS) {
+            a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
+          } else {
+            const cplx cu = a.cpart[(size_t)(2 * n) * M + i], cv = a.cpart[(size_t)(2 * n + 1) * M + i];
+            const cplx pu = make_double2(cu.x + a.kappa * fu.x, cu.y + a.kappa * fu.y);
+            const cplx pv = make_double2(cv.x + a.kappa * fv.x, cv.y + a.kappa * fv.y);
+            F[(2 * s) * M + i] = pu; F[(2 * s + 1) * M + i] = pv;
+            E[(s << lgM) + i] = cabs2(pu) + cabs2(pv);
+          }
+        }
+      }
+    }
+    if (MODE == OC_CORR) {
+      __syncthreads();
+      oc_reduce(E, cnt, lgM, s_sn);
+      __syncthreads();
+      if (tid < cnt) s_sn[tid] = a.normalize ? 1.0 / sqrt(a.dV * s_sn[tid]) : 1.0;
+      __syncthreads();
+      // ---- phase 3: normalise (Alg. 2 step 8), write phi_new once, accumulate its densities (Eqs. 7a, 7b, 7e)
+#pragma unroll
+      for (int kk = 0; kk < OC_MAXPT; ++kk) {
+        if (kk < PT) {
+          const int i = (tid + OC_THREADS * kk) & (M - 1);
+          for (int s = s0; s < cnt; s += SSTEP) {
+            const int64_t n = n0 + s;
+            const double sn = s_sn[s];
+            const cplx u = cscale(F[(2 * s) * M + i], sn), v = cscale(F[(2 * s + 1) * M + i], sn);
+            a.out[(size_t)(2 * n) * M + i] = u; a.out[(size_t)(2 * n + 1) * M + i] = v;
+            if (a.do_dens) {
+              const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n], wn = 0.5 * cp * (wb - wa);
+              acc[kk][0] += cp * wa * cabs2(u);
+              acc[kk][1] += cp * wb * cabs2(v);
+              acc[kk][2] += wn * (u.x * v.x + u.y * v.y);
+              acc[kk][3] += wn * (u.y * v.x - u.x * v.y);
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (MODE == OC_CORR && a.do_dens) {
+    const int slots = PT * OC_THREADS;
+    double* dp = a.dpart + (size_t)blockIdx.x * 4 * slots;
+#pragma unroll
+    for (int kk = 0; kk < OC_MAXPT; ++kk)
+      if (kk < PT)
+#pragma unroll
+        for (int f = 0; f < 4; ++f) dp[f * slots + tid + OC_THREADS * kk] = acc[kk][f];
+  }
+}
+
+// raw[f][i] = sum over CTAs and duplicate slots of a lattice point, in a fixed order (one warp per output)
+__global__ void k_oc_dens_final(const double* dpart, int n_cta, int slots, int64_t M, double* raw) {
+  const int64_t o = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (o >= 4 * M) return;
+  const int f = (int)(o / M); const int64_t i = o - f * M;
+  const int dup = (int)(slots / M), terms = n_cta * dup;
+  double s = 0.0;
+  for (int t = lane; t < terms; t += 32) {
+    const int cta = t / dup, d = t - cta * dup;
+    s += dpart[((size_t)cta * 4 + f) * slots + i + (int64_t)d * M];
+  }
+  for (int k = 16; k > 0; k >>= 1) s += __shfl_xor_sync(0xffffffffu, s, k);
+  if (lane == 0) raw[o] = s;
+}
+
+// ---- host side ------------------------------------------------------------------------------------------------
+static bool g_oc_attr_done = false;
+static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, const double* scale, int64_t n0, int64_t n,
+                      cplx* out, const cplx* cpart, double kappa, int do_dens, double* eps_user) {
+  const Plan& P = c->P;
+  OCArgs a;
+  a.L = c->L; a.psi = psi; a.scale = scale; a.kperp2 = c->kperp2 + n0; a.F = fields_of(c);
+  a.out = out; a.cpart = cpart; a.kappa = kappa; a.dV = c->dV;
+  a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.eps_out = eps_user;
+  a.do_dens = do_dens; a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.dpart = c->oc_dpart;
+  a.n = n; a.S = P.ocS;
+  const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
+  if (!g_oc_attr_done) {
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    g_oc_attr_done = true;
+  }
+  const int64_t nbat = (n + P.ocS - 1) / P.ocS;
+  const int grid = (int)(nbat < P.oc_grid ? nbat : P.oc_grid);
+  const double lgM = (double)(P.lg[0] + P.lg[1] + P.lg[2]);
+  WORK(c, 32.0 * P.M * n * (mode == OC_CORR ? 3.0 : 2.0), 5.0 * P.M * lgM * 2.0 * 2.0 * n);
+  if (mode == OC_APPLY) LAUNCHN(c, "k_onchip_apply", k_onchip_stage<OC_APPLY>, grid, OC_THREADS, smem, st, a);
+  else if (mode == OC_CORR) LAUNCHN(c, "k_onchip_corr", k_onchip_stage<OC_CORR>, grid, OC_THREADS, smem, st, a);
+  else LAUNCHN(c, "k_onchip_rhs", k_onchip_stage<OC_RHS>, grid, OC_THREADS, smem, st, a);
+  if (mode == OC_CORR && do_dens) {
+    const int slots = (int)(P.M > 256 ? P.M : 256);
+    LAUNCH(c, k_oc_dens_final, nb(4 * P.M * 32, 256), 256, 0, st, c->oc_dpart, grid, slots, P.M, c->raw);
+  }
+}
+
+static wslda_status oc_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
+                               cudaStream_t st) {
+  const int64_t M = c->P.M;
+  if (n_count > 0)
+    oc_launch(c, st, OC_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0,
+              eps_dev ? eps_dev + n_first : c->eps + n_first);
+  return cuda_check(c, "apply_h");
+}

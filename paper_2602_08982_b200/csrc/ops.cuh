@@ -142,6 +142,9 @@ extern "C" wslda_status wslda_set_field(wslda_ctx* c, int id, const void* src, v
 static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
                                cudaStream_t st);
 
+static wslda_status oc_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
+                               cudaStream_t st);
+
 static Fields fields_of(const wslda_ctx* c) {
   Fields F;
   F.alpha_a = c->alpha_a; F.alpha_b = c->alpha_b; F.lap_a = c->lap_a; F.lap_b = c->lap_b; F.U_a = c->U_a; F.U_b = c->U_b;
@@ -190,6 +193,7 @@ extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi
   const int64_t M = c->P.M;
   cudaStream_t st = S(stream);
   if (c->P.fast) return f3_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
+  if (c->P.oc) return oc_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
     const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
     h_chunk(c, psi + 2 * n0 * M, nullptr, n0, cnt, hpsi + 2 * n0 * M, true, st);
@@ -219,7 +223,8 @@ static void dens_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_
   d.w_a = c->w_a + n0; d.w_b = c->w_b + n0; d.nd = P.nd; d.M = M; d.n_count = cnt; d.per_group = per; d.mask = mask;
   WORK(c, 32.0 * M * cnt, 0);
   LAUNCH(c, k_density, dim3(P.nblk, (unsigned)G), P.pt_threads, 0, st, d, c->dpart);
-  LAUNCH(c, k_density_reduce, dim3(nb(M, 256), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
+  if (G > 16) LAUNCH(c, k_density_reduce_wide, dim3(nb(M, 8), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
+  else LAUNCH(c, k_density_reduce, dim3(nb(M, 256), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
 }
 
 extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t n_first, int64_t n_count, unsigned mask,
