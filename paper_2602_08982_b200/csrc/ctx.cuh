@@ -113,11 +113,12 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   }
   P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
   if (const char* e = getenv("WSLDA_ONCHIP")) if (atoi(e) == 0) P.oc = 0;
-  { int64_t S = 8192 / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
-  { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS; P.oc_grid = (int)(nb_ < 148 ? nb_ : 148); }
+  // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
+  { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
+  { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS, cap = M <= 512 ? 296 : 148; P.oc_grid = (int)(nb_ < cap ? nb_ : cap); }
   if (const char* e = getenv("WSLDA_ONCHIP_CTAS")) { int v = atoi(e); if (v > 0 && v < P.oc_grid) P.oc_grid = v; }
   P.off_oc = o; P.oc_dpart_bytes = 0;
-  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 256 ? M : 256) * 8); o += P.oc_dpart_bytes; }
+  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes; }
   P.total = o;
   return 0;
 }

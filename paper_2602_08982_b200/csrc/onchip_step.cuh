@@ -12,9 +12,7 @@
 #include "ops.cuh"
 
 enum { OC_APPLY = 0, OC_CORR = 1, OC_RHS = 2 };
-#define OC_THREADS 256
-#define OC_MAXS 64
-#define OC_MAXPT 16            // lattice points per thread: max(1, M / 256)
+#define OC_MAXS 64              // spinors per CTA batch (s_eps / s_sn arrays)
 
 struct OCArgs {
   Lat L;
@@ -37,7 +35,7 @@ struct OCArgs {
 // per-spinor sums of E[s][i] over the lattice: warp w takes spinors w, w + 8, ...; fixed order
 __device__ __forceinline__ void oc_reduce(const double* E, int cnt, int lgM, double* out_s) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, M = 1 << lgM;
-  for (int s = warp; s < cnt; s += OC_THREADS / 32) {
+  for (int s = warp; s < cnt; s += (blockDim.x >> 5)) {
     double v = 0.0;
     for (int i = lane; i < M; i += 32) v += E[(s << lgM) + i];
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -45,27 +43,29 @@ __device__ __forceinline__ void oc_reduce(const double* E, int cnt, int lgM, dou
   }
 }
 
-template <int MODE>
-__global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
+// MAXPT = compile-time bound on the lattice points per thread, max(1, M / blockDim.x): 2 (256 threads, M <= 512,
+// two CTAs per SM) or 8 (512 threads for M up to 4096, one CTA per SM)
+template <int MODE, int MAXPT>
+__global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_stage(OCArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Lat& L = a.L;
-  const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x;
+  const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x, NT = blockDim.x;
   cplx* F = reinterpret_cast<cplx*>(smem_raw);                       // [S][2][M]
   double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);       // [S][M]
   __shared__ double s_eps[OC_MAXS], s_sn[OC_MAXS];
   // slots of this thread: lattice points i(kk) = (tid + 256 kk) & (M - 1), kk < PT; spinors s0, s0 + SSTEP, ...
-  const int PT = M >= OC_THREADS ? M / OC_THREADS : 1;
-  const int SSTEP = M >= OC_THREADS ? 1 : OC_THREADS / M, s0 = M >= OC_THREADS ? 0 : tid >> lgM;
-  double acc[OC_MAXPT][4];
+  const int PT = M >= NT ? M / NT : 1;
+  const int SSTEP = M >= NT ? 1 : NT / M, s0 = M >= NT ? 0 : tid >> lgM;
+  double acc[MAXPT][4];
 #pragma unroll
-  for (int kk = 0; kk < OC_MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
+  for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
   const int64_t n_batches = (a.n + S - 1) / S;
   for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const int64_t n0 = b * S;
     const int cnt = (int)((a.n - n0 < S) ? a.n - n0 : S);
     const int tot = S * 2 * M, used = cnt * 2 * M;
     const cplx* src = a.psi + (size_t)n0 * 2 * M;
-    for (int idx = tid; idx < tot; idx += OC_THREADS) {
+    for (int idx = tid; idx < tot; idx += NT) {
       cplx v = make_double2(0.0, 0.0);
       if (idx < used) { v = src[idx]; if (a.scale) v = cscale(v, a.scale[n0 + (idx >> (lgM + 1))]); }
       F[idx] = v;
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
     if (L.nd > 2) fft_axis<false>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
     if (L.nd > 1) fft_axis<false>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
     fft_axis<false>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
-    for (int idx = tid; idx < used; idx += OC_THREADS) {
+    for (int idx = tid; idx < used; idx += NT) {
       const int i = idx & (M - 1);
       const int j2 = i & (L.N[2] - 1), j1 = (i >> L.lg[2]) & (L.N[1] - 1), j0 = i >> (L.lg[1] + L.lg[2]);
       F[idx] = cscale(F[idx], kfactor(L, 0, j0, j1, j2).x);          // -k^2 / M at the stored (digit-reversed) position
@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
     if (L.nd > 2) fft_axis<true>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
     // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order)
     for (int kk = 0; kk < PT; ++kk) {
-      const int i = (tid + OC_THREADS * kk) & (M - 1);
+      const int i = (tid + NT * kk) & (M - 1);
       const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
       const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b;
       for (int s = s0; s < cnt; s += SSTEP) {
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
     if (MODE != OC_APPLY) {
       // ---- phase 2: f = -i (H - eps) psi;  RHS writes it, CORR forms phi_new = C_part + kappa f in place
       for (int kk = 0; kk < PT; ++kk) {
-        const int i = (tid + OC_THREADS * kk) & (M - 1);
+        const int i = (tid + NT * kk) & (M - 1);
         for (int s = s0; s < cnt; s += SSTEP) {
           const int64_t n = n0 + s;
           const double sc = a.scale ? a.scale[n] : 1.0, e = s_eps[s];
@@ -145,9 +145,9 @@ __global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
       __syncthreads();
       // ---- phase 3: normalise (Alg. 2 step 8), write phi_new once, accumulate its densities (Eqs. 7a, 7b, 7e)
 #pragma unroll
-      for (int kk = 0; kk < OC_MAXPT; ++kk) {
+      for (int kk = 0; kk < MAXPT; ++kk) {
         if (kk < PT) {
-          const int i = (tid + OC_THREADS * kk) & (M - 1);
+          const int i = (tid + NT * kk) & (M - 1);
           for (int s = s0; s < cnt; s += SSTEP) {
             const int64_t n = n0 + s;
             const double sn = s_sn[s];
@@ -167,13 +167,117 @@ __global__ void __launch_bounds__(OC_THREADS, 1) k_onchip_stage(OCArgs a) {
     __syncthreads();
   }
   if (MODE == OC_CORR && a.do_dens) {
-    const int slots = PT * OC_THREADS;
+    const int slots = PT * NT;
     double* dp = a.dpart + (size_t)blockIdx.x * 4 * slots;
 #pragma unroll
-    for (int kk = 0; kk < OC_MAXPT; ++kk)
+    for (int kk = 0; kk < MAXPT; ++kk)
       if (kk < PT)
 #pragma unroll
-        for (int f = 0; f < 4; ++f) dp[f * slots + tid + OC_THREADS * kk] = acc[kk][f];
+        for (int f = 0; f < 4; ++f) dp[f * slots + tid + NT * kk] = acc[kk][f];
+  }
+}
+
+// Alg. 2 steps 1-2 on chip: P = phi + dt sum b_i f_i and C_part = phi + dt sum_{i>=1} c_i f_i in one
+// sweep over phi and the history, |P| reduced inside the CTA, the NORMALISED predictor written over phi, C_part over
+// the oldest history buffer, and the densities of the predictor accumulated per CTA: 5 reads + 2 writes, nothing else.
+struct OCPred {
+  Lat L;
+  cplx* phi; HistPtrs h; cplx* cpart; AbmCoef k;
+  double dV; int normalize;
+  int do_dens; const double *cpref, *w_a, *w_b; double* dpart;
+  int64_t n; int S;
+};
+
+template <int MAXPT>
+__global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_pred(OCPred a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Lat& L = a.L;
+  const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x, NT = blockDim.x;
+  cplx* F = reinterpret_cast<cplx*>(smem_raw);
+  double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);
+  __shared__ double s_sn[OC_MAXS];
+  const int PT = M >= NT ? M / NT : 1;
+  const int SSTEP = M >= NT ? 1 : NT / M, s0 = M >= NT ? 0 : tid >> lgM;
+  double acc[MAXPT][4];
+#pragma unroll
+  for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
+  const int64_t n_batches = (a.n + S - 1) / S;
+  for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
+    const int64_t n0 = b * S;
+    const int cnt = (int)((a.n - n0 < S) ? a.n - n0 : S);
+    // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP); two slots per round so that 2 x 2 x (1 + m)
+    // independent 16-byte loads are in flight before the first use
+    const int nsp = cnt > s0 ? (cnt - s0 + SSTEP - 1) / SSTEP : 0, W = PT * nsp;
+    for (int w0 = 0; w0 < W; w0 += 2) {
+      cplx ph[2][2], fh[2][2][5];
+      size_t off[2][2];
+      int si[2], ii[2];
+#pragma unroll
+      for (int r = 0; r < 2; ++r) {
+        const int w = w0 + r < W ? w0 + r : W - 1;               // the tail repeats the last slot (harmless: same values)
+        ii[r] = (tid + NT * (w % PT)) & (M - 1); si[r] = s0 + (w / PT) * SSTEP;
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+          off[r][cc] = (size_t)(2 * (n0 + si[r]) + cc) * M + ii[r];
+          ph[r][cc] = __ldg(a.phi + off[r][cc]);
+#pragma unroll
+          for (int j = 0; j < 5; ++j)
+            if (j < a.k.ab || j + 1 < a.k.am) fh[r][cc][j] = __ldg(a.h.f[j] + off[r][cc]);
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 2; ++r) {
+        if (w0 + r >= W) break;
+        double nrm = 0.0;
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc) {
+          cplx p = ph[r][cc], q = p;
+#pragma unroll
+          for (int j = 0; j < 5; ++j) {
+            if (j < a.k.ab) { p.x += a.k.b[j] * fh[r][cc][j].x; p.y += a.k.b[j] * fh[r][cc][j].y; }
+            if (j + 1 < a.k.am) { q.x += a.k.c[j + 1] * fh[r][cc][j].x; q.y += a.k.c[j + 1] * fh[r][cc][j].y; }
+          }
+          a.cpart[off[r][cc]] = q;
+          F[(2 * si[r] + cc) * M + ii[r]] = p;
+          nrm += cabs2(p);
+        }
+        E[(si[r] << lgM) + ii[r]] = nrm;
+      }
+    }
+    __syncthreads();
+    oc_reduce(E, cnt, lgM, s_sn);
+    __syncthreads();
+    if (tid < cnt) s_sn[tid] = a.normalize ? 1.0 / sqrt(a.dV * s_sn[tid]) : 1.0;
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < MAXPT; ++kk) {
+      if (kk < PT) {
+        const int i = (tid + NT * kk) & (M - 1);
+        for (int s = s0; s < cnt; s += SSTEP) {
+          const int64_t n = n0 + s;
+          const double sn = s_sn[s];
+          const cplx u = cscale(F[(2 * s) * M + i], sn), v = cscale(F[(2 * s + 1) * M + i], sn);
+          a.phi[(size_t)(2 * n) * M + i] = u; a.phi[(size_t)(2 * n + 1) * M + i] = v;
+          if (a.do_dens) {
+            const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n], wn = 0.5 * cp * (wb - wa);
+            acc[kk][0] += cp * wa * cabs2(u);
+            acc[kk][1] += cp * wb * cabs2(v);
+            acc[kk][2] += wn * (u.x * v.x + u.y * v.y);
+            acc[kk][3] += wn * (u.y * v.x - u.x * v.y);
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (a.do_dens) {
+    const int slots = PT * NT;
+    double* dp = a.dpart + (size_t)blockIdx.x * 4 * slots;
+#pragma unroll
+    for (int kk = 0; kk < MAXPT; ++kk)
+      if (kk < PT)
+#pragma unroll
+        for (int f = 0; f < 4; ++f) dp[f * slots + tid + NT * kk] = acc[kk][f];
   }
 }
 
@@ -206,20 +310,26 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   a.n = n; a.S = P.ocS;
   const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
   if (!g_oc_attr_done) {
-    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    cudaFuncSetAttribute(k_onchip_stage<OC_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    cudaFuncSetAttribute(k_onchip_stage<OC_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     g_oc_attr_done = true;
   }
+  const bool small = P.M <= 512;
+  const int NT = small ? 256 : 512;
   const int64_t nbat = (n + P.ocS - 1) / P.ocS;
   const int grid = (int)(nbat < P.oc_grid ? nbat : P.oc_grid);
   const double lgM = (double)(P.lg[0] + P.lg[1] + P.lg[2]);
   WORK(c, 32.0 * P.M * n * (mode == OC_CORR ? 3.0 : 2.0), 5.0 * P.M * lgM * 2.0 * 2.0 * n);
-  if (mode == OC_APPLY) LAUNCHN(c, "k_onchip_apply", k_onchip_stage<OC_APPLY>, grid, OC_THREADS, smem, st, a);
-  else if (mode == OC_CORR) LAUNCHN(c, "k_onchip_corr", k_onchip_stage<OC_CORR>, grid, OC_THREADS, smem, st, a);
-  else LAUNCHN(c, "k_onchip_rhs", k_onchip_stage<OC_RHS>, grid, OC_THREADS, smem, st, a);
+  void (*k)(OCArgs);
+  if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
+  else k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8> : k_onchip_stage<OC_RHS, 8>;
+  LAUNCHN(c, mode == OC_APPLY ? "k_onchip_apply" : mode == OC_CORR ? "k_onchip_corr" : "k_onchip_rhs", k, grid, NT, smem, st, a);
   if (mode == OC_CORR && do_dens) {
-    const int slots = (int)(P.M > 256 ? P.M : 256);
+    const int slots = (int)(P.M > NT ? P.M : NT);
     LAUNCH(c, k_oc_dens_final, nb(4 * P.M * 32, 256), 256, 0, st, c->oc_dpart, grid, slots, P.M, c->raw);
   }
 }
@@ -231,4 +341,29 @@ static wslda_status oc_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double
     oc_launch(c, st, OC_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0,
               eps_dev ? eps_dev + n_first : c->eps + n_first);
   return cuda_check(c, "apply_h");
+}
+
+static void oc_pred(wslda_ctx* c, cudaStream_t st, cplx* phi, const HistPtrs& h, cplx* cpart, const AbmCoef& k, int do_dens) {
+  const Plan& P = c->P;
+  OCPred a;
+  a.L = c->L; a.phi = phi; a.h = h; a.cpart = cpart; a.k = k; a.dV = c->dV; a.normalize = c->f.normalize;
+  a.do_dens = do_dens; a.cpref = c->cpref; a.w_a = c->w_a; a.w_b = c->w_b; a.dpart = c->oc_dpart; a.n = P.n_wf; a.S = P.ocS;
+  const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(k_onchip_pred<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_pred<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    attr = true;
+  }
+  const bool small = P.M <= 512;
+  const int NT = small ? 256 : 512;
+  const int64_t nbat = (P.n_wf + P.ocS - 1) / P.ocS;
+  const int grid = (int)(nbat < P.oc_grid ? nbat : P.oc_grid);
+  WORK(c, 32.0 * P.M * P.n_wf * (1 + c->m + 2), 0);
+  if (small) LAUNCHN(c, "k_onchip_pred", k_onchip_pred<2>, grid, NT, smem, st, a);
+  else LAUNCHN(c, "k_onchip_pred", k_onchip_pred<8>, grid, NT, smem, st, a);
+  if (do_dens) {
+    const int slots = (int)(P.M > NT ? P.M : NT);
+    LAUNCH(c, k_oc_dens_final, nb(4 * P.M * 32, 256), 256, 0, st, c->oc_dpart, grid, slots, P.M, c->raw);
+  }
 }

@@ -181,14 +181,9 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
   const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
   const unsigned mask = step_mask(c);
   if (c->P.oc && (fixed || mask == (WSLDA_D_RHO | WSLDA_D_NU))) {   // fused on-chip stages (onchip_step.cuh)
-    const double* scg = c->f.normalize ? c->scale : nullptr;
-    for (int64_t n0 = 0; n0 < n_wf; n0 += P.chunk_n) {
-      const int64_t cnt = chunk_len(c, n0);
-      stage1(c, b, n0, cnt, st);
-      if (!fixed) dens_chunk(c, b.phi + 2 * n0 * M, scg ? scg + n0 : nullptr, n0, cnt, mask, n0 > 0, st);
-    }
+    oc_pred(c, st, b.phi, b.h, b.cpart, b.k, !fixed);       // the predictor is stored normalised: no scale afterwards
     if (!fixed) potentials(c, st);
-    oc_launch(c, st, OC_CORR, b.phi, scg, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed, c->eps);
+    oc_launch(c, st, OC_CORR, b.phi, nullptr, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed, c->eps);
     if (!fixed) potentials(c, st);
     oc_launch(c, st, OC_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0, c->eps);
   } else if (f3_step_ok(c)) {                            // fused 3-D path (fast_step.cuh)
