@@ -13,6 +13,7 @@
 
 enum { OC_APPLY = 0, OC_CORR = 1, OC_RHS = 2 };
 #define OC_MAXS 64              // spinors per CTA batch (s_eps / s_sn arrays)
+#define OC_SLOTS 8              // (lattice point, spinor) pairs per thread and batch
 
 struct OCArgs {
   Lat L;
@@ -43,6 +44,14 @@ __device__ __forceinline__ void oc_reduce(const double* E, int cnt, int lgM, dou
   }
 }
 
+// acc[w mod PT] += (a0..a3) with a register-resident accumulator array: the index is resolved by predication
+template <int MAXPT>
+__device__ __forceinline__ void oc_dens_acc(double (&acc)[MAXPT][4], int w, int PT, double a0, double a1, double a2, double a3) {
+#pragma unroll
+  for (int kk = 0; kk < MAXPT; ++kk)
+    if ((w & (PT - 1)) == kk) { acc[kk][0] += a0; acc[kk][1] += a1; acc[kk][2] += a2; acc[kk][3] += a3; }
+}
+
 // MAXPT = compile-time bound on the lattice points per thread, max(1, M / blockDim.x): 2 (256 threads, M <= 512,
 // two CTAs per SM) or 8 (512 threads for M up to 4096, one CTA per SM)
 template <int MODE, int MAXPT>
@@ -59,16 +68,31 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
   double acc[MAXPT][4];
 #pragma unroll
   for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
+  // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP), at most OC_SLOTS of them; the spinor
+  // values of the slots stay in registers from the load to the last phase (psi is read from HBM exactly once)
+  const int nsp_full = S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
   const int64_t n_batches = (a.n + S - 1) / S;
   for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const int64_t n0 = b * S;
     const int cnt = (int)((a.n - n0 < S) ? a.n - n0 : S);
-    const int tot = S * 2 * M, used = cnt * 2 * M;
+    const int used = cnt * 2 * M;
     const cplx* src = a.psi + (size_t)n0 * 2 * M;
-    for (int idx = tid; idx < tot; idx += NT) {
-      cplx v = make_double2(0.0, 0.0);
-      if (idx < used) { v = src[idx]; if (a.scale) v = cscale(v, a.scale[n0 + (idx >> (lgM + 1))]); }
-      F[idx] = v;
+    cplx ru[OC_SLOTS], rv[OC_SLOTS];
+#pragma unroll
+    for (int w = 0; w < OC_SLOTS; ++w) {
+      ru[w] = rv[w] = make_double2(0.0, 0.0);
+      if (w < PT * nsp_full) {
+        const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+        if (sp < cnt) { ru[w] = __ldg(src + (size_t)(2 * sp) * M + i); rv[w] = __ldg(src + (size_t)(2 * sp + 1) * M + i); }
+      }
+    }
+#pragma unroll
+    for (int w = 0; w < OC_SLOTS; ++w) {
+      if (w < PT * nsp_full) {
+        const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+        if (a.scale && sp < cnt) { const double sc = a.scale[n0 + sp]; ru[w] = cscale(ru[w], sc); rv[w] = cscale(rv[w], sc); }
+        F[(2 * sp) * M + i] = ru[w]; F[(2 * sp + 1) * M + i] = rv[w];
+      }
     }
     __syncthreads();
     const int G = 2 * S;
@@ -84,25 +108,47 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     fft_axis<true>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
     if (L.nd > 1) fft_axis<true>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
     if (L.nd > 2) fft_axis<true>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
-    // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order)
-    for (int kk = 0; kk < PT; ++kk) {
-      const int i = (tid + NT * kk) & (M - 1);
-      const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
-      const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b;
-      for (int s = s0; s < cnt; s += SSTEP) {
-        const int64_t n = n0 + s;
-        const double sc = a.scale ? a.scale[n] : 1.0, kp2 = a.kperp2[n];
-        const cplx u = cscale(src[(size_t)(2 * s) * M + i], sc), v = cscale(src[(size_t)(2 * s + 1) * M + i], sc);
-        const cplx lu = F[(2 * s) * M + i], lv = F[(2 * s + 1) * M + i];
-        const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
-        const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
-        const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                    // Eqs. 5, 15
-        const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, pb)));
-        E[(s << lgM) + i] = u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
-        if (MODE == OC_APPLY) {
-          a.out[(size_t)(2 * n) * M + i] = Hu; a.out[(size_t)(2 * n + 1) * M + i] = Hv;
-        } else {
-          F[(2 * s) * M + i] = Hu; F[(2 * s + 1) * M + i] = Hv;
+    // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order).  CORR leaves
+    // X = C_part - i kappa H psi in F (phi_new = X + i kappa eps psi once eps_n is known): C_part is consumed here,
+    // four slots at a time so that its loads are in flight together without holding 16 more values in registers.
+#pragma unroll
+    for (int w0 = 0; w0 < OC_SLOTS; w0 += 4) {
+      cplx cu[4], cv[4];
+      if (MODE == OC_CORR) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          const int w = w0 + r;
+          if (w < PT * nsp_full) {
+            const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+            if (sp < cnt) { cu[r] = __ldg(a.cpart + (size_t)(2 * (n0 + sp)) * M + i); cv[r] = __ldg(a.cpart + (size_t)(2 * (n0 + sp) + 1) * M + i); }
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const int w = w0 + r;
+        if (w < PT * nsp_full) {
+          const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+          if (sp < cnt) {
+            const int64_t n = n0 + sp;
+            const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
+            const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b, kp2 = a.kperp2[n];
+            const cplx u = ru[w], v = rv[w];
+            const cplx lu = F[(2 * sp) * M + i], lv = F[(2 * sp + 1) * M + i];
+            const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
+            const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
+            const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                    // Eqs. 5, 15
+            const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, pb)));
+            E[(sp << lgM) + i] = u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
+            if (MODE == OC_APPLY) {
+              a.out[(size_t)(2 * n) * M + i] = Hu; a.out[(size_t)(2 * n + 1) * M + i] = Hv;
+            } else if (MODE == OC_RHS) {
+              F[(2 * sp) * M + i] = Hu; F[(2 * sp + 1) * M + i] = Hv;
+            } else {
+              F[(2 * sp) * M + i] = make_double2(cu[r].x + a.kappa * Hu.y, cu[r].y - a.kappa * Hu.x);
+              F[(2 * sp + 1) * M + i] = make_double2(cv[r].x + a.kappa * Hv.y, cv[r].y - a.kappa * Hv.x);
+            }
+          }
         }
       }
     }
@@ -117,22 +163,25 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     __syncthreads();
     if (MODE != OC_APPLY) {
       // ---- phase 2: f = -i (H - eps) psi;  RHS writes it, CORR forms phi_new = C_part + kappa f in place
-      for (int kk = 0; kk < PT; ++kk) {
-        const int i = (tid + NT * kk) & (M - 1);
-        for (int s = s0; s < cnt; s += SSTEP) {
-          const int64_t n = n0 + s;
-          const double sc = a.scale ? a.scale[n] : 1.0, e = s_eps[s];
-          const cplx u = cscale(src[(size_t)(2 * s) * M + i], sc), v = cscale(src[(size_t)(2 * s + 1) * M + i], sc);
-          const cplx Hu = F[(2 * s) * M + i], Hv = F[(2 * s + 1) * M + i];
-          const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
-          if (MODE == OC_RHS) {
-            a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
-          } else {
-            const cplx cu = a.cpart[(size_t)(2 * n) * M + i], cv = a.cpart[(size_t)(2 * n + 1) * M + i];
-            const cplx pu = make_double2(cu.x + a.kappa * fu.x, cu.y + a.kappa * fu.y);
-            const cplx pv = make_double2(cv.x + a.kappa * fv.x, cv.y + a.kappa * fv.y);
-            F[(2 * s) * M + i] = pu; F[(2 * s + 1) * M + i] = pv;
-            E[(s << lgM) + i] = cabs2(pu) + cabs2(pv);
+#pragma unroll
+      for (int w = 0; w < OC_SLOTS; ++w) {
+        if (w < PT * nsp_full) {
+          const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+          if (sp < cnt) {
+            const int64_t n = n0 + sp;
+            const double e = s_eps[sp];
+            const cplx u = ru[w], v = rv[w];
+            const cplx Hu = F[(2 * sp) * M + i], Hv = F[(2 * sp + 1) * M + i];
+            if (MODE == OC_RHS) {
+              const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
+              a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
+            } else {
+              const double ke = a.kappa * e;                           // F holds X: phi_new = X + i kappa eps psi
+              const cplx pu = make_double2(Hu.x - ke * u.y, Hu.y + ke * u.x);
+              const cplx pv = make_double2(Hv.x - ke * v.y, Hv.y + ke * v.x);
+              ru[w] = pu; rv[w] = pv;                                  // phi_new stays in registers
+              E[(sp << lgM) + i] = cabs2(pu) + cabs2(pv);
+            }
           }
         }
       }
@@ -145,20 +194,17 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       __syncthreads();
       // ---- phase 3: normalise (Alg. 2 step 8), write phi_new once, accumulate its densities (Eqs. 7a, 7b, 7e)
 #pragma unroll
-      for (int kk = 0; kk < MAXPT; ++kk) {
-        if (kk < PT) {
-          const int i = (tid + NT * kk) & (M - 1);
-          for (int s = s0; s < cnt; s += SSTEP) {
-            const int64_t n = n0 + s;
-            const double sn = s_sn[s];
-            const cplx u = cscale(F[(2 * s) * M + i], sn), v = cscale(F[(2 * s + 1) * M + i], sn);
+      for (int w = 0; w < OC_SLOTS; ++w) {
+        if (w < PT * nsp_full) {
+          const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+          if (sp < cnt) {
+            const int64_t n = n0 + sp;
+            const double sn = s_sn[sp];
+            const cplx u = cscale(ru[w], sn), v = cscale(rv[w], sn);
             a.out[(size_t)(2 * n) * M + i] = u; a.out[(size_t)(2 * n + 1) * M + i] = v;
             if (a.do_dens) {
               const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n], wn = 0.5 * cp * (wb - wa);
-              acc[kk][0] += cp * wa * cabs2(u);
-              acc[kk][1] += cp * wb * cabs2(v);
-              acc[kk][2] += wn * (u.x * v.x + u.y * v.y);
-              acc[kk][3] += wn * (u.y * v.x - u.x * v.y);
+              oc_dens_acc<MAXPT>(acc, w, PT, cp * wa * cabs2(u), cp * wb * cabs2(v), wn * (u.x * v.x + u.y * v.y), wn * (u.y * v.x - u.x * v.y));
             }
           }
         }
