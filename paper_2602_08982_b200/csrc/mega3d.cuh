@@ -39,7 +39,7 @@ struct F3Mega {
   const double* scale;         // per spinor (nullable)
   const double* kperp2;        // per spinor
   F3Fields F;
-  const cplx* pack;            // [M][3]: (q_a, q_b), Delta + Delta_ext, (alpha_a, alpha_b)  -- see k_f3_pack
+  const cplx* pack;            // [3][M]: (q_a, q_b), Delta + Delta_ext, (alpha_a, alpha_b)  -- see k_f3_pack
   const double *ky2, *kz2;
   double kx2[32];
   double invM, dV, kappa;
@@ -64,9 +64,9 @@ __global__ void k_f3_pack(F3Fields F, int sym, int64_t M, cplx* pack) {
   if (i >= M) return;
   const double qa = F.U[0][i] - F.mu[0] + (sym ? 0.25 * F.lap[0][i] : 0.0);
   const double qb = F.U[1][i] - F.mu[1] + (sym ? 0.25 * F.lap[1][i] : 0.0);
-  pack[3 * i] = make_double2(qa, qb);
-  pack[3 * i + 1] = cadd(F.delta[i], F.dext[i]);
-  pack[3 * i + 2] = make_double2(F.alpha[0][i], F.alpha[1][i]);
+  pack[i] = make_double2(qa, qb);
+  pack[M + i] = cadd(F.delta[i], F.dext[i]);
+  pack[2 * M + i] = make_double2(F.alpha[0][i], F.alpha[1][i]);
 }
 
 __device__ __forceinline__ cplx ldcg2(const cplx* p) { return __ldcg(p); }
@@ -88,6 +88,12 @@ __device__ __forceinline__ cplx ld_pol(const cplx* p, uint64_t pol) {        // 
 }
 __device__ __forceinline__ void st_pol(cplx* p, cplx v, uint64_t pol) {
   asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
+// same store without the compiler memory barrier: lets the plain loads of the next loop iterations be hoisted above it
+// (volatile asm statements keep their order among themselves, ordinary loads may pass them)
+__device__ __forceinline__ void st_pol_nb(cplx* p, cplx v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol));
 }
 
 __device__ __forceinline__ void f3_pf1(const void* p) { asm volatile("prefetch.global.L1 [%0];" :: "l"(p)); }
@@ -202,7 +208,7 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
         f3_pf1(pu8 + q * 128); f3_pf1(pu8 + M * 16 + q * 128);
         if (MODE == F3_CORR) { f3_pf1(cu8 + q * 128); f3_pf1(cu8 + M * 16 + q * 128); }
       }
-      for (int q = lane; q < 3 * LW; q += 32) f3_pf1((const char*)(a.pack + 3 * r0) + q * 128);
+      for (int q = lane; q < LW; q += 32) { f3_pf1((const char*)(a.pack + r0) + q * 128); f3_pf1((const char*)(a.pack + M + r0) + q * 128); }
     }
     const cplx* sp = (t ? a.spec1 : a.spec0) + (ring + c) * M + pl;
 #pragma unroll
@@ -229,15 +235,26 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
     cplx* ou = (MODE == F3_APPLY ? a.out + (size_t)(2 * n) * M : a.X + ring * M) + pl;
     cplx* ov = ou + M;
     const cplx* cu = a.cpart + (size_t)(2 * n) * M + pl;
-    const cplx* pk = a.pack + 3 * pl;
-#pragma unroll 4
-    for (int jj = 0; jj < ROWS; ++jj) {
-      const int j = wl * ROWS + jj, i = j * F3_N + lane, si = j * F3_PITCH + lane;
-      const cplx u = cscale(pu[i], s), v = cscale(pv[i], s);
+    const cplx* pk = a.pack + pl;
+#pragma unroll
+    for (int jj0 = 0; jj0 < ROWS; jj0 += 4) {
+     // four rows at a time: every global load of the chunk is issued before the first use
+     cplx gu[4], gv[4], gq[4], gD[4], gA[4], g0[4], g1[4];
+#pragma unroll
+     for (int r = 0; r < 4; ++r) {
+       const int i = (wl * ROWS + jj0 + r) * F3_N + lane;
+       gu[r] = pu[i]; gv[r] = pv[i]; gq[r] = pk[i]; gD[r] = pk[M + i];
+       if (SYM && kp2 != 0.0) gA[r] = pk[2 * M + i];
+       if (MODE == F3_CORR) { g0[r] = cu[i]; g1[r] = cu[M + i]; }
+     }
+#pragma unroll
+     for (int r = 0; r < 4; ++r) {
+      const int j = wl * ROWS + jj0 + r, i = j * F3_N + lane, si = j * F3_PITCH + lane;
+      const cplx u = cscale(gu[r], s), v = cscale(gv[r], s);
       const cplx Lu = tb[(NS - 1) * TILE + si], Lv = tb[(2 * NS - 1) * TILE + si];
-      const cplx q = pk[3 * i], D = pk[3 * i + 1];
+      const cplx q = gq[r], D = gD[r];
       double ha = 0.5 * kp2, hb = 0.5 * kp2;
-      if (SYM && kp2 != 0.0) { const cplx al2 = pk[3 * i + 2]; ha *= al2.x; hb *= al2.y; }
+      if (SYM && kp2 != 0.0) { ha *= gA[r].x; hb *= gA[r].y; }
       cplx Ku, Kv;
       if (SYM) {                                                       // Eq. 40; its +(lap alpha) w / 4 term sits in q
         const cplx Tu = tb[si], Tv = tb[NS * TILE + si];
@@ -250,18 +267,19 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
       const cplx Hu = cadd(Ku, cadd(cscale(u, q.x), cmul(D, v)));                               // Eqs. 5, 15
       const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, q.y)));
       e += u.x * Hu.x + u.y * Hu.y + v.x * Hv.x + v.y * Hv.y;
-      if (MODE == F3_APPLY) { st_pol(ou + i, Hu, pol.drop); st_pol(ov + i, Hv, pol.drop); }
-      else if (MODE == F3_RHS) { st_pol(ou + i, make_double2(Hu.y, -Hu.x), pol.keep); st_pol(ov + i, make_double2(Hv.y, -Hv.x), pol.keep); }   // -i H
+      if (MODE == F3_APPLY) { st_pol_nb(ou + i, Hu, pol.drop); st_pol_nb(ov + i, Hv, pol.drop); }
+      else if (MODE == F3_RHS) { st_pol_nb(ou + i, make_double2(Hu.y, -Hu.x), pol.keep); st_pol_nb(ov + i, make_double2(Hv.y, -Hv.x), pol.keep); }   // -i H
       else {
-        const cplx c0 = cu[i], c1 = cu[M + i];
+        const cplx c0 = g0[r], c1 = g1[r];
         const cplx xu = make_double2(c0.x + a.kappa * Hu.y, c0.y - a.kappa * Hu.x);             // C_part - i kappa H
         const cplx xv = make_double2(c1.x + a.kappa * Hv.y, c1.y - a.kappa * Hv.x);
-        st_pol(ou + i, xu, pol.keep); st_pol(ov + i, xv, pol.keep);
+        st_pol_nb(ou + i, xu, pol.keep); st_pol_nb(ov + i, xv, pol.keep);
         xx += cabs2(xu) + cabs2(xv);
         xpr += xu.x * u.x + xu.y * u.y + xv.x * v.x + xv.y * v.y;
         xpi += xu.x * u.y - xu.y * u.x + xv.x * v.y - xv.y * v.x;
         pp += cabs2(u) + cabs2(v);
       }
+     }
     }
   }
   F3_T(2, 4);
@@ -335,22 +353,32 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
     if (MODE == F3_CORR) {
       const double sP = a.scale ? a.scale[n] : 1.0, ke = a.kappa * e, sn = s_sn[nl];
       const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n];
+      cplx gxu[PTS], gxv[PTS], gpu[PTS], gpv[PTS];          // all loads of this spinor first, then the arithmetic
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        const cplx xu = ld_pol(Xu + r * 128, pol.drop), xv = ld_pol(Xu + M + r * 128, pol.drop);
-        const cplx wu = cscale(pu[r * 128], sP), wv = cscale(pu[M + r * 128], sP);
+        gxu[r] = __ldcg(Xu + r * 128); gxv[r] = __ldcg(Xu + M + r * 128); gpu[r] = pu[r * 128]; gpv[r] = pu[M + r * 128];
+      }
+#pragma unroll
+      for (int r = 0; r < PTS; ++r) {
+        const cplx xu = gxu[r], xv = gxv[r];
+        const cplx wu = cscale(gpu[r], sP), wv = cscale(gpv[r], sP);
         const cplx u = make_double2((xu.x - ke * wu.y) * sn, (xu.y + ke * wu.x) * sn);
         const cplx v = make_double2((xv.x - ke * wv.y) * sn, (xv.y + ke * wv.x) * sn);
-        st_pol(ou + r * 128, u, pol.drop); st_pol(ou + M + r * 128, v, pol.drop);
+        st_pol_nb(ou + r * 128, u, pol.drop); st_pol_nb(ou + M + r * 128, v, pol.drop);
         if (a.do_dens) f3_dens_add(acc[r], u, v, cp, wa, wb);
       }
     } else {
+      cplx gxu[PTS], gxv[PTS], gpu[PTS], gpv[PTS];
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        const cplx yu = ld_pol(Xu + r * 128, pol.drop), yv = ld_pol(Xu + M + r * 128, pol.drop);
-        const cplx u = pu[r * 128], v = pu[M + r * 128];
-        st_pol(ou + r * 128, make_double2(yu.x - e * u.y, yu.y + e * u.x), pol.drop);
-        st_pol(ou + M + r * 128, make_double2(yv.x - e * v.y, yv.y + e * v.x), pol.drop);
+        gxu[r] = __ldcg(Xu + r * 128); gxv[r] = __ldcg(Xu + M + r * 128); gpu[r] = pu[r * 128]; gpv[r] = pu[M + r * 128];
+      }
+#pragma unroll
+      for (int r = 0; r < PTS; ++r) {
+        const cplx yu = gxu[r], yv = gxv[r];
+        const cplx u = gpu[r], v = gpv[r];
+        st_pol_nb(ou + r * 128, make_double2(yu.x - e * u.y, yu.y + e * u.x), pol.drop);
+        st_pol_nb(ou + M + r * 128, make_double2(yv.x - e * v.y, yv.y + e * v.x), pol.drop);
       }
     }
   }
