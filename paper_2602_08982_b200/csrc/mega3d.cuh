@@ -100,22 +100,33 @@ __device__ __forceinline__ void f3_pf1(const void* p) { asm volatile("prefetch.g
 __device__ __forceinline__ void f3_pf(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 
-// one thread waits until *ctr >= target (bounded), then the whole CTA proceeds
+// one thread waits until *ctr >= target (bounded), then the whole CTA proceeds.  The counter is read with acquire
+// semantics (no separate fence) and bumped with a release reduction: the PTX memory model's release/acquire pair on
+// the counter orders the producers' stores (made visible to thread 0 by the CTA barrier) before the consumers' loads.
+// (Deferring the release into the next item's load phase was measured: it hides the release latency but delays the
+// dependants more than it saves.)
+__device__ __forceinline__ int f3_ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void f3_red_release(int* p) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], 1;" :: "l"(p) : "memory");
+}
 __device__ __forceinline__ void f3_wait(int* ctr, int target, F3Sync* sy) {
   if (threadIdx.x == 0) {
     int spins = 0;
-    while (*(volatile int*)ctr < target) {
+    while (f3_ld_acquire(ctr) < target) {
       __nanosleep(200);
       if (++spins > (1 << 23)) { sy->error = 1; break; }
     }
-    __threadfence();
   }
   __syncthreads();
 }
 __device__ __forceinline__ void f3_signal(int* ctr, int* next, int& ticket) {
-  if (threadIdx.x == 0) ticket = atomicAdd(next, 1);       // the next ticket travels while the barrier and the fence complete
+  if (threadIdx.x == 0) ticket = atomicAdd(next, 1);       // the next ticket travels while the barrier and the release complete
   __syncthreads();
-  if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1); }
+  if (threadIdx.x == 0) f3_red_release(ctr);
 }
 
 // ---- A: forward plane transforms of 4 component planes (one per warp) ----------------------------------------
@@ -399,21 +410,21 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
 // will read from HBM -- psi of group t+1 (A items) and C_part of group t-1 (C items of tick t+1) -- so that those
 // loads find their lines in L2.  Needs no ticket look-ahead, hence adds no dependency latency.
 template <int MODE>
-__device__ __forceinline__ void f3_prefetch_tick(const F3Mega& a, int tick, int r, int IT) {
+__device__ __forceinline__ void f3_prefetch_tick(const F3Mega& a, int tick, int r, int chunk, int lines) {
   const size_t M = (size_t)a.NX * F3_PLANE;
-  const long lines = (long)a.gs * 2 * M * 16 / 128;              // 128-byte lines of one group of one buffer
-  const long chunk = (lines + IT - 1) / IT, q0 = (long)r * chunk;
-  long q1 = q0 + chunk; if (q1 > lines) q1 = lines;
+  const int lpc = (int)(M * 16 / 128) * 2;                        // 128-byte lines per spinor
+  const int q0 = r * chunk + threadIdx.x;
+  int q1 = (r + 1) * chunk; if (q1 > lines) q1 = lines;
   const int ga = tick + 1, gc = tick - 1;
   if (ga < a.G) {
-    const long lim = (long)((a.n - ga * a.gs < a.gs) ? a.n - ga * a.gs : a.gs) * 2 * M * 16 / 128;
+    const int rem = a.n - ga * a.gs, lim = (rem < a.gs ? rem : a.gs) * lpc;
     const char* base = (const char*)(a.psi + (size_t)ga * a.gs * 2 * M);
-    for (long q = q0 + threadIdx.x; q < q1 && q < lim; q += 128) f3_pf(base + q * 128);
+    for (int q = q0; q < q1 && q < lim; q += 128) f3_pf(base + (size_t)q * 128);
   }
   if (MODE == F3_CORR && gc >= 0 && gc < a.G) {
-    const long lim = (long)((a.n - gc * a.gs < a.gs) ? a.n - gc * a.gs : a.gs) * 2 * M * 16 / 128;
+    const int rem = a.n - gc * a.gs, lim = (rem < a.gs ? rem : a.gs) * lpc;
     const char* base = (const char*)(a.cpart + (size_t)gc * a.gs * 2 * M);
-    for (long q = q0 + threadIdx.x; q < q1 && q < lim; q += 128) f3_pf(base + q * 128);
+    for (int q = q0; q < q1 && q < lim; q += 128) f3_pf(base + (size_t)q * 128);
   }
 }
 
@@ -432,6 +443,7 @@ __global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3_mega(F3Mega a) {
   const int nA = a.gs * 2 * NX / 4, nB = a.gs * 16, nC = SYM ? a.gs * NX : a.gs * NX / 2;
   const int nD = MODE == F3_APPLY ? 0 : NX * F3_DSPLIT;
   const int IT = nA + nB + nC + nD, total = (G + 3) * IT;
+  const int pf_lines = a.gs * 2 * NX * (F3_PLANE * 16 / 128), pf_chunk = (pf_lines + IT - 1) / IT;
   int t1 = 0;
   if (threadIdx.x == 0) t1 = atomicAdd(&a.sync->next, 1);
   for (;;) {
@@ -443,7 +455,7 @@ __global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3_mega(F3Mega a) {
     if (item >= total) break;
     const int tick = item / IT, r = item - tick * IT;
     bool drew = false;
-    f3_prefetch_tick<MODE>(a, tick, r, IT);
+    f3_prefetch_tick<MODE>(a, tick, r, pf_chunk, pf_lines);
     F3_T(4, 0);
     if (r < nA) {
       const int g = tick;
