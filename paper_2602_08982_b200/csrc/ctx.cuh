@@ -86,7 +86,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
            f->kin_form != WSLDA_KIN_DIVGRAD;
   if (const char* e = getenv("WSLDA_FAST")) if (atoi(e) == 0) P.fast = 0;
-  P.fc = 16; P.ns = 3;
+  P.fc = 32; P.ns = 3;
   if (const char* e = getenv("WSLDA_FAST_CHUNK")) { int v = atoi(e); if (v > 0) P.fc = v; }
   if (const char* e = getenv("WSLDA_FAST_STREAMS")) { int v = atoi(e); if (v > 0 && v <= 4) P.ns = v; }
   if (P.fc > n_wf) P.fc = (int)n_wf;
@@ -97,7 +97,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
-  P.mega = P.fast; P.gs = 4;
+  P.mega = P.fast; P.gs = 5;
   if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
   if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
   if (P.gs > n_wf) P.gs = (int)n_wf;
