@@ -9,6 +9,7 @@
 #include "fft_large.cuh"
 #include "fast3d.cuh"
 #include "mega3d.cuh"
+#include "mega64.cuh"
 #include "kernels.cuh"
 
 struct Plan {
@@ -26,6 +27,9 @@ struct Plan {
   // fused on-chip stages (onchip_step.cuh): enabled flag, spinors per CTA batch, persistent grid, density partials
   int oc, ocS, oc_grid;
   size_t off_oc, oc_dpart_bytes;
+  // 64^3 persistent kernels (mega64.cuh)
+  int f6;
+  size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes;
   int mega, gs, mG;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
@@ -111,6 +115,17 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_pack_bytes = align_up((size_t)M * 48);
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
+  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40;
+  if (const char* e = getenv("WSLDA_MEGA64")) if (atoi(e) == 0) P.f6 = 0;
+  P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = 0;
+  if (P.f6) {
+    P.f6_ring_bytes = align_up((size_t)F6_RING * M * 16);
+    P.f6_part_bytes = align_up((size_t)F3_NPART * 2 * n_wf * F6_N * 8);
+    P.f6_acc_bytes = align_up((size_t)F6_RING * 4 * M * 8);
+    P.f6_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * 2 * n_wf * sizeof(int));
+    P.f6_pack_bytes = align_up((size_t)M * 48);
+    o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes;
+  }
   P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
   if (const char* e = getenv("WSLDA_ONCHIP")) if (atoi(e) == 0) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
@@ -142,6 +157,9 @@ struct wslda_ctx {
   F3Sync* m_sync;
   cplx* m_pack;
   double* oc_dpart;
+  cplx *s_spec0, *s_spec1, *s_X, *s_pack;   // 64^3 rings
+  double *s_part, *s_acc;
+  F3Sync* s_sync;
   int mega_grid;
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -191,12 +209,12 @@ static inline void prof_end(wslda_ctx* c, cudaStream_t st) { cudaEventRecord((*c
 // 5 N log2 N per line transform) -- only used by the profile report
 #define WORK(c, bytes, flops) do { (c)->work_bytes = (double)(bytes); (c)->work_flops = (double)(flops); } while (0)
 
-// stored position p of the in-place DIF transform (radix 4 from L = n down, then radix 2) <-> frequency index
+// stored position p of the in-place DIF transform (radix 8 from L = n down, then the remaining 4 or 2) <-> frequency index
 static void scrambled_freq(int n, std::vector<int>& fr) {
   fr.resize(n);
   for (int p = 0; p < n; ++p) {
     int L = n, rem = p, k = 0, mult = 1;
-    while (L > 1) { int r = (L >= 4) ? 4 : 2, sub = L / r, m = rem / sub; rem %= sub; k += m * mult; mult *= r; L = sub; }
+    while (L > 1) { int r = (L >= 8) ? 8 : L, sub = L / r, m = rem / sub; rem %= sub; k += m * mult; mult *= r; L = sub; }
     fr[p] = k;
   }
 }
@@ -314,6 +332,18 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
     c->mega_grid = best * sms;
     if (const char* e = getenv("WSLDA_MEGA_CTAS")) { int v = atoi(e); if (v > 0) c->mega_grid = v; }
+  }
+  if (P.f6) {
+    char* b = base + P.off_f6;
+    c->s_spec0 = (cplx*)b; c->s_spec1 = (cplx*)(b + P.f6_ring_bytes); c->s_X = (cplx*)(b + 2 * P.f6_ring_bytes);
+    b += 3 * P.f6_ring_bytes;
+    c->s_part = (double*)b; b += P.f6_part_bytes;
+    c->s_acc = (double*)b; b += P.f6_acc_bytes;
+    c->s_sync = (F3Sync*)b; b += P.f6_sync_bytes;
+    c->s_pack = (cplx*)b;
+    cudaFuncSetAttribute(k_f6_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
+    cudaFuncSetAttribute(k_f6_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
+    cudaFuncSetAttribute(k_f6_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
   }
   if (P.oc) c->oc_dpart = (double*)(base + P.off_oc);
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1

@@ -82,6 +82,42 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
           4 * F3_TILE_BYTES, st, a);
 }
 
+// ---- 64^3 (mega64.cuh) -------------------------------------------------------------------------------------------
+// eps_n from the per-(component, x-plane) partial sums of an APPLY launch: one warp per spinor
+__global__ void k_f6_scal(const double* part, int n, double dV, double* eps, double* eps_user) {
+  const int s = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (s >= n) return;
+  const double* pp = part + (size_t)(2 * s) * F6_N;
+  double t = (pp[lane] + pp[32 + lane]) + (pp[64 + lane] + pp[96 + lane]);
+  t = warp_sum(t);
+  if (lane == 0) { eps[s] = dV * t; if (eps_user) eps_user[s] = dV * t; }
+}
+
+static void f6_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, const double* scale, int64_t n0, int64_t n,
+                    cplx* out, const cplx* cpart, double kappa, int do_dens) {
+  const Plan& P = c->P;
+  F6Mega a;
+  a.psi = psi; a.scale = scale; a.kperp2 = c->kperp2 + n0; a.F = f3_fields(c); a.pack = c->s_pack;
+  a.kx2 = c->k2n[0]; a.ky2 = c->k2n[1]; a.kz2 = c->k2n[2];
+  a.invM = c->L.invM; a.dV = c->dV; a.kappa = kappa;
+  a.spec0 = c->s_spec0; a.spec1 = c->s_spec1; a.X = c->s_X; a.out = out; a.cpart = cpart; a.part = c->s_part;
+  a.eps_out = mode == F3_APPLY ? nullptr : c->eps + n0;
+  a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.do_dens = do_dens;
+  a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.acc = c->s_acc; a.sync = c->s_sync;
+  a.n = (int)n; a.G = (int)(2 * n);
+  cudaMemsetAsync(c->s_sync, 0, sizeof(F3Sync) + (size_t)4 * a.G * sizeof(int), st);
+  LAUNCH(c, k_f3_pack, nb(P.M, 256), 256, 0, st, a.F, 1, P.M, c->s_pack);
+  const int IT = F6_N / 2 + F6_N / 2 + F6_N + (mode == F3_APPLY ? 0 : F6_ND);
+  const long total = (long)(a.G + 4) * IT;
+  int sms = 148;
+  const int grid = (int)(total < sms ? total : sms);
+  const double M = (double)P.M;
+  WORK(c, M * n * (mode == F3_CORR ? 96.0 : 64.0), 5.0 * M * 18.0 * 2.0 * 2 * 2 * n);
+  void (*k)(F6Mega) = mode == F3_APPLY ? k_f6_mega<F3_APPLY> : mode == F3_CORR ? k_f6_mega<F3_CORR> : k_f6_mega<F3_RHS>;
+  LAUNCHN(c, mode == F3_APPLY ? "k_f6_mega_apply" : mode == F3_CORR ? "k_f6_mega_corr" : "k_f6_mega_rhs", k, grid, F6_THREADS,
+          2 * F6_TILE * 16, st, a);
+}
+
 static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, int mode, int use_shift, double kappa,
                     double* eps_user) {
   F3Scal s;
@@ -93,6 +129,14 @@ static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, i
 static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double* eps_dev, int64_t n_first, int64_t n_count,
                                cudaStream_t st) {
   const int64_t M = c->P.M;
+  if (c->P.f6) {
+    if (n_count > 0) {
+      f6_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0);
+      LAUNCH(c, k_f6_scal, (unsigned)((n_count + 3) / 4), 128, 0, st, c->s_part, (int)n_count, c->dV, c->eps + n_first,
+             eps_dev ? eps_dev + n_first : (double*)nullptr);
+    }
+    return cuda_check(c, "apply_h");
+  }
   if (c->P.mega && n_count > 0) {
     f3_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0);
     F3Scal s;

@@ -2,79 +2,67 @@
 // PAPER.md:360-371).  Forward = decimation in frequency, in place, natural order in -> digit-reversed
 // order out; inverse = the exact transpose (decimation in time), digit-reversed in -> natural out.  The
 // k-space multiply runs on the digit-reversed data with k-tables stored in that order, so no reordering
-// pass and no second buffer are needed.  Radix 4 with a final radix-2 stage when log2 N is odd.
+// pass and no second buffer are needed.  Radix 8 (register butterflies) with a final radix-4 / radix-2 stage.
 #pragma once
 #include "common.cuh"
+#include "regfft.cuh"
 
 // One axis of a block laid out [A][n][B] (element (a,j,b) at (a*n + j)*B + b) in shared memory.
 // All sizes are powers of two; lgn = log2 n, lgB = log2 B.  tw[j] = exp(-2 pi i j / n).
+// Radix plan: 8 while the remaining length is >= 8, then the remainder (4 or 2): 8 -> one pass, 64 -> two, 128 -> three.
+// Each thread pulls the R strided points of a butterfly into registers, runs the unrolled register transform of
+// regfft.cuh, applies the twiddles and writes back in place -- R-fold fewer shared-memory passes and barriers than
+// radix-2, and the butterfly arithmetic runs out of registers with full ILP.
+template <bool INV, int R>
+__device__ inline void fft_stage(cplx* s, int A, int lgn, int lgL, int lgB, const cplx* __restrict__ tw) {
+  constexpr int lgR = R == 8 ? 3 : R == 4 ? 2 : 1;
+  const int lgq = lgL - lgR, items = A << (lgn - lgR + lgB), Bm = (1 << lgB) - 1;
+  for (int t = threadIdx.x; t < items; t += blockDim.x) {
+    const int b = t & Bm, r = t >> lgB;
+    const int qq = r & ((1 << (lgn - lgR)) - 1), a = r >> (lgn - lgR);
+    const int q = qq & ((1 << lgq) - 1), blk = qq >> lgq;
+    cplx* p = s + ((((size_t)a << lgn) + ((size_t)blk << lgL) + q) << lgB) + b;
+    const size_t st = (size_t)1 << (lgq + lgB);
+    const int e = q << (lgn - lgL);                            // W_L^q = tw[q * n / L]
+    cplx x[R];
+#pragma unroll
+    for (int m = 0; m < R; ++m) x[m] = p[m * st];
+    if (!INV) {                                                // DIF: butterfly, then twiddle W_L^(q m)
+      fft_reg<R, false>(x);
+      if (q) {
+#pragma unroll
+        for (int m = 1; m < R; ++m) x[m] = cmul(x[m], __ldg(tw + m * e));
+      }
+    } else {                                                   // DIT: conj twiddle, then the inverse butterfly
+      if (q) {
+#pragma unroll
+        for (int m = 1; m < R; ++m) x[m] = cmul(x[m], cconj(__ldg(tw + m * e)));
+      }
+#pragma unroll
+      for (int m = 0; m < R; ++m) x[m] = cconj(x[m]);          // inverse = conj(forward(conj))
+      fft_reg<R, false>(x);
+#pragma unroll
+      for (int m = 0; m < R; ++m) x[m] = cconj(x[m]);
+    }
+#pragma unroll
+    for (int m = 0; m < R; ++m) p[m * st] = x[m];
+  }
+  __syncthreads();
+}
+
 template <bool INV>
 __device__ inline void fft_axis(cplx* s, int A, int lgn, int lgB, const cplx* __restrict__ tw) {
-  const int n = 1 << lgn;
-  if (n == 1) return;
-  const int Bm = (1 << lgB) - 1;
-  const bool odd = lgn & 1;
+  if (lgn == 0) return;
+  const int rem = lgn % 3;                                     // last (smallest) stage: radix 2^rem
   if (!INV) {
-    for (int lgL = lgn; lgL >= 2; lgL -= 2) {                 // radix-4 DIF stages, L = n, n/4, ...
-      const int lgq = lgL - 2, items = A << (lgn - 2 + lgB);
-      for (int t = threadIdx.x; t < items; t += blockDim.x) {
-        int b = t & Bm, r = t >> lgB;
-        int qq = r & ((n >> 2) - 1), a = r >> (lgn - 2);
-        int q = qq & ((1 << lgq) - 1), blk = qq >> lgq;
-        cplx* p = s + ((((size_t)a << lgn) + ((size_t)blk << lgL) + q) << lgB) + b;
-        const size_t st = (size_t)1 << (lgq + lgB);
-        cplx a0 = p[0], a1 = p[st], a2 = p[2 * st], a3 = p[3 * st];
-        cplx b0 = cadd(a0, a2), b1 = csub(a0, a2), b2 = cadd(a1, a3), d = csub(a1, a3);
-        cplx b3 = make_double2(d.y, -d.x);                    // (a1 - a3) * (-i)
-        cplx y0 = cadd(b0, b2), y1 = cadd(b1, b3), y2 = csub(b0, b2), y3 = csub(b1, b3);
-        if (q) {
-          int e = q << (lgn - lgL);                           // W_L^q = tw[q * n / L]
-          y1 = cmul(y1, tw[e]); y2 = cmul(y2, tw[2 * e]); y3 = cmul(y3, tw[3 * e]);
-        }
-        p[0] = y0; p[st] = y1; p[2 * st] = y2; p[3 * st] = y3;
-      }
-      __syncthreads();
-    }
-    if (odd) {                                                // final radix-2 stage, L = 2, no twiddle
-      const int items = A << (lgn - 1 + lgB);
-      for (int t = threadIdx.x; t < items; t += blockDim.x) {
-        int b = t & Bm, r = t >> lgB;
-        cplx* p = s + ((size_t)(2 * r) << lgB) + b;
-        cplx a0 = p[0], a1 = p[(size_t)1 << lgB];
-        p[0] = cadd(a0, a1); p[(size_t)1 << lgB] = csub(a0, a1);
-      }
-      __syncthreads();
-    }
+    int lgL = lgn;
+    for (; lgL >= 3; lgL -= 3) fft_stage<false, 8>(s, A, lgn, lgL, lgB, tw);
+    if (rem == 2) fft_stage<false, 4>(s, A, lgn, 2, lgB, tw);
+    else if (rem == 1) fft_stage<false, 2>(s, A, lgn, 1, lgB, tw);
   } else {
-    if (odd) {
-      const int items = A << (lgn - 1 + lgB);
-      for (int t = threadIdx.x; t < items; t += blockDim.x) {
-        int b = t & Bm, r = t >> lgB;
-        cplx* p = s + ((size_t)(2 * r) << lgB) + b;
-        cplx a0 = p[0], a1 = p[(size_t)1 << lgB];
-        p[0] = cadd(a0, a1); p[(size_t)1 << lgB] = csub(a0, a1);
-      }
-      __syncthreads();
-    }
-    for (int lgL = odd ? 3 : 2; lgL <= lgn; lgL += 2) {       // radix-4 DIT stages, L = 4 (8), ..., n
-      const int lgq = lgL - 2, items = A << (lgn - 2 + lgB);
-      for (int t = threadIdx.x; t < items; t += blockDim.x) {
-        int b = t & Bm, r = t >> lgB;
-        int qq = r & ((n >> 2) - 1), a = r >> (lgn - 2);
-        int q = qq & ((1 << lgq) - 1), blk = qq >> lgq;
-        cplx* p = s + ((((size_t)a << lgn) + ((size_t)blk << lgL) + q) << lgB) + b;
-        const size_t st = (size_t)1 << (lgq + lgB);
-        cplx y0 = p[0], y1 = p[st], y2 = p[2 * st], y3 = p[3 * st];
-        if (q) {
-          int e = q << (lgn - lgL);
-          y1 = cmul(y1, cconj(tw[e])); y2 = cmul(y2, cconj(tw[2 * e])); y3 = cmul(y3, cconj(tw[3 * e]));
-        }
-        cplx b0 = cadd(y0, y2), b1 = csub(y0, y2), b2 = cadd(y1, y3), d = csub(y1, y3);
-        cplx b3 = make_double2(-d.y, d.x);                    // (y1 - y3) * (+i)
-        p[0] = cadd(b0, b2); p[st] = cadd(b1, b3); p[2 * st] = csub(b0, b2); p[3 * st] = csub(b1, b3);
-      }
-      __syncthreads();
-    }
+    if (rem == 2) fft_stage<true, 4>(s, A, lgn, 2, lgB, tw);
+    else if (rem == 1) fft_stage<true, 2>(s, A, lgn, 1, lgB, tw);
+    for (int lgL = rem + 3; lgL <= lgn; lgL += 3) fft_stage<true, 8>(s, A, lgn, lgL, lgB, tw);
   }
 }
 

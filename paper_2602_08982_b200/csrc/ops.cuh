@@ -192,7 +192,7 @@ extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi
   const cplx* psi = (const cplx*)psi_; cplx* hpsi = (cplx*)hpsi_;
   const int64_t M = c->P.M;
   cudaStream_t st = S(stream);
-  if (c->P.fast) return f3_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
+  if (c->P.fast || c->P.f6) return f3_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
   if (c->P.oc) return oc_apply_h(c, psi, hpsi, eps_dev, n_first, n_count, st);
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
     const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;

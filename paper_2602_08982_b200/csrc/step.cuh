@@ -186,6 +186,21 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
     oc_launch(c, st, OC_CORR, b.phi, nullptr, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed, c->eps);
     if (!fixed) potentials(c, st);
     oc_launch(c, st, OC_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0, c->eps);
+  } else if (c->P.f6 && (fixed || mask == (WSLDA_D_RHO | WSLDA_D_NU))) {   // 64^3 persistent kernels (mega64.cuh)
+    const double* scg = c->f.normalize ? c->scale : nullptr;
+    for (int64_t n0 = 0; n0 < n_wf; n0 += P.chunk_n) {
+      const int64_t cnt = chunk_len(c, n0);
+      stage1(c, b, n0, cnt, st);
+      if (!fixed) dens_chunk(c, b.phi + 2 * n0 * M, scg ? scg + n0 : nullptr, n0, cnt, mask, n0 > 0, st);
+    }
+    if (!fixed) potentials(c, st);
+    f6_mega(c, st, F3_CORR, b.phi, scg, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed);
+    if (!fixed) {
+      const int slots = (int)(n_wf < F6_RING ? n_wf : F6_RING);
+      LAUNCH(c, k_f3_dens_final, nb(4 * M, 256), 256, 0, st, c->s_acc, slots, (int64_t)(4 * M), M, c->raw);
+      potentials(c, st);
+    }
+    f6_mega(c, st, F3_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0);
   } else if (f3_step_ok(c)) {                            // fused 3-D path (fast_step.cuh)
     F3Step s; s.phi = b.phi; s.h = b.h; s.cpart = b.cpart; s.k = b.k; s.c0dt = b.c0dt; s.user = st;
     f3_abm_step(c, s);

@@ -299,3 +299,31 @@ def test_cfg4_full_size_sampled_against_oracle():
     assert float(torch.max(torch.abs(nrm - 1.0))) < 1e-12          # property at any size: every spinor normalised
     del phi, hist
     torch.cuda.empty_cache()
+
+
+# ---- 64^3: pair-of-threads lines, component-granular persistent kernels (mega64.cuh) -------------------------------
+def test_mega64_apply_h():
+    w = generic((64, 64, 64), (1.0, 0.95, 1.05), 3, 1, n_modes=1)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi)
+    h, e = g.apply_h(to_gpu(psi))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    assert any(k.startswith("k_f6") for k in _kernels_of(g, lambda: g.apply_h(to_gpu(psi))))
+    h2, _ = g.apply_h(to_gpu(psi), n_first=1, n_count=2)
+    h2 = to_np(h2)
+    assert relerr(h2[1:3], ref[1:3]) < TOL_H and not h2[:1].any()
+
+
+@pytest.mark.parametrize("case", ["cfg5_fixed", "slda_selfconsistent"])
+def test_mega64_abm_matches_oracle(case):
+    if case == "cfg5_fixed":
+        w = wl.cfg5(n_wf=7, n_steps=3)                       # configs[4] recipe: h_a != h_b, fixed smooth fields
+    else:
+        w = wl.cfg4(n_side=64, n_wf=6, kin_form=1, n_steps=2)  # self-consistent SLDA on 64^3 (densities in the D items)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    if w.func_id:
+        for f in ("delta", "U_a", "rho_a", "nu"):
+            assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
