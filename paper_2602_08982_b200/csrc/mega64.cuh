@@ -54,28 +54,37 @@ __device__ __forceinline__ void f6_dit(cplx* x, int p) { fft_reg<32, false>(x); 
 __device__ __forceinline__ void f6_dif(cplx* x, int p) { F6Dif<0>::run(x, p); fft_reg<32, false>(x); }
 
 // forward 2-D transform of a plane held as interleaved lines along the slow axis (x[j] = (2 j + p, q)):
-// returns x[k] = (k_fast = k + 32 p, k_slow = q).  S = the 128-thread group's tile; CTA-wide barriers.
+// returns x[k] = (k_fast = k + 32 p, k_slow = q).  S = the 128-thread group's tile; CTA-wide barriers.  The two
+// line transforms share one loop body so that the unrolled butterflies exist once per kernel site (instruction cache).
 __device__ __forceinline__ void f6_plane_fwd(cplx* x, cplx* S, int q, int p) {
-  f6_dit(x, p);
+#pragma unroll 1
+  for (int pass = 0; pass < 2; ++pass) {
+    f6_dit(x, p);
+    if (pass == 0) {
 #pragma unroll
-  for (int k = 0; k < 32; ++k) S[(k + 32 * p) * F6_PITCH + q] = x[k];
-  __syncthreads();
+      for (int k = 0; k < 32; ++k) S[(k + 32 * p) * F6_PITCH + q] = x[k];
+      __syncthreads();
 #pragma unroll
-  for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + 2 * j + p];
-  __syncthreads();
-  f6_dit(x, p);
+      for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + 2 * j + p];
+      __syncthreads();
+    }
+  }
 }
 // inverse counterpart on conjugated data: in x[j] = conj spectrum (k_fast = j + 32 p, k_slow = q), out x[k] = conj of
 // the value at (slow = 2 k + p, fast = q)
 __device__ __forceinline__ void f6_plane_inv(cplx* x, cplx* S, int q, int p) {
-  f6_dif(x, p);
+#pragma unroll 1
+  for (int pass = 0; pass < 2; ++pass) {
+    f6_dif(x, p);
+    if (pass == 0) {
 #pragma unroll
-  for (int k = 0; k < 32; ++k) S[(2 * k + p) * F6_PITCH + q] = x[k];
-  __syncthreads();
+      for (int k = 0; k < 32; ++k) S[(2 * k + p) * F6_PITCH + q] = x[k];
+      __syncthreads();
 #pragma unroll
-  for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + j + 32 * p];
-  __syncthreads();
-  f6_dif(x, p);
+      for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + j + 32 * p];
+      __syncthreads();
+    }
+  }
 }
 
 struct F6Mega {
