@@ -29,7 +29,7 @@ struct Plan {
   size_t off_oc, oc_dpart_bytes;
   // 64^3 persistent kernels (mega64.cuh)
   int f6;
-  size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes;
+  size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes, f6_partn_bytes;
   int mega, gs, mG;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
@@ -117,14 +117,15 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   }
   P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40;
   if (const char* e = getenv("WSLDA_MEGA64")) if (atoi(e) == 0) P.f6 = 0;
-  P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = 0;
+  P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = P.f6_partn_bytes = 0;
   if (P.f6) {
     P.f6_ring_bytes = align_up((size_t)F6_RING * M * 16);
     P.f6_part_bytes = align_up((size_t)F3_NPART * 2 * n_wf * F6_N * 8);
     P.f6_acc_bytes = align_up((size_t)F6_RING * 4 * M * 8);
     P.f6_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * 2 * n_wf * sizeof(int));
     P.f6_pack_bytes = align_up((size_t)M * 48);
-    o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes;
+    P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
+    o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
   P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
   if (const char* e = getenv("WSLDA_ONCHIP")) if (atoi(e) == 0) P.oc = 0;
@@ -158,7 +159,7 @@ struct wslda_ctx {
   cplx* m_pack;
   double* oc_dpart;
   cplx *s_spec0, *s_spec1, *s_X, *s_pack;   // 64^3 rings
-  double *s_part, *s_acc;
+  double *s_part, *s_acc, *s_partn;
   F3Sync* s_sync;
   int mega_grid;
   double *f_part[4], *f_partn[4], *f_acc[4];
@@ -340,7 +341,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->s_part = (double*)b; b += P.f6_part_bytes;
     c->s_acc = (double*)b; b += P.f6_acc_bytes;
     c->s_sync = (F3Sync*)b; b += P.f6_sync_bytes;
-    c->s_pack = (cplx*)b;
+    c->s_pack = (cplx*)b; b += P.f6_pack_bytes;
+    c->s_partn = (double*)b;
     cudaFuncSetAttribute(k_f6_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);

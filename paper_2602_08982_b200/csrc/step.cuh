@@ -188,12 +188,20 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
     oc_launch(c, st, OC_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0, c->eps);
   } else if (c->P.f6 && (fixed || mask == (WSLDA_D_RHO | WSLDA_D_NU))) {   // 64^3 persistent kernels (mega64.cuh)
     const double* scg = c->f.normalize ? c->scale : nullptr;
-    for (int64_t n0 = 0; n0 < n_wf; n0 += P.chunk_n) {
-      const int64_t cnt = chunk_len(c, n0);
-      stage1(c, b, n0, cnt, st);
-      if (!fixed) dens_chunk(c, b.phi + 2 * n0 * M, scg ? scg + n0 : nullptr, n0, cnt, mask, n0 > 0, st);
+    if (fixed) {                                         // no density barrier: one predictor launch over the whole batch
+      WORK(c, 32.0 * M * n_wf * (1 + c->m + 2), 0);
+      LAUNCH(c, k_abm_combine, dim3(P.nblk, (unsigned)n_wf), P.pt_threads, 0, st, b.phi, b.h, b.cpart, b.k, M,
+             c->f.normalize ? c->s_partn : (double*)nullptr, P.nblk);
+      if (c->f.normalize)
+        LAUNCH(c, k_from_partials, nb(n_wf * 32, 128), 128, 0, st, c->s_partn, P.nblk, n_wf, c->dV, 1, c->scale, (double*)nullptr);
+    } else {
+      for (int64_t n0 = 0; n0 < n_wf; n0 += P.chunk_n) {
+        const int64_t cnt = chunk_len(c, n0);
+        stage1(c, b, n0, cnt, st);
+        dens_chunk(c, b.phi + 2 * n0 * M, scg ? scg + n0 : nullptr, n0, cnt, mask, n0 > 0, st);
+      }
+      potentials(c, st);
     }
-    if (!fixed) potentials(c, st);
     f6_mega(c, st, F3_CORR, b.phi, scg, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed);
     if (!fixed) {
       const int slots = (int)(n_wf < F6_RING ? n_wf : F6_RING);
