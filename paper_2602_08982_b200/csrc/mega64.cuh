@@ -53,36 +53,40 @@ __device__ __forceinline__ void f6_dit(cplx* x, int p) { fft_reg<32, false>(x); 
 // block line (x[j] = line[j + 32 p]) -> interleaved spectrum (x[k] = LINE[2 k + p])
 __device__ __forceinline__ void f6_dif(cplx* x, int p) { F6Dif<0>::run(x, p); fft_reg<32, false>(x); }
 
+// barrier over the 128 threads of one half (h = 0, 1): the halves work on independent planes in the transforms,
+// so they only meet at CTA-wide barriers where an item really needs both (C epilogue, dispatch)
+__device__ __forceinline__ void f6_half_sync(int h) { asm volatile("bar.sync %0, 128;" :: "r"(h + 1) : "memory"); }
+
 // forward 2-D transform of a plane held as interleaved lines along the slow axis (x[j] = (2 j + p, q)):
-// returns x[k] = (k_fast = k + 32 p, k_slow = q).  S = the 128-thread group's tile; CTA-wide barriers.  The two
+// returns x[k] = (k_fast = k + 32 p, k_slow = q).  S = the 128-thread group's tile; barriers over that group.  The two
 // line transforms share one loop body so that the unrolled butterflies exist once per kernel site (instruction cache).
-__device__ __forceinline__ void f6_plane_fwd(cplx* x, cplx* S, int q, int p) {
+__device__ __forceinline__ void f6_plane_fwd(cplx* x, cplx* S, int q, int p, int h) {
 #pragma unroll 1
   for (int pass = 0; pass < 2; ++pass) {
     f6_dit(x, p);
     if (pass == 0) {
 #pragma unroll
       for (int k = 0; k < 32; ++k) S[(k + 32 * p) * F6_PITCH + q] = x[k];
-      __syncthreads();
+      f6_half_sync(h);
 #pragma unroll
       for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + 2 * j + p];
-      __syncthreads();
+      f6_half_sync(h);
     }
   }
 }
 // inverse counterpart on conjugated data: in x[j] = conj spectrum (k_fast = j + 32 p, k_slow = q), out x[k] = conj of
 // the value at (slow = 2 k + p, fast = q)
-__device__ __forceinline__ void f6_plane_inv(cplx* x, cplx* S, int q, int p) {
+__device__ __forceinline__ void f6_plane_inv(cplx* x, cplx* S, int q, int p, int h) {
 #pragma unroll 1
   for (int pass = 0; pass < 2; ++pass) {
     f6_dif(x, p);
     if (pass == 0) {
 #pragma unroll
       for (int k = 0; k < 32; ++k) S[(2 * k + p) * F6_PITCH + q] = x[k];
-      __syncthreads();
+      f6_half_sync(h);
 #pragma unroll
       for (int j = 0; j < 32; ++j) x[j] = S[q * F6_PITCH + j + 32 * p];
-      __syncthreads();
+      f6_half_sync(h);
     }
   }
 }
@@ -134,7 +138,7 @@ __device__ __forceinline__ void f6_body_a(const F6Mega& a, const F3Pol& pol, int
       if (tt) f *= al[(2 * j + t.p) * F6_N + t.q];
       x[j] = cscale(x[j], f);
     }
-    f6_plane_fwd(x, S, t.q, t.p);
+    f6_plane_fwd(x, S, t.q, t.p, t.h);
     cplx* dst = (tt == 0 ? a.spec0 : a.spec1) + sb;
 #pragma unroll
     for (int k = 0; k < 32; ++k) st_pol(dst + (k + 32 * t.p) * F6_N + t.q, x[k], pol.keep);     // [kz][ky]
@@ -178,7 +182,7 @@ __device__ __forceinline__ void f6_body_c(const F6Mega& a, const F3Pol& pol, int
     for (int j = 0; j < 32; ++j) x[j] = ld_pol(sp + (j + 32 * t.p) * F6_N + t.q, pol.drop);   // (kz = j + 32 p, ky = q)
 #pragma unroll
     for (int j = 0; j < 32; ++j) x[j] = cconj(x[j]);
-    f6_plane_inv(x, S, t.q, t.p);                                  // conj of the value at (y = 2 k + p, z = q)
+    f6_plane_inv(x, S, t.q, t.p, t.h);                                  // conj of the value at (y = 2 k + p, z = q)
     const double* al = a.F.alpha[c] + pl;
 #pragma unroll
     for (int k = 0; k < 32; ++k) {
