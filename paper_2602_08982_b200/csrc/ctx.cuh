@@ -10,6 +10,7 @@
 #include "fast3d.cuh"
 #include "mega3d.cuh"
 #include "mega64.cuh"
+#include "mega32p.cuh"
 #include "kernels.cuh"
 
 struct Plan {
@@ -162,6 +163,7 @@ struct wslda_ctx {
   double *s_part, *s_acc, *s_partn;
   F3Sync* s_sync;
   int mega_grid;
+  int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
@@ -329,6 +331,16 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
     WS_MEGA_ATTR((k_f3_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<false, F3_RHS>));
 #undef WS_MEGA_ATTR
+    c->pair32 = 0;                   // measured slower than one thread per line (127k vs 141k spinor-steps/s): opt-in
+    if (const char* e = getenv("WSLDA_PAIR")) c->pair32 = atoi(e) != 0 && P.N[0] == 32;
+    if (c->pair32) {
+      cudaFuncSetAttribute(k_f5_mega<true, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+      cudaFuncSetAttribute(k_f5_mega<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+      cudaFuncSetAttribute(k_f5_mega<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+      cudaFuncSetAttribute(k_f5_mega<false, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+      cudaFuncSetAttribute(k_f5_mega<false, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+      cudaFuncSetAttribute(k_f5_mega<false, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
+    }
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
     c->mega_grid = best * sms;

@@ -78,6 +78,13 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   void (*k)(F3Mega);
   if (sym) k = mode == F3_APPLY ? k_f3_mega<true, F3_APPLY> : mode == F3_CORR ? k_f3_mega<true, F3_CORR> : k_f3_mega<true, F3_RHS>;
   else k = mode == F3_APPLY ? k_f3_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3_mega<false, F3_CORR> : k_f3_mega<false, F3_RHS>;
+  if (c->pair32) {                                         // 32^3: pair-of-threads lines, 256-thread CTAs
+    if (sym) k = mode == F3_APPLY ? k_f5_mega<true, F3_APPLY> : mode == F3_CORR ? k_f5_mega<true, F3_CORR> : k_f5_mega<true, F3_RHS>;
+    else k = mode == F3_APPLY ? k_f5_mega<false, F3_APPLY> : mode == F3_CORR ? k_f5_mega<false, F3_CORR> : k_f5_mega<false, F3_RHS>;
+    LAUNCHN(c, mode == F3_APPLY ? "k_f5_mega_apply" : mode == F3_CORR ? "k_f5_mega_corr" : "k_f5_mega_rhs", k, grid, F5_THREADS,
+            4 * F3_TILE_BYTES, st, a);
+    return;
+  }
   LAUNCHN(c, mode == F3_APPLY ? "k_f3_mega_apply" : mode == F3_CORR ? "k_f3_mega_corr" : "k_f3_mega_rhs", k, grid, 128,
           4 * F3_TILE_BYTES, st, a);
 }

@@ -314,15 +314,15 @@ __device__ __forceinline__ void f3_body_c(const F3Mega& a, const F3Pol& pol, int
 // ---- D: per-spinor scalars of the group, then the final combination of half an x-plane for every spinor ---------
 // CORR: phi_new = (X + i kappa eps w) * scale_new over P (Alg. 2 steps 4, 8) + densities of phi_new;
 // RHS : f_new = Y + i eps phi (Alg. 2 step 9, Eq. 45b).
-template <int MODE>
+template <int MODE, int NT = 128>
 __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int g, int id, double* s_eps, double* s_sn) {
-  constexpr int PTS = F3_PLANE / F3_DSPLIT / 128;
+  constexpr int PTS = F3_PLANE / F3_DSPLIT / NT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ix = id / F3_DSPLIT, half = id - ix * F3_DSPLIT;
   const int cnt = (a.n - g * a.gs < a.gs) ? a.n - g * a.gs : a.gs;
   const size_t M = (size_t)a.NX * F3_PLANE, np = (size_t)a.n * a.NX;
   F3_T0();
-  for (int nl = warp; nl < cnt; nl += 4) {
+  for (int nl = warp; nl < cnt; nl += NT / 32) {
     const int n = g * a.gs + nl;
     double v[F3_NPART];
 #pragma unroll
@@ -358,7 +358,7 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
     if (nl + 1 < cnt && (threadIdx.x & 7) == 0) {                 // one request per 128-byte line
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        f3_pf1(pu + 2 * M + r * 128); f3_pf1(pu + 3 * M + r * 128);
+        f3_pf1(pu + 2 * M + r * NT); f3_pf1(pu + 3 * M + r * NT);
       }
     }
     if (MODE == F3_CORR) {
@@ -367,7 +367,7 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
       cplx gxu[PTS], gxv[PTS], gpu[PTS], gpv[PTS];          // all loads of this spinor first, then the arithmetic
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        gxu[r] = __ldcg(Xu + r * 128); gxv[r] = __ldcg(Xu + M + r * 128); gpu[r] = pu[r * 128]; gpv[r] = pu[M + r * 128];
+        gxu[r] = __ldcg(Xu + r * NT); gxv[r] = __ldcg(Xu + M + r * NT); gpu[r] = pu[r * NT]; gpv[r] = pu[M + r * NT];
       }
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
@@ -375,21 +375,21 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
         const cplx wu = cscale(gpu[r], sP), wv = cscale(gpv[r], sP);
         const cplx u = make_double2((xu.x - ke * wu.y) * sn, (xu.y + ke * wu.x) * sn);
         const cplx v = make_double2((xv.x - ke * wv.y) * sn, (xv.y + ke * wv.x) * sn);
-        st_pol_nb(ou + r * 128, u, pol.drop); st_pol_nb(ou + M + r * 128, v, pol.drop);
+        st_pol_nb(ou + r * NT, u, pol.drop); st_pol_nb(ou + M + r * NT, v, pol.drop);
         if (a.do_dens) f3_dens_add(acc[r], u, v, cp, wa, wb);
       }
     } else {
       cplx gxu[PTS], gxv[PTS], gpu[PTS], gpv[PTS];
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
-        gxu[r] = __ldcg(Xu + r * 128); gxv[r] = __ldcg(Xu + M + r * 128); gpu[r] = pu[r * 128]; gpv[r] = pu[M + r * 128];
+        gxu[r] = __ldcg(Xu + r * NT); gxv[r] = __ldcg(Xu + M + r * NT); gpu[r] = pu[r * NT]; gpv[r] = pu[M + r * NT];
       }
 #pragma unroll
       for (int r = 0; r < PTS; ++r) {
         const cplx yu = gxu[r], yv = gxv[r];
         const cplx u = gpu[r], v = gpv[r];
-        st_pol_nb(ou + r * 128, make_double2(yu.x - e * u.y, yu.y + e * u.x), pol.drop);
-        st_pol_nb(ou + M + r * 128, make_double2(yv.x - e * v.y, yv.y + e * v.x), pol.drop);
+        st_pol_nb(ou + r * NT, make_double2(yu.x - e * u.y, yu.y + e * u.x), pol.drop);
+        st_pol_nb(ou + M + r * NT, make_double2(yv.x - e * v.y, yv.y + e * v.x), pol.drop);
       }
     }
   }
@@ -400,7 +400,7 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
     for (int r = 0; r < PTS; ++r)
 #pragma unroll
       for (int f = 0; f < 4; ++f) {
-        double* q = ac + f * M + r * 128;
+        double* q = ac + f * M + r * NT;
         *q = (g < F3_RING ? 0.0 : __ldcg(q)) + acc[r][f];
       }
   }
@@ -409,7 +409,7 @@ __device__ __forceinline__ void f3_body_d(const F3Mega& a, const F3Pol& pol, int
 // Cooperative L2 prefetch: every item of tick t fetches its 1/IT share of the read-only inputs the NEXT tick
 // will read from HBM -- psi of group t+1 (A items) and C_part of group t-1 (C items of tick t+1) -- so that those
 // loads find their lines in L2.  Needs no ticket look-ahead, hence adds no dependency latency.
-template <int MODE>
+template <int MODE, int NT = 128>
 __device__ __forceinline__ void f3_prefetch_tick(const F3Mega& a, int tick, int r, int chunk, int lines) {
   const size_t M = (size_t)a.NX * F3_PLANE;
   const int lpc = (int)(M * 16 / 128) * 2;                        // 128-byte lines per spinor
@@ -419,12 +419,12 @@ __device__ __forceinline__ void f3_prefetch_tick(const F3Mega& a, int tick, int 
   if (ga < a.G) {
     const int rem = a.n - ga * a.gs, lim = (rem < a.gs ? rem : a.gs) * lpc;
     const char* base = (const char*)(a.psi + (size_t)ga * a.gs * 2 * M);
-    for (int q = q0; q < q1 && q < lim; q += 128) f3_pf(base + (size_t)q * 128);
+    for (int q = q0; q < q1 && q < lim; q += NT) f3_pf(base + (size_t)q * 128);
   }
   if (MODE == F3_CORR && gc >= 0 && gc < a.G) {
     const int rem = a.n - gc * a.gs, lim = (rem < a.gs ? rem : a.gs) * lpc;
     const char* base = (const char*)(a.cpart + (size_t)gc * a.gs * 2 * M);
-    for (int q = q0; q < q1 && q < lim; q += 128) f3_pf(base + (size_t)q * 128);
+    for (int q = q0; q < q1 && q < lim; q += NT) f3_pf(base + (size_t)q * 128);
   }
 }
 
