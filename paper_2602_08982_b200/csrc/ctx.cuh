@@ -10,6 +10,7 @@
 #include "fast3d.cuh"
 #include "mega3d.cuh"
 #include "mega64.cuh"
+#include "mega64s.cuh"
 #include "mega32p.cuh"
 #include "kernels.cuh"
 
@@ -123,7 +124,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.f6_ring_bytes = align_up((size_t)F6_RING * M * 16);
     P.f6_part_bytes = align_up((size_t)F3_NPART * 2 * n_wf * F6_N * 8);
     P.f6_acc_bytes = align_up((size_t)F6_RING * 4 * M * 8);
-    P.f6_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * 2 * n_wf * sizeof(int));
+    P.f6_sync_bytes = align_up(sizeof(F3Sync) + (size_t)5 * 2 * n_wf * sizeof(int));
     P.f6_pack_bytes = align_up((size_t)M * 48);
     P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
@@ -163,6 +164,7 @@ struct wslda_ctx {
   double *s_part, *s_acc, *s_partn;
   F3Sync* s_sync;
   int mega_grid;
+  int f6_version;                  // 64^3 tiling: 1 = two planes per 256-thread CTA, 2 = one plane per 128-thread CTA
   int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -358,6 +360,11 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f6_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
+    cudaFuncSetAttribute(k_f6s_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
+    cudaFuncSetAttribute(k_f6s_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
+    cudaFuncSetAttribute(k_f6s_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
+    c->f6_version = 1;               // measured: 11.5k (two planes per CTA) vs 10.0k (one plane per CTA) spinor-steps/s
+    if (const char* e = getenv("WSLDA_MEGA64_V")) c->f6_version = atoi(e) == 2 ? 2 : 1;
   }
   if (P.oc) c->oc_dpart = (double*)(base + P.off_oc);
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1

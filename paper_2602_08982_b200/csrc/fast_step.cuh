@@ -112,17 +112,24 @@ static void f6_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.do_dens = do_dens;
   a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.acc = c->s_acc; a.sync = c->s_sync;
   a.n = (int)n; a.G = (int)(2 * n);
-  cudaMemsetAsync(c->s_sync, 0, sizeof(F3Sync) + (size_t)4 * a.G * sizeof(int), st);
+  cudaMemsetAsync(c->s_sync, 0, sizeof(F3Sync) + (size_t)5 * a.G * sizeof(int), st);
   LAUNCH(c, k_f3_pack, nb(P.M, 256), 256, 0, st, a.F, 1, P.M, c->s_pack);
-  const int IT = F6_N / 2 + F6_N / 2 + F6_N + (mode == F3_APPLY ? 0 : F6_ND);
-  const long total = (long)(a.G + 4) * IT;
-  int sms = 148;
-  const int grid = (int)(total < sms ? total : sms);
   const double M = (double)P.M;
   WORK(c, M * n * (mode == F3_CORR ? 96.0 : 64.0), 5.0 * M * 18.0 * 2.0 * 2 * 2 * n);
-  void (*k)(F6Mega) = mode == F3_APPLY ? k_f6_mega<F3_APPLY> : mode == F3_CORR ? k_f6_mega<F3_CORR> : k_f6_mega<F3_RHS>;
-  LAUNCHN(c, mode == F3_APPLY ? "k_f6_mega_apply" : mode == F3_CORR ? "k_f6_mega_corr" : "k_f6_mega_rhs", k, grid, F6_THREADS,
-          2 * F6_TILE * 16, st, a);
+  const char* name = mode == F3_APPLY ? "k_f6_mega_apply" : mode == F3_CORR ? "k_f6_mega_corr" : "k_f6_mega_rhs";
+  if (c->f6_version == 2) {                                // one plane per 128-thread CTA, two CTAs per SM
+    const int IT = 4 * F6_N + (mode == F3_APPLY ? 0 : (int)F6S_ND);
+    const long total = (long)(a.G + 5) * IT;
+    const int grid = (int)(total < 296 ? total : 296);
+    void (*k)(F6Mega) = mode == F3_APPLY ? k_f6s_mega<F3_APPLY> : mode == F3_CORR ? k_f6s_mega<F3_CORR> : k_f6s_mega<F3_RHS>;
+    LAUNCHN(c, name, k, grid, F6S_THREADS, F6_TILE * 16, st, a);
+  } else {
+    const int IT = F6_N / 2 + F6_N / 2 + F6_N + (mode == F3_APPLY ? 0 : F6_ND);
+    const long total = (long)(a.G + 4) * IT;
+    const int grid = (int)(total < 148 ? total : 148);
+    void (*k)(F6Mega) = mode == F3_APPLY ? k_f6_mega<F3_APPLY> : mode == F3_CORR ? k_f6_mega<F3_CORR> : k_f6_mega<F3_RHS>;
+    LAUNCHN(c, name, k, grid, F6_THREADS, 2 * F6_TILE * 16, st, a);
+  }
 }
 
 static void f3_scal(wslda_ctx* c, int q, cudaStream_t st, int64_t n0, int cnt, int mode, int use_shift, double kappa,

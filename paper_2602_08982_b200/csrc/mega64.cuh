@@ -18,7 +18,7 @@
 #define F6_PITCH 65
 #define F6_PLANE (F6_N * F6_N)
 #define F6_TILE (F6_N * F6_PITCH)
-#define F6_RING 5
+#define F6_RING 6
 #define F6_THREADS 256
 #define F6_M ((size_t)F6_N * F6_PLANE)
 #define F6_ND 256              // D items per spinor (1024 points of both components each)
@@ -106,7 +106,7 @@ struct F6Mega {
   double* eps_out;
   int use_shift, normalize, do_dens;
   const double *cpref, *w_a, *w_b;
-  double* acc;                 // ring [F6_RING][4][M]  (slot of the spinor's odd group)
+  double* acc;                 // ring [F6_RING][4][M]  (slot n % F6_RING)
   F3Sync* sync;                // followed by done[4][G]
   int n, G;                    // spinors, groups = 2 n
 };
@@ -252,7 +252,7 @@ __device__ __forceinline__ void f6_body_c(const F6Mega& a, const F3Pol& pol, int
 
 // ---- D: per spinor n (dispatched with its odd component group): scalars from both components' partial sums, then
 // 1024 points of both components per item: CORR phi_new = (X + i kappa eps w) s_n (+ densities), RHS f = Y + i eps phi --
-template <int MODE>
+template <int MODE, int NT = F6_THREADS>
 __device__ __forceinline__ void f6_body_d(const F6Mega& a, const F3Pol& pol, int n, int id, double* s_sc) {
   const int tid = threadIdx.x, lane = tid & 31;
   const size_t np = (size_t)a.G * F6_N;
@@ -279,7 +279,7 @@ __device__ __forceinline__ void f6_body_d(const F6Mega& a, const F3Pol& pol, int
   }
   __syncthreads();
   const double e = s_sc[0], sn = s_sc[1];
-  const size_t p0 = (size_t)id * 1024 + tid;
+  const size_t p0 = (size_t)id * (4 * NT) + tid;
   const cplx* Xu = a.X + (size_t)((2 * n) % F6_RING) * F6_M + p0;
   const cplx* Xv = a.X + (size_t)((2 * n + 1) % F6_RING) * F6_M + p0;
   const cplx* pu = a.psi + (size_t)(2 * n) * F6_M + p0;
@@ -287,24 +287,24 @@ __device__ __forceinline__ void f6_body_d(const F6Mega& a, const F3Pol& pol, int
   cplx gxu[4], gxv[4], gpu[4], gpv[4];
 #pragma unroll
   for (int r = 0; r < 4; ++r) {
-    gxu[r] = __ldcg(Xu + r * 256); gxv[r] = __ldcg(Xv + r * 256); gpu[r] = pu[r * 256]; gpv[r] = pu[F6_M + r * 256];
+    gxu[r] = __ldcg(Xu + r * NT); gxv[r] = __ldcg(Xv + r * NT); gpu[r] = pu[r * NT]; gpv[r] = pu[F6_M + r * NT];
   }
   if (MODE == F3_CORR) {
     const double sP = a.scale ? a.scale[n] : 1.0, ke = a.kappa * e;
     const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n];
-    double* ac = a.acc + (size_t)((2 * n + 1) % F6_RING) * 4 * F6_M + p0;
+    double* ac = a.acc + (size_t)(n % F6_RING) * 4 * F6_M + p0;
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
       const cplx wu = cscale(gpu[r], sP), wv = cscale(gpv[r], sP);
       const cplx u = make_double2((gxu[r].x - ke * wu.y) * sn, (gxu[r].y + ke * wu.x) * sn);
       const cplx v = make_double2((gxv[r].x - ke * wv.y) * sn, (gxv[r].y + ke * wv.x) * sn);
-      st_pol_nb(ou + r * 256, u, pol.drop); st_pol_nb(ou + F6_M + r * 256, v, pol.drop);
+      st_pol_nb(ou + r * NT, u, pol.drop); st_pol_nb(ou + F6_M + r * NT, v, pol.drop);
       if (a.do_dens) {
         double d4[4] = {0.0, 0.0, 0.0, 0.0};
         f3_dens_add(d4, u, v, cp, wa, wb);
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
-          double* qd = ac + f * F6_M + r * 256;
+          double* qd = ac + f * F6_M + r * NT;
           *qd = (n < F6_RING ? 0.0 : __ldcg(qd)) + d4[f];
         }
       }
@@ -312,8 +312,8 @@ __device__ __forceinline__ void f6_body_d(const F6Mega& a, const F3Pol& pol, int
   } else {
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-      st_pol_nb(ou + r * 256, make_double2(gxu[r].x - e * gpu[r].y, gxu[r].y + e * gpu[r].x), pol.drop);
-      st_pol_nb(ou + F6_M + r * 256, make_double2(gxv[r].x - e * gpv[r].y, gxv[r].y + e * gpv[r].x), pol.drop);
+      st_pol_nb(ou + r * NT, make_double2(gxu[r].x - e * gpu[r].y, gxu[r].y + e * gpu[r].x), pol.drop);
+      st_pol_nb(ou + F6_M + r * NT, make_double2(gxv[r].x - e * gpv[r].y, gxv[r].y + e * gpv[r].x), pol.drop);
     }
   }
 }

@@ -220,6 +220,20 @@ def _kernels_of(g, fn):
     return list(rep)
 
 
+def test_fast3d_multikernel_fallback(small_fast_chunks, monkeypatch):
+    """WSLDA_MEGA=0: the three-pass chunk pipeline on concurrent streams (fast3d.cuh kernels) instead of the persistent kernel."""
+    monkeypatch.setenv("WSLDA_MEGA", "0")
+    w = wl.cfg4(n_side=32, n_wf=10, kin_form=1, n_steps=3)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    assert "k_f3_pass_c" in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+
+
 @pytest.mark.parametrize("kin_form", [0, 1])
 def test_pair_line_kernel_32cubed(small_fast_chunks, monkeypatch, kin_form):
     """The opt-in pair-of-threads 32^3 stage kernel (mega32p.cuh, WSLDA_PAIR=1): H psi and self-consistent steps."""
@@ -336,8 +350,11 @@ def test_mega64_apply_h():
     assert relerr(h2[1:3], ref[1:3]) < TOL_H and not h2[:1].any()
 
 
-@pytest.mark.parametrize("case", ["cfg5_fixed", "slda_selfconsistent"])
-def test_mega64_abm_matches_oracle(case):
+@pytest.mark.parametrize("case", ["cfg5_fixed", "slda_selfconsistent", "cfg5_fixed_one_plane_per_cta"])
+def test_mega64_abm_matches_oracle(case, monkeypatch):
+    if case.endswith("one_plane_per_cta"):
+        monkeypatch.setenv("WSLDA_MEGA64_V", "2")            # the opt-in tiling of mega64s.cuh
+        case = "cfg5_fixed"
     if case == "cfg5_fixed":
         w = wl.cfg5(n_wf=7, n_steps=3)                       # configs[4] recipe: h_a != h_b, fixed smooth fields
     else:
