@@ -215,11 +215,13 @@ static inline void prof_end(wslda_ctx* c, cudaStream_t st) { cudaEventRecord((*c
 #define WORK(c, bytes, flops) do { (c)->work_bytes = (double)(bytes); (c)->work_flops = (double)(flops); } while (0)
 
 // stored position p of the in-place DIF transform (radix 8 from L = n down, then the remaining 4 or 2) <-> frequency index
+static int ws_fft_radix() { const char* e = getenv("WSLDA_FFT_RADIX"); return (e && atoi(e) == 4) ? 4 : 8; }
 static void scrambled_freq(int n, std::vector<int>& fr) {
   fr.resize(n);
+  const int maxr = ws_fft_radix();
   for (int p = 0; p < n; ++p) {
     int L = n, rem = p, k = 0, mult = 1;
-    while (L > 1) { int r = (L >= 8) ? 8 : L, sub = L / r, m = rem / sub; rem %= sub; k += m * mult; mult *= r; L = sub; }
+    while (L > 1) { int r = (L >= maxr) ? maxr : L, sub = L / r, m = rem / sub; rem %= sub; k += m * mult; mult *= r; L = sub; }
     fr[p] = k;
   }
 }
@@ -255,6 +257,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->dx[d] = dx[d];
     if (d < P.nd) c->dV *= dx[d]; else c->Lperp *= dims[d] * dx[d];
   }
+  { const int lgr = ws_fft_radix() == 4 ? 2 : 3; cudaMemcpyToSymbol(g_ws_lgr, &lgr, sizeof(int)); }
   char* base = (char*)ws;
   const int64_t M = P.M;
   Lat& L = c->L;

@@ -50,19 +50,26 @@ __device__ inline void fft_stage(cplx* s, int A, int lgn, int lgL, int lgB, cons
   __syncthreads();
 }
 
+// largest radix of the plan (log2): 3 = radix 8, 2 = radix 4; set once per process from WSLDA_FFT_RADIX (ctx.cuh keeps
+// the permuted k-tables consistent with it)
+__device__ int g_ws_lgr = 3;
+
 template <bool INV>
 __device__ inline void fft_axis(cplx* s, int A, int lgn, int lgB, const cplx* __restrict__ tw) {
   if (lgn == 0) return;
-  const int rem = lgn % 3;                                     // last (smallest) stage: radix 2^rem
+  const int lgr = g_ws_lgr, rem = lgn % lgr;                   // last (smallest) stage: radix 2^rem
   if (!INV) {
-    int lgL = lgn;
-    for (; lgL >= 3; lgL -= 3) fft_stage<false, 8>(s, A, lgn, lgL, lgB, tw);
+    for (int lgL = lgn; lgL >= lgr; lgL -= lgr) {
+      if (lgr == 3) fft_stage<false, 8>(s, A, lgn, lgL, lgB, tw); else fft_stage<false, 4>(s, A, lgn, lgL, lgB, tw);
+    }
     if (rem == 2) fft_stage<false, 4>(s, A, lgn, 2, lgB, tw);
     else if (rem == 1) fft_stage<false, 2>(s, A, lgn, 1, lgB, tw);
   } else {
     if (rem == 2) fft_stage<true, 4>(s, A, lgn, 2, lgB, tw);
     else if (rem == 1) fft_stage<true, 2>(s, A, lgn, 1, lgB, tw);
-    for (int lgL = rem + 3; lgL <= lgn; lgL += 3) fft_stage<true, 8>(s, A, lgn, lgL, lgB, tw);
+    for (int lgL = rem + lgr; lgL <= lgn; lgL += lgr) {
+      if (lgr == 3) fft_stage<true, 8>(s, A, lgn, lgL, lgB, tw); else fft_stage<true, 4>(s, A, lgn, lgL, lgB, tw);
+    }
   }
 }
 
