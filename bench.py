@@ -90,7 +90,7 @@ class ClockSampler:
     def __init__(self, index):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
-            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                                        "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -233,6 +233,7 @@ def run_gpu(args):
     hist = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(g.m)]
     torch.cuda.synchronize()
     hist = g.abm_init(phi, hist, w.dt, 0)            # zero-history start: the timed steps are plain Alg. 2 steps
+    sampler = ClockSampler(local) if rank == 0 else None      # samples through the warm-up and the timed steps (same load)
     for _ in range(args.warmup):
         hist = g.abm_step(phi, hist, w.dt)
     torch.cuda.synchronize()
@@ -242,7 +243,6 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    sampler = ClockSampler(local) if rank == 0 else None
     barrier()
     l0 = g.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
