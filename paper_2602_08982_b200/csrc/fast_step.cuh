@@ -196,7 +196,7 @@ static void f3_stage1(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int
   HistPtrs h = s.h;
   for (int j = 0; j < 5; ++j) if (h.f[j]) h.f[j] += off;
   WORK(c, 32.0 * P.M * cnt * (1 + c->m + 2), 0);
-  LAUNCH(c, k_abm_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, s.phi + off, h, s.cpart + off, s.k, P.M,
+  LAUNCH(c, k_f3_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, s.phi + off, h, s.cpart + off, s.k, P.M,
          c->f.normalize ? c->f_partn[q] : (double*)nullptr, P.nblk);
   if (c->f.normalize)
     LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->f_partn[q], P.nblk, (int64_t)cnt, c->dV, 1, c->scale + n0, (double*)nullptr);

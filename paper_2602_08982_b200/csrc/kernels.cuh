@@ -35,6 +35,41 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_abm_combine(cplx* phi, HistPt
 }
 
 // per-block partial sums of |psi|^2 only (norm of an existing buffer)
+// The same predictor sweep for the fused 3-D path (chunks of a few dozen MB on concurrent streams): the history and
+// phi are read for the last time in this stage (L2 evict_first), C_part is not needed before the next stage
+// (evict_first), while P is re-read by the density kernel of the same chunk and must stay in L2 (evict_last).
+__global__ void __launch_bounds__(WS_PT_THREADS) k_f3_combine(cplx* phi, HistPtrs h, cplx* cpart, AbmCoef k, int64_t M,
+                                                              double* part, int nblk) {
+  __shared__ double sh[32];
+  const F3Pol pol = f3_policies();
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, n = blockIdx.y;
+  double acc = 0.0;
+  if (i < M) {
+    cplx p0[2], fh[2][5];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {                               // all loads of the point first
+      const int64_t o = (2 * n + c) * M + i;
+      p0[c] = ld_pol(phi + o, pol.drop);
+#pragma unroll
+      for (int j = 0; j < 5; ++j)
+        if (j < k.ab || j + 1 < k.am) fh[c][j] = ld_pol(h.f[j] + o, pol.drop);
+    }
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int64_t o = (2 * n + c) * M + i;
+      cplx p = p0[c], q = p;
+#pragma unroll
+      for (int j = 0; j < 5; ++j) {
+        if (j < k.ab) { p.x += k.b[j] * fh[c][j].x; p.y += k.b[j] * fh[c][j].y; }
+        if (j + 1 < k.am) { q.x += k.c[j + 1] * fh[c][j].x; q.y += k.c[j + 1] * fh[c][j].y; }
+      }
+      st_pol_nb(phi + o, p, pol.keep); st_pol_nb(cpart + o, q, pol.drop);
+      acc += cabs2(p);
+    }
+  }
+  if (part) { double r = block_sum(acc, sh); if (threadIdx.x == 0) part[n * nblk + blockIdx.x] = r; }
+}
+
 __global__ void __launch_bounds__(WS_PT_THREADS) k_norm_partials(const cplx* psi, int64_t M, double* part, int nblk) {
   __shared__ double sh[32];
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, n = blockIdx.y;
