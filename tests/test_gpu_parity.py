@@ -365,3 +365,75 @@ def test_mega64_abm_matches_oracle(case, monkeypatch):
     if w.func_id:
         for f in ("delta", "U_a", "rho_a", "nu"):
             assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+
+
+# ---- the other configs at BASELINE.json's full size, on seeded samples (same technique as configs[3] above) ----------
+def _full_size_sampled(w, n_sample, n_steps, seed):
+    import copy
+    import torch
+    shape = (w.n_wf, 2) + w.shape
+    need = (2 + w.history) * w.n_wf * 32 * w.M + 3e9
+    if torch.cuda.mem_get_info()[0] < need:
+        pytest.skip("not enough free device memory for the full-size batch")
+    u = wl.uniform01(seed, 0, n_sample)
+    sample = sorted(set([0, 1, w.n_wf - 1] + [int(x * w.n_wf) for x in u]))
+    S = len(sample)
+    wa, wb = np.zeros(w.n_wf), np.zeros(w.n_wf)
+    wa[sample], wb[sample] = w.w_a[sample], w.w_b[sample]
+    if not (wa[sample].any() or wb[sample].any()):
+        wb[sample] = 1.0                                           # make sure the sample carries density
+    wf = copy.copy(w); wf.w_a, wf.w_b = wa, wb
+    g = make_gpu(wf)
+    phi = torch.empty(shape, dtype=torch.complex128, device="cuda")
+    wl.spinors_device(w, 0, w.n_wf, phi)
+    psi_s = to_np(phi[sample])
+    ws_ = copy.copy(w); ws_.n_wf = S; ws_.w_a, ws_.w_b = wa[sample], wb[sample]
+    if w.kperp is not None:                                        # one mode entry per sampled spinor
+        mo = np.asarray(w.mode_of)[sample]
+        ws_.kperp, ws_.mult = np.asarray(w.kperp)[mo], np.asarray(w.mult)[mo]
+        ws_.first = np.arange(S + 1, dtype=np.int64)
+        ws_.mode_of = np.arange(S)
+    o = make_oracle(ws_)
+    hist = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(g.m)]
+    if w.func_id:
+        o.densities(psi_s); o.update_potentials()
+        g.densities(phi); g.update_potentials()
+        for f in ("rho_a", "rho_b", "nu", "delta", "U_a"):
+            assert relerr(to_np(g.get_field(f)), o.get_field(f)) < TOL_D, f
+    h, e = g.apply_h(phi, hpsi=hist[0])
+    href, eref = o.apply_h(psi_s)
+    assert relerr(to_np(h[sample]), href) < TOL_H
+    assert relerr(to_np(e[sample]), eref) < TOL_H
+    hist[0].zero_()
+    phi_o = psi_s.copy()
+    hist_o = [np.zeros_like(psi_s) for _ in range(o.m)]
+    hist_o = o.abm_init(phi_o, hist_o, w.dt, 0)
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    for _ in range(n_steps):
+        hist_o = o.abm_step(phi_o, hist_o, w.dt)
+        hist = g.abm_step(phi, hist, w.dt)
+    assert relerr(to_np(phi[sample]), phi_o) < TOL_ABM
+    assert relerr(to_np(hist[0][sample]), hist_o[0]) < TOL_ABM
+    if w.func_id:
+        for f in ("delta", "U_a", "rho_a"):
+            assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-9, f
+    nd = len(w.shape)
+    nrm = torch.sum(phi.real ** 2 + phi.imag ** 2, dim=tuple(range(1, nd + 2))) * w.dV
+    assert float(torch.max(torch.abs(nrm - 1.0))) < 1e-12
+    del phi, hist, h
+    torch.cuda.empty_cache()
+
+
+def test_cfg2_full_size_sampled_against_oracle():
+    """configs[1]: quasi-1D, 262144 spinors over 1024 transverse modes, self-consistent (fused on-chip stages)."""
+    _full_size_sampled(wl.cfg2(), 96, 2, 5151)
+
+
+def test_cfg3_full_size_sampled_against_oracle():
+    """configs[2]: quasi-2D 64^2, 65536 spinors over 16 k_z modes, vortex imprint, self-consistent."""
+    _full_size_sampled(wl.cfg3(), 40, 2, 5252)
+
+
+def test_cfg5_full_size_sampled_against_oracle():
+    """configs[4]: 64^3, 2048 resident spinors, fixed smooth h_a != h_b fields (64^3 persistent kernels)."""
+    _full_size_sampled(wl.cfg5(n_wf=2048), 10, 2, 5353)
