@@ -9,6 +9,7 @@
 #include "fft_large.cuh"
 #include "fast3d.cuh"
 #include "mega3d.cuh"
+#include "cluster3d.cuh"
 #include "mega64.cuh"
 #include "mega64s.cuh"
 #include "mega32p.cuh"
@@ -165,6 +166,7 @@ struct wslda_ctx {
   F3Sync* s_sync;
   int mega_grid;
   int f6_version;                  // 64^3 tiling: 1 = two planes per 256-thread CTA, 2 = one plane per 128-thread CTA
+  int c3, c3_grid;                 // 32^3: H psi inside one thread-block cluster (cluster3d.cuh); grid = clusters x 8
   int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -321,6 +323,21 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
+  }
+  c->c3 = 0; c->c3_grid = 0;
+  if (const char* e = getenv("WSLDA_CLUSTER")) c->c3 = atoi(e) != 0 && P.fast && P.N[0] == 32;
+  if (c->c3) {
+    int ncl = 0;
+#define WS_C3_ATTR(K) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, C3_SMEM); \
+      cudaLaunchConfig_t lc = {}; lc.gridDim = dim3(C3_CS * 64); lc.blockDim = dim3(C3_NT); lc.dynamicSmemBytes = C3_SMEM; \
+      int v = 0; if (cudaOccupancyMaxActiveClusters(&v, K, &lc) == cudaSuccess && v > 0 && (ncl == 0 || v < ncl)) ncl = v; } while (0)
+    WS_C3_ATTR((k_c3_hpsi<true, F3_APPLY>)); WS_C3_ATTR((k_c3_hpsi<true, F3_CORR>)); WS_C3_ATTR((k_c3_hpsi<true, F3_RHS>));
+    WS_C3_ATTR((k_c3_hpsi<false, F3_APPLY>)); WS_C3_ATTR((k_c3_hpsi<false, F3_CORR>)); WS_C3_ATTR((k_c3_hpsi<false, F3_RHS>));
+#undef WS_C3_ATTR
+    cudaGetLastError();
+    if (ncl <= 0) ncl = 16;
+    if (const char* e = getenv("WSLDA_CLUSTERS")) { int v = atoi(e); if (v > 0) ncl = v; }
+    c->c3_grid = ncl * C3_CS;
   }
   if (P.mega) {
     char* b = base + P.off_mega;

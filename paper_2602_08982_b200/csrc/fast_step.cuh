@@ -25,6 +25,20 @@ static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk,
   const bool sym = c->f.kin_form == WSLDA_KIN_SYM40;
   const int nspec = sym ? 2 : 1;
   const double fl_plane = 5.0 * M * 10.0 * 2 * cnt * nspec, fl_x = 5.0 * M * P.lg[0] * 2.0 * 2 * cnt * nspec;
+  if (c->c3) {                                             // the three passes inside one thread-block cluster per spinor
+    C3Args k;
+    k.psi = psi_chunk; k.scale = scale_chunk; k.kperp2 = c->kperp2 + n0; k.F = f3_fields(c);
+    k.ky2 = c->k2n[1]; k.kz2 = c->k2n[2];
+    for (int j = 0; j < 32; ++j) k.kx2[j] = c->hk2[0][j];
+    k.invM = c->L.invM; k.kappa = kappa; k.out = out; k.cpart = cpart; k.part = c->f_part[q]; k.cnt = cnt;
+    const int want = cnt * C3_CS, grid = want < c->c3_grid ? want : c->c3_grid;
+    WORK(c, (mode == F3_RHS ? 32.0 : 64.0) * M * cnt, 2 * fl_plane + fl_x);
+    void (*kc)(C3Args);
+    if (sym) kc = mode == F3_APPLY ? k_c3_hpsi<true, F3_APPLY> : mode == F3_CORR ? k_c3_hpsi<true, F3_CORR> : k_c3_hpsi<true, F3_RHS>;
+    else kc = mode == F3_APPLY ? k_c3_hpsi<false, F3_APPLY> : mode == F3_CORR ? k_c3_hpsi<false, F3_CORR> : k_c3_hpsi<false, F3_RHS>;
+    LAUNCHN(c, "k_c3_hpsi", kc, grid, C3_NT, C3_SMEM, st, k);
+    return;
+  }
   F3PassA a;
   a.psi = psi_chunk; a.scale = scale_chunk; a.alpha[0] = c->alpha_a; a.alpha[1] = c->alpha_b;
   a.spec0 = c->f_spec0[q]; a.spec1 = c->f_spec1[q]; a.n_items = cnt * 2 * NX; a.NX = NX;
@@ -151,7 +165,7 @@ static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double
     }
     return cuda_check(c, "apply_h");
   }
-  if (c->P.mega && n_count > 0) {
+  if (c->P.mega && !c->c3 && n_count > 0) {
     f3_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0);
     F3Scal s;
     s.part = c->m_part; s.cnt = (int)n_count; s.NX = c->P.N[0]; s.mode = F3_APPLY; s.use_shift = 1; s.normalize = 0;
@@ -244,7 +258,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
   const int used = (int)(n_chunks < ns ? n_chunks : ns);
   auto cnt_of = [&](int64_t k) { return (int)((n_wf - k * fc < fc) ? n_wf - k * fc : fc); };
   const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
-  if (P.mega) {                                          // stage 1 in chunks, stages 2 and 3 as persistent dataflow kernels
+  if (P.mega && !c->c3) {                                // stage 1 in chunks, stages 2 and 3 as persistent dataflow kernels
     f3_fork(c, s);
     for (int64_t k = 0; k < n_chunks; ++k) {
       const int q = (int)(k % ns); cudaStream_t st = f3_stream(c, s, q);
