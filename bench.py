@@ -212,10 +212,19 @@ def run_gpu(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
+    if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
+        os.environ["NCCL_DEBUG"] = "WARN"              # keep NCCL's version banner off stdout: rank 0 prints ONE JSON line
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    elif args.shard:                                   # a 1-rank group, so that the collective path can be run on one GPU
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29655", rank=0, world_size=1,
+                                device_id=torch.device("cuda", local))
     ws.build()
     w, desc = make_workload(args.config, args.n_wf)
+    w_full, n_lo = w, 0
+    if args.shard:                                     # shard the spinor index, all-reduce the densities
+        n_lo, n_hi = wl.shard_range(w_full.n_wf, rank, world)
+        w = wl.shard(w_full, n_lo, n_hi)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -227,9 +236,11 @@ def run_gpu(args):
 
     # ---- resident state: every rank holds its own replica of the workload ("replicas only")
     g = make_gpu(w)
+    if args.shard:
+        g.set_density_allreduce()
     shape = (w.n_wf, 2) + w.shape
     phi = torch.empty(shape, dtype=torch.complex128, device="cuda")
-    wl.spinors_device(w, 0, w.n_wf, phi)
+    wl.spinors_device(w_full, n_lo, n_lo + w.n_wf, phi)
     hist = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(g.m)]
     torch.cuda.synchronize()
     hist = g.abm_init(phi, hist, w.dt, 0)            # zero-history start: the timed steps are plain Alg. 2 steps
@@ -256,7 +267,7 @@ def run_gpu(args):
     clocks = sampler.stop() if sampler else None
     ms = max_over_ranks(ms, world, "cuda")
     finite = bool(torch.isfinite(torch.view_as_real(phi[:: max(1, w.n_wf // 64)])).all())
-    value = job_value(w.n_wf, args.steps, world, ms)
+    value = w_full.n_wf * args.steps / (ms * 1e-3) if args.shard else job_value(w.n_wf, args.steps, world, ms)
 
     # ---- per-kernel device times (separate pass, event pairs around every launch) -> dominant kernel
     prof_steps = min(args.steps, 2)
@@ -301,7 +312,7 @@ def run_gpu(args):
 
     # ---- end to end: the same step through wslda_abm_step_host (pinned HOST buffers, copies inside the timed region)
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.shard:
         n_e = min(w.n_wf, max(1, int(2 ** 31 // (32 * w.M))))          # <= 2 GiB per buffer on the host
         we = restrict(w, n_e)
         del g
@@ -341,17 +352,18 @@ def run_gpu(args):
 
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-               "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
                "dtype": "c128", "data": "synthetic",
                "config": {"workload": desc, "name": w.name, "n_wf_per_gpu": w.n_wf, "M": w.M, "mode": w.mode,
                           "kin_form": w.kin_form, "func_id": w.func_id, "ab_am": [w.ab_order, w.am_order], "dt": w.dt,
-                          "resident_bytes": (1 + w.history) * w.n_wf * 32 * w.M, "parallelism": f"replicas x{world}",
+                          "resident_bytes": (1 + w.history) * w.n_wf * 32 * w.M, "parallelism": (f"spinor index sharded x{world}, one NCCL all-reduce of the density block per density build"
+                                          if args.shard else f"replicas x{world}"),
                           "l2": "inputs larger than L2 (no flush)" if (1 + w.history) * w.n_wf * 32 * w.M > 4e8
                                 else "working set near L2 size: numbers are L2-assisted"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof,
                "kernels": kernels, "cpu_baseline": cpu, "finite": finite}
         print(json.dumps(out))
-    if world > 1:
+    if world > 1 or args.shard:
         dist.destroy_process_group()
 
 
@@ -364,6 +376,8 @@ def main():
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--n-wf", type=int, default=None)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

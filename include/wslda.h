@@ -126,6 +126,19 @@ wslda_status wslda_abm_step(wslda_ctx*, void* phi_dev, void** f_hist, double dt,
  * stream.  phi_host / f_hist_host[i]: host (pinned for full speed); f_hist_host is permuted like f_hist_dev. */
 wslda_status wslda_abm_step_host(wslda_ctx*, void* phi_host, void** f_hist_host, void* phi_dev, void** f_hist_dev,
                                  double dt, void* cuda_stream);
+/* Sharding over the spinor index n (the paper's multi-GPU mode): every rank owns
+ * a context over its own contiguous range of spinors (with their weights and transverse modes) and the same
+ * lattice, functional and external fields.  All step kernels are local; the one exchange is the sum of the
+ * density block over the ranks, needed each time a density build is complete and before any potential is formed
+ * from it (twice per ABM step, once per Taylor start-up stage, and in wslda_update_potentials / wslda_get_field
+ * of a density after wslda_densities).  The hook is called on the HOST, from inside those calls, while their
+ * work is being enqueued: it must enqueue, on `cuda_stream`, an IN-PLACE sum over the ranks of `count` doubles at
+ * the DEVICE pointer `block` (ncclAllReduce, torch.distributed.all_reduce, ...) and return; it must not
+ * synchronise against later work of the same call.  Every rank must make the same sequence of library calls.
+ * hook = NULL removes it (single-GPU behaviour).  With a hook installed, wslda_densities(accumulate = 1) onto a
+ * block that has already been reduced is WSLDA_EINVAL.  The fixed-potential functional never calls the hook. */
+typedef void (*wslda_reduce_hook)(void* user, double* block, int64_t count, void* cuda_stream);
+wslda_status wslda_set_reduce_hook(wslda_ctx*, wslda_reduce_hook hook, void* user);
 /* Per-kernel device timing for the bench's roofline accounting: while enabled (enable = 1 also clears the
  * record) every kernel launch is bracketed by a CUDA event pair on its own stream (at most 20000 launches are
  * recorded).  wslda_profile_report synchronises the device and writes one line

@@ -44,7 +44,8 @@ SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "ws
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
-           "wslda_profile_report"]
+           "wslda_profile_report", "wslda_set_reduce_hook"]
+REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 _lib = None
 
@@ -76,6 +77,7 @@ def lib():
         L.wslda_abm_step.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
         L.wslda_abm_step_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p,
                                           C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
+        L.wslda_set_reduce_hook.argtypes = [C.c_void_p, REDUCE_HOOK, C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
         L.wslda_profile_report.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.wslda_launch_count.restype = C.c_int64
@@ -248,6 +250,39 @@ class Context:
                                             self._stream()), "abm_step_host")
         byh = {x.data_ptr(): x for x in f_hist_host}
         return [byh[p] for p in hp], self._reorder(f_hist, list(dp))
+
+    # -- sharding over the spinor index (include/wslda.h: wslda_set_reduce_hook)
+    def set_reduce_hook(self, fn):
+        """fn(block, stream_ptr): sum the float64 CUDA tensor `block` (a view of this context's density block) in
+        place over the ranks, enqueued on the CUDA stream `stream_ptr`.  None removes the hook."""
+        if fn is None:
+            self._hook = None
+            self._chk(lib().wslda_set_reduce_hook(self.ctx, C.cast(None, REDUCE_HOOK), None), "set_reduce_hook")
+            return
+        t, base = self.torch, self.workspace.data_ptr()
+
+        def _cb(_user, block, count, stream):
+            off = int(block) - base
+            fn(self.workspace[off:off + 8 * int(count)].view(t.float64), int(stream or 0))
+
+        self._hook = REDUCE_HOOK(_cb)                       # keep the trampoline alive as long as the context
+        self._chk(lib().wslda_set_reduce_hook(self.ctx, self._hook, None), "set_reduce_hook")
+
+    def set_density_allreduce(self, group=None):
+        """Shard the spinors over the ranks of a torch.distributed group (NCCL over NVLink/NVSwitch): every density
+        build is summed over the ranks with one all-reduce on the stream the step runs on."""
+        import torch.distributed as dist
+        t = self.torch
+
+        def _allreduce(block, stream):
+            cur = t.cuda.current_stream()
+            if stream and stream != cur.cuda_stream:
+                with t.cuda.stream(t.cuda.ExternalStream(stream)):
+                    dist.all_reduce(block, op=dist.ReduceOp.SUM, group=group)
+            else:
+                dist.all_reduce(block, op=dist.ReduceOp.SUM, group=group)
+
+        self.set_reduce_hook(_allreduce)
 
     def profile(self, enable=True):
         self._chk(lib().wslda_profile(self.ctx, int(bool(enable))), "profile")

@@ -150,6 +150,9 @@ struct wslda_ctx {
   int m;
   double mu_a, mu_b;
   int lambda_valid;
+  wslda_reduce_hook reduce_hook;   // multi-GPU: in-place sum over ranks of the density block (nullable)
+  void* reduce_user;
+  int raw_local;                   // the density block holds this rank's partial sums (not yet reduced)
   double *kperp2, *cpref, *w_a, *w_b, *scale, *eps, *scale2;
   double* k2n[3];                  // k_d^2 in natural index order
   double hk2[3][64];               // host copy (kernel parameters)

@@ -238,7 +238,7 @@ static void f3_stage3(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int
   LAUNCH(c, k_f3_fin3, dim3(nb(2 * P.M, 256), (unsigned)cnt), 256, 0, st, c->f_X[q], s.phi + off, c->eps + n0, s.cpart + off, 2 * P.M);
 }
 
-static void potentials(wslda_ctx* c, cudaStream_t st);
+static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh = true);
 static unsigned step_mask(const wslda_ctx* c);
 
 static void f3_dens_final(wslda_ctx* c, int used, cudaStream_t st) {

@@ -100,6 +100,14 @@ extern "C" wslda_status wslda_set_potentials(wslda_ctx* c, const double* aa, con
   return cuda_check(c, "set_potentials");
 }
 
+static void reduce_densities(wslda_ctx* c, cudaStream_t st);
+
+extern "C" wslda_status wslda_set_reduce_hook(wslda_ctx* c, wslda_reduce_hook hook, void* user) {
+  if (!c) return WSLDA_EINVAL;
+  c->reduce_hook = hook; c->reduce_user = user;
+  return WSLDA_OK;
+}
+
 extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* stream) {
   if (!c || !dst) return fail(c, WSLDA_EINVAL, "get_field: null argument");
   const int64_t M = c->P.M;
@@ -116,6 +124,7 @@ extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* s
   }
   if (src) { cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st); return cuda_check(c, "get_field"); }
   if (id < 0 || id > WSLDA_F_JB_Z) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
+  if (c->reduce_hook && c->raw_local) reduce_densities(c, st);
   LAUNCH(c, k_get_density, nb(M, 256), 256, 0, st, c->raw, M, c->f.spin_symmetric, id, (double*)dst);
   return cuda_check(c, "get_field");
 }
@@ -132,10 +141,12 @@ extern "C" wslda_status wslda_set_field(wslda_ctx* c, int id, const void* src, v
     case WSLDA_F_NU:   // interleaved complex -> two planes
       cudaMemcpy2DAsync(c->raw + DP_NU_RE * M, 8, src, 16, 8, M, cudaMemcpyDeviceToDevice, st);
       cudaMemcpy2DAsync(c->raw + DP_NU_IM * M, 8, (const char*)src + 8, 16, 8, M, cudaMemcpyDeviceToDevice, st);
+      c->raw_local = 0;
       return cuda_check(c, "set_field");
     default: return fail(c, WSLDA_EINVAL, "set_field: only raw rho/tau/nu and lambda_c can be set");
   }
   cudaMemcpyAsync(dst, src, M * 8, cudaMemcpyDeviceToDevice, st);
+  if (id != WSLDA_F_LAMBDA_C) c->raw_local = 0;            // the caller supplies whole-system densities
   return cuda_check(c, "set_field");
 }
 
@@ -232,6 +243,8 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
   if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
   if (n_first < 0 || n_count < 0 || n_first + n_count > c->P.n_wf) return fail(c, WSLDA_EINVAL, "densities: spinor range out of bounds");
   if (!mask || (mask & ~WSLDA_D_ALL)) return fail(c, WSLDA_EINVAL, "densities: bad which_mask");
+  if (c->reduce_hook && accumulate && !c->raw_local) return fail(c, WSLDA_EINVAL, "densities: accumulate onto a block already summed over the ranks");
+  c->raw_local = 1;
   cudaStream_t st = S(stream);
   if (n_count == 0 && !accumulate) {
     LAUNCH(c, k_density_reduce, dim3(nb(c->P.M, 256), DP_COUNT), 256, 0, st, c->dpart, 0, c->raw, c->P.M, mask, 0);
@@ -243,8 +256,17 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
   return cuda_check(c, "densities");
 }
 
-static void potentials(wslda_ctx* c, cudaStream_t st) {
+// Sharded runs (wslda_set_reduce_hook): the density block holds this rank's partial sums until the hook has summed it
+// over the ranks; every potential is formed from the reduced block.
+static void reduce_densities(wslda_ctx* c, cudaStream_t st) {
+  if (c->reduce_hook) c->reduce_hook(c->reduce_user, c->raw, (int64_t)DP_COUNT * c->P.M, (void*)st);
+  c->raw_local = 0;
+}
+
+// fresh: the block was just rebuilt from this rank's spinors (every call inside a step)
+static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
   if (c->f.func_id == WSLDA_FUNC_FIXED) return;
+  if (fresh || c->raw_local) reduce_densities(c, st);
   const int64_t M = c->P.M;
   FuncParams fp;
   fp.func_id = c->f.func_id; fp.force_a1 = c->f.force_a1; fp.spin_symmetric = c->f.spin_symmetric;
@@ -259,6 +281,6 @@ static void potentials(wslda_ctx* c, cudaStream_t st) {
 
 extern "C" wslda_status wslda_update_potentials(wslda_ctx* c, void* stream) {
   if (!c) return WSLDA_EINVAL;
-  potentials(c, S(stream));
+  potentials(c, S(stream), false);
   return cuda_check(c, "update_potentials");
 }

@@ -459,3 +459,111 @@ def test_cfg3_full_size_sampled_against_oracle():
 def test_cfg5_full_size_sampled_against_oracle():
     """configs[4]: 64^3, 2048 resident spinors, fixed smooth h_a != h_b fields (64^3 persistent kernels)."""
     _full_size_sampled(wl.cfg5(n_wf=2048), 10, 2, 5353)
+
+
+# ---- NEXT-2: the spinor index sharded over ranks, one density sum per build (include/wslda.h: wslda_set_reduce_hook) --
+def _run_sharded(w, psi0, n_steps, n_shards, selfstart=1):
+    """n_shards contexts on this GPU, each over its own share of the spinors and stepped by its own host thread;
+    the reduce hook is a host rendezvous that sums the density blocks of all shards (what ncclAllReduce does across
+    GPUs).  Nothing on the device waits on another launch.  Returns (phi, f_hist[0]) gathered in spinor order."""
+    import threading
+    import torch
+    bounds = [wl.shard_range(w.n_wf, r, n_shards) for r in range(n_shards)]
+    blocks, tmp, out, errs = [None] * n_shards, [None] * n_shards, [None] * n_shards, []
+    bar = threading.Barrier(n_shards)
+    calls = [0] * n_shards
+
+    def worker(r):
+        try:
+            n0, n1 = bounds[r]
+            g = make_gpu(wl.shard(w, n0, n1))
+
+            def hook(block, stream):
+                calls[r] += 1
+                torch.cuda.synchronize()
+                blocks[r] = block
+                bar.wait(timeout=120)
+                tmp[r] = torch.stack([blocks[q] for q in range(n_shards)]).sum(0)      # same order on every shard
+                torch.cuda.synchronize()
+                bar.wait(timeout=120)
+                block.copy_(tmp[r])
+                torch.cuda.synchronize()
+
+            g.set_reduce_hook(hook)
+            phi = to_gpu(psi0[n0:n1])
+            hist = [torch.zeros_like(phi) for _ in range(g.m)]
+            hist = g.abm_init(phi, hist, w.dt, selfstart)
+            for _ in range(n_steps):
+                hist = g.abm_step(phi, hist, w.dt)
+            out[r] = (to_np(phi), to_np(hist[0]), {f: to_np(g.get_field(f)) for f in ("rho_a", "nu", "delta", "U_a")})
+        except BaseException as e:                     # release the other threads, then report
+            errs.append(e)
+            bar.abort()
+
+    th = [threading.Thread(target=worker, args=(r,)) for r in range(n_shards)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    if errs:
+        raise errs[0]
+    assert len(set(calls)) == 1 and calls[0] > 0          # every shard made the same number of reductions
+    return (np.concatenate([o[0] for o in out]), np.concatenate([o[1] for o in out]), [o[2] for o in out])
+
+
+@pytest.mark.parametrize("case", ["mega32_sym40", "onchip_cfg3", "general_divgrad"])
+def test_sharded_contexts_match_unsharded_oracle(case, small_fast_chunks):
+    if case == "mega32_sym40":
+        w = wl.cfg4(n_side=32, n_wf=11, kin_form=1, n_steps=2)
+    elif case == "onchip_cfg3":
+        w = wl.cfg3(n_side=16, n_kz=3, nz=8, n_steps=2)           # three k_z modes: the split cuts through a mode
+    else:
+        w = wl.cfg4(n_side=8, n_wf=9, kin_form=2, n_steps=2)
+    psi0 = w.spinors()
+    o = make_oracle(w)
+    phi_o = psi0.copy()
+    hist_o = [np.zeros_like(psi0) for _ in range(o.m)]
+    hist_o = o.abm_init(phi_o, hist_o, w.dt, 1)
+    for _ in range(w.n_steps):
+        hist_o = o.abm_step(phi_o, hist_o, w.dt)
+    for n_shards in (2, 3):
+        phi, f0, fields = _run_sharded(w, psi0, w.n_steps, n_shards)
+        assert relerr(phi, phi_o) < TOL_ABM and relerr(f0, hist_o[0]) < TOL_ABM
+        for fl in fields:                                          # every shard ends with the whole-system fields
+            for f in ("rho_a", "nu", "delta", "U_a"):
+                assert relerr(fl[f], o.get_field(f)) < 1e-8, f
+
+
+def test_density_allreduce_through_nccl_single_rank():
+    """The torch.distributed plumbing of Context.set_density_allreduce on a 1-rank NCCL group: the hook runs inside
+    the step, on the step's stream, and a sum over one rank changes nothing."""
+    import torch
+    import torch.distributed as dist
+    if not dist.is_available() or not dist.is_nccl_available():
+        pytest.skip("no NCCL in this torch build")
+    created = False
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29613", rank=0, world_size=1)
+        created = True
+    try:
+        w = wl.cfg4(n_side=32, n_wf=6, kin_form=1, n_steps=2)
+        psi0 = w.spinors()
+        res = []
+        for hooked in (False, True):
+            g = make_gpu(w)
+            if hooked:
+                g.set_density_allreduce()
+            phi = to_gpu(psi0)
+            hist = [torch.zeros_like(phi) for _ in range(g.m)]
+            s = torch.cuda.Stream()
+            s.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(s):                          # a non-default stream: the collective must follow it
+                hist = g.abm_init(phi, hist, w.dt, 1)
+                for _ in range(w.n_steps):
+                    hist = g.abm_step(phi, hist, w.dt)
+            s.synchronize()
+            res.append((to_np(phi), to_np(g.get_field("delta"))))
+        assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+    finally:
+        if created:
+            dist.destroy_process_group()

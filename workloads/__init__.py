@@ -94,6 +94,7 @@ class Workload:
     vext_b: np.ndarray = None
     delta_ext: np.ndarray = None
     fixed: dict = field(default_factory=dict)   # alpha_a, alpha_b, U_a, U_b, delta for func_id == 0
+    n_base: int = 0               # global index of spinor 0 (non-zero for one rank's shard, see shard())
 
     @property
     def shape(self):
@@ -137,7 +138,7 @@ class Workload:
             out[i, 1] = v * pw
         if self.noise > 0:
             cnt = (n1 - n0) * 4 * self.M
-            z = normal(self.noise_seed, n0 * 4 * self.M, cnt).reshape((n1 - n0, 2) + shape + (2,))
+            z = normal(self.noise_seed, (self.n_base + n0) * 4 * self.M, cnt).reshape((n1 - n0, 2) + shape + (2,))
             out += self.noise * (z[..., 0] + 1j * z[..., 1]) / np.sqrt(vol)
             nrm = np.sqrt(np.sum(np.abs(out) ** 2, axis=tuple(range(1, nd + 2)), keepdims=True) * self.dV)
             out /= nrm
@@ -181,6 +182,29 @@ def spinors_device(w: "Workload", n0: int, n1: int, out):
             nrm = torch.sqrt(torch.sum(o.real ** 2 + o.imag ** 2, dim=tuple(range(1, nd + 2)), keepdim=True) * w.dV)
             o /= nrm
     return out
+
+
+def shard_range(n_wf: int, rank: int, world: int):
+    """Contiguous near-equal share [n0, n1) of the spinor index for `rank` of `world` (nwf/np each)."""
+    return n_wf * rank // world, n_wf * (rank + 1) // world
+
+
+def shard(w: "Workload", n0: int, n1: int) -> "Workload":
+    """The workload restricted to spinors n0..n1-1 -- one rank's share when the spinor index is sharded over GPUs:
+    weights and plane-wave table sliced, transverse-mode table shifted and clipped (modes outside the range become
+    empty), lattice, functional and external fields unchanged.  v.spinors() returns the same spinors as
+    w.spinors(n0, n1)."""
+    import copy
+    v = copy.copy(w)
+    v.n_wf = n1 - n0
+    v.n_base = w.n_base + n0
+    for k in ("kidx", "branch", "mode_of", "w_a", "w_b", "E"):
+        a = getattr(w, k)
+        if a is not None:
+            setattr(v, k, a[n0:n1])
+    if w.first is not None:
+        v.first = np.clip(np.asarray(w.first) - n0, 0, n1 - n0)
+    return v
 
 
 def _coords_centered(shape, dx):
