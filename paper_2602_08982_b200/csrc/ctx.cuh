@@ -9,6 +9,7 @@
 #include "fft_large.cuh"
 #include "fast3d.cuh"
 #include "mega3d.cuh"
+#include "mega3s.cuh"
 #include "cluster3d.cuh"
 #include "mega64.cuh"
 #include "mega64s.cuh"
@@ -33,7 +34,7 @@ struct Plan {
   // 64^3 persistent kernels (mega64.cuh)
   int f6;
   size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes, f6_partn_bytes;
-  int mega, gs, mG;
+  int mega, gs, mG, sep;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
@@ -104,8 +105,12 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
-  P.mega = P.fast; P.gs = 5;
+  P.mega = P.fast;
   if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
+  // 32^3 with the Eq. 40 operator: the axis-by-axis stage kernel (mega3s.cuh), whose only ring is Q: large groups
+  P.sep = P.mega && P.N[0] == 32 && f->kin_form == WSLDA_KIN_SYM40;
+  if (const char* e = getenv("WSLDA_SEP")) if (atoi(e) == 0) P.sep = 0;
+  P.gs = P.sep ? 32 : 5;
   if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
   if (P.gs > n_wf) P.gs = (int)n_wf;
   P.mG = (int)((n_wf + P.gs - 1) / P.gs);
@@ -170,6 +175,7 @@ struct wslda_ctx {
   int mega_grid;
   int f6_version;                  // 64^3 tiling: 1 = two planes per 256-thread CTA, 2 = one plane per 128-thread CTA
   int c3, c3_grid;                 // 32^3: H psi inside one thread-block cluster (cluster3d.cuh); grid = clusters x 8
+  int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
   int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
   double* raw;
@@ -355,6 +361,10 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, K, 128, 4 * F3_TILE_BYTES); if (occ > 0 && occ < best) best = occ; } while (0)
     WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
     WS_MEGA_ATTR((k_f3_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<false, F3_RHS>));
+    c->sep3 = P.sep;
+    if (c->sep3) {
+      WS_MEGA_ATTR((k_f3s_mega<F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<F3_RHS>));
+    }
 #undef WS_MEGA_ATTR
     c->pair32 = 0;                   // measured slower than one thread per line (127k vs 141k spinor-steps/s): opt-in
     if (const char* e = getenv("WSLDA_PAIR")) c->pair32 = atoi(e) != 0 && P.N[0] == 32;
