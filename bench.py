@@ -276,9 +276,11 @@ def run_gpu(args):
         hist = g.abm_step(phi, hist, w.dt)
     rep = g.profile_report()
     g.profile(False)
-    tot_ms = sum(v[1] for v in rep.values()) or 1.0
-    kern = sorted(rep.items(), key=lambda kv: -kv[1][1])
-    top, (top_cnt, top_ms, top_bytes, top_flops) = kern[0]
+    # launches on the three stage-1 streams overlap: rank and share by the attributed time (it adds up to the busy
+    # time), keep the raw event-pair duration for the kernel's own achieved rate
+    tot_ms = sum(v[4] for v in rep.values()) or 1.0
+    kern = sorted(rep.items(), key=lambda kv: -kv[1][4])
+    top, (top_cnt, top_ms, top_bytes, top_flops, top_share) = kern[0]
     t_b, t_f = top_bytes / (hbm_peak * 1e9), top_flops / fp64_peak
     if t_b >= t_f:
         ach = top_bytes / (top_ms * 1e-3) / 1e9
@@ -296,7 +298,7 @@ def run_gpu(args):
             roof["traffic_source"] = tr["source"] + ", per-spinor DRAM bytes x n_wf"
     except (OSError, ValueError, KeyError):
         pass
-    roof.update({"share_of_step": top_ms / tot_ms, "launches_per_step": top_cnt / prof_steps,
+    roof.update({"share_of_step": top_share / tot_ms, "launches_per_step": top_cnt / prof_steps,
                  "avg_launch_ms": top_ms / top_cnt, "alg_bytes_per_launch": top_bytes / top_cnt,
                  "alg_flops_per_launch": top_flops / top_cnt})
     B, F = alg_bytes_per_spinor_step(w), alg_flops_per_spinor_step(w)
@@ -306,7 +308,7 @@ def run_gpu(args):
                  "frac": t_roof * value / world, "bytes_per_spinor_step": B, "flops_per_spinor_step": F,
                  "hbm_gbs_achieved": B * value / world / 1e9, "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak / 1e12}
     kernels = {k: {"launches_per_step": v[0] / prof_steps, "ms_per_step": round(v[1] / prof_steps, 4),
-                   "share": round(v[1] / tot_ms, 4)} for k, v in kern}
+                   "attributed_ms_per_step": round(v[4] / prof_steps, 4), "share": round(v[4] / tot_ms, 4)} for k, v in kern}
     del hist, phi
     torch.cuda.empty_cache()
 

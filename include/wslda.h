@@ -142,9 +142,11 @@ wslda_status wslda_set_reduce_hook(wslda_ctx*, wslda_reduce_hook hook, void* use
 /* Per-kernel device timing for the bench's roofline accounting: while enabled (enable = 1 also clears the
  * record) every kernel launch is bracketed by a CUDA event pair on its own stream (at most 20000 launches are
  * recorded).  wslda_profile_report synchronises the device and writes one line
- *   "kernel_name launches total_ms algorithmic_bytes algorithmic_flops"
- * per kernel into buf (host, buf_bytes long); the last two are the sums of the compulsory HBM bytes and the
- * 5 N log2 N FFT flops the library attributes to those launches.  Returns the number
+ *   "kernel_name launches total_ms algorithmic_bytes algorithmic_flops attributed_ms"
+ * per kernel into buf (host, buf_bytes long); bytes and flops are the sums of the compulsory HBM bytes and the
+ * 5 N log2 N FFT flops the library attributes to those launches; attributed_ms splits every
+ * moment of the timeline equally among the launches active in it (launches on concurrent streams overlap, so
+ * their raw durations add up to more than the elapsed time).  Returns the number
  * of kernels, -1 on bad arguments. */
 wslda_status wslda_profile(wslda_ctx*, int enable);
 int wslda_profile_report(wslda_ctx*, char* buf, size_t buf_bytes);

@@ -288,13 +288,14 @@ class Context:
         self._chk(lib().wslda_profile(self.ctx, int(bool(enable))), "profile")
 
     def profile_report(self):
-        """{kernel name: (launches, total_ms, algorithmic bytes, algorithmic flops)} recorded since profile(True); synchronises the device."""
+        """{kernel name: (launches, total_ms, algorithmic bytes, algorithmic flops, attributed_ms)} recorded since
+        profile(True); synchronises the device.  attributed_ms shares overlapped time among concurrent launches."""
         buf = C.create_string_buffer(1 << 16)
         lib().wslda_profile_report(self.ctx, buf, len(buf))
         out = {}
         for line in buf.value.decode().splitlines():
-            name, cnt, ms, nbytes, flops = line.split()
-            out[name] = (int(cnt), float(ms), float(nbytes), float(flops))
+            name, cnt, ms, nbytes, flops, share = line.split()
+            out[name] = (int(cnt), float(ms), float(nbytes), float(flops), float(share))
         return out
 
     def launch_count(self):

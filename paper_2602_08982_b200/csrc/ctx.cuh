@@ -5,6 +5,8 @@
 #include <stdlib.h>
 #include <string.h>
 #include <vector>
+#include <algorithm>
+#include <utility>
 #include "density.cuh"
 #include "fft_large.cuh"
 #include "fast3d.cuh"
@@ -175,6 +177,7 @@ struct wslda_ctx {
   int mega_grid;
   int f6_version;                  // 64^3 tiling: 1 = two planes per 256-thread CTA, 2 = one plane per 128-thread CTA
   int c3, c3_grid;                 // 32^3: H psi inside one thread-block cluster (cluster3d.cuh); grid = clusters x 8
+  int sep_pm, sep_em;              // mega3s.cuh: x-planes per P item, row pairs per XE item
   int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
   int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
@@ -361,7 +364,9 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, K, 128, 4 * F3_TILE_BYTES); if (occ > 0 && occ < best) best = occ; } while (0)
     WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
     WS_MEGA_ATTR((k_f3_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<false, F3_RHS>));
-    c->sep3 = P.sep;
+    c->sep3 = P.sep; c->sep_pm = 4; c->sep_em = 2;     // measured: (1,1) 152k, (2,1) 155k, (4,2) 158k spinor-steps/s at 32 per group
+    if (const char* e = getenv("WSLDA_SEP_PM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4 || v == 8) c->sep_pm = v; }
+    if (const char* e = getenv("WSLDA_SEP_EM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4) c->sep_em = v; }
     if (c->sep3) {
       WS_MEGA_ATTR((k_f3s_mega<F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<F3_RHS>));
     }
@@ -434,18 +439,40 @@ extern "C" wslda_status wslda_profile(wslda_ctx* c, int enable) {
 extern "C" int wslda_profile_report(wslda_ctx* c, char* buf, size_t buf_bytes) {
   if (!c || !buf || !buf_bytes) return -1;
   cudaDeviceSynchronize();
-  std::vector<const char*> names; std::vector<double> ms, by, fl; std::vector<long> cnt;
-  for (int i = 0; i < c->prof_n; ++i) {
-    float t = 0.f;
-    cudaEventElapsedTime(&t, (*c->prof_ev)[2 * i], (*c->prof_ev)[2 * i + 1]);
+  std::vector<const char*> names; std::vector<double> ms, by, fl, sh; std::vector<long> cnt;
+  // launches on concurrent streams overlap in time: besides the raw event-pair duration, attribute every moment of
+  // the timeline in equal parts to the launches active in it (the attributed times add up to the busy time)
+  const int N = c->prof_n;
+  std::vector<double> t0(N), t1(N), share(N, 0.0);
+  std::vector<std::pair<double, int>> ends;                      // (time, +(i+1) start | -(i+1) stop)
+  for (int i = 0; i < N; ++i) {
+    float a = 0.f, b = 0.f;
+    cudaEventElapsedTime(&a, (*c->prof_ev)[0], (*c->prof_ev)[2 * i]);
+    cudaEventElapsedTime(&b, (*c->prof_ev)[2 * i], (*c->prof_ev)[2 * i + 1]);
+    t0[i] = a; t1[i] = (double)a + b;
+    ends.push_back({t0[i], i + 1}); ends.push_back({t1[i], -(i + 1)});
+  }
+  std::sort(ends.begin(), ends.end(), [](const std::pair<double, int>& x, const std::pair<double, int>& y) {
+    return x.first < y.first || (x.first == y.first && x.second < y.second); });
+  std::vector<int> active;
+  for (size_t e = 0; e < ends.size(); ++e) {
+    if (e && !active.empty()) {
+      const double dt = (ends[e].first - ends[e - 1].first) / (double)active.size();
+      for (int i : active) share[i] += dt;
+    }
+    const int id = ends[e].second;
+    if (id > 0) active.push_back(id - 1);
+    else for (size_t q = 0; q < active.size(); ++q) if (active[q] == -id - 1) { active[q] = active.back(); active.pop_back(); break; }
+  }
+  for (int i = 0; i < N; ++i) {
     size_t k = 0;
     while (k < names.size() && strcmp(names[k], (*c->prof_name)[i])) ++k;
-    if (k == names.size()) { names.push_back((*c->prof_name)[i]); ms.push_back(0.0); by.push_back(0.0); fl.push_back(0.0); cnt.push_back(0); }
-    ms[k] += t; cnt[k]++; by[k] += (*c->prof_work)[2 * i]; fl[k] += (*c->prof_work)[2 * i + 1];
+    if (k == names.size()) { names.push_back((*c->prof_name)[i]); ms.push_back(0.0); by.push_back(0.0); fl.push_back(0.0); sh.push_back(0.0); cnt.push_back(0); }
+    ms[k] += t1[i] - t0[i]; sh[k] += share[i]; cnt[k]++; by[k] += (*c->prof_work)[2 * i]; fl[k] += (*c->prof_work)[2 * i + 1];
   }
   size_t o = 0; buf[0] = 0;
   for (size_t k = 0; k < names.size(); ++k) {
-    int w = snprintf(buf + o, buf_bytes - o, "%s %ld %.6f %.6e %.6e\n", names[k], cnt[k], ms[k], by[k], fl[k]);
+    int w = snprintf(buf + o, buf_bytes - o, "%s %ld %.6f %.6e %.6e %.6f\n", names[k], cnt[k], ms[k], by[k], fl[k], sh[k]);
     if (w < 0 || (size_t)w >= buf_bytes - o) break;
     o += w;
   }

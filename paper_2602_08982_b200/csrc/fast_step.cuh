@@ -94,9 +94,9 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   else k = mode == F3_APPLY ? k_f3_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3_mega<false, F3_CORR> : k_f3_mega<false, F3_RHS>;
   if (c->sep3 && sym && !c->pair32) {                      // 32^3 Eq. 40: axis-by-axis Laplacian, two passes (mega3s.cuh)
     F3SMega A;
-    A.m = a;
+    A.m = a; A.pm = c->sep_pm; A.em = c->sep_em;
     for (int j = 0; j < 32; ++j) { A.k2zy[j] = c->hk2[2][j]; A.k2zy[32 + j] = c->hk2[1][j]; }
-    const int ITs = a.gs * 32 / F3S_PMULT + a.gs * 16 / F3S_EMULT + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
+    const int ITs = a.gs * 32 / A.pm + a.gs * 16 / A.em + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
     const long tot = (long)(a.G + 2) * ITs;
     const int gr = (int)(tot < c->mega_grid ? tot : c->mega_grid);
     void (*ks)(F3SMega) = mode == F3_APPLY ? k_f3s_mega<F3_APPLY> : mode == F3_CORR ? k_f3s_mega<F3_CORR> : k_f3s_mega<F3_RHS>;

@@ -17,15 +17,16 @@
 #pragma once
 #include "mega3d.cuh"
 
-#ifndef F3S_PMULT
-#define F3S_PMULT 4            // x-planes per P item (measured: 1 -> 152k, 2 -> 155k, 4 -> 158k spinor-steps/s)
-#endif
-#ifndef F3S_EMULT
-#define F3S_EMULT 2            // row pairs per XE item
-#endif
+// L1-allocating load with an L2 eviction policy
+__device__ __forceinline__ cplx ld_ca_pol(const cplx* p, uint64_t pol) {
+  cplx v;
+  asm volatile("ld.global.ca.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+  return v;
+}
 
 struct F3SMega {
   F3Mega m;                      // spec0 = Q ring [R][gs][2][M]; spec1 unused
+  int pm, em;                    // x-planes per P item (1, 2, 4, 8), row pairs per XE item (1, 2, 4)
   double k2zy[64];               // k_z^2 (0..31) then k_y^2 (32..63), natural order (kernel parameters: constant bank)
 };
 
@@ -64,7 +65,7 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
       for (int j = 0; j < F3_N; ++j) {
         double f = s;
         if (t) f *= al[j * F3_N + lane];
-        x[j] = cscale(src[j * F3_N + lane], f);                 // (y = j, z = lane); the second pass hits L1 / L2
+        x[j] = cscale(ld_ca_pol(src + j * F3_N + lane, pol.keep), f);   // (y = j, z = lane); the second pass hits L1 / L2; XE and D re-read it
       }
       if (pass == 0) F3_T(0, 0); else F3_T(0, 2);
       if (pass == 0) {                                          // z-lines: transpose, differentiate, transpose back
@@ -167,7 +168,7 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
         b[r].u = pu[i]; b[r].v = pv[i]; b[r].q = pk[i]; b[r].D = pk[M + i];
         if (kp2 != 0.0) { const cplx t = pk[2 * M + i]; b[r].Aa = t.x; b[r].Ab = t.y; } else { b[r].Aa = b[r].Ab = 0.0; }
         b[r].Qu = ld_pol(Qu + i, pol.drop); b[r].Qv = ld_pol(Qu + M + i, pol.drop);    // last use of Q
-        if (MODE == F3_CORR) { b[r].cu = cu[i]; b[r].cv = cu[M + i]; }
+        if (MODE == F3_CORR) { b[r].cu = ld_pol(cu + i, pol.drop); b[r].cv = ld_pol(cu + M + i, pol.drop); }   // read once
       }
     };
     auto comp = [&](const F3SRow* b, int j0) {
@@ -226,8 +227,11 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
 }
 
 // tick t: P(t), XE(t-1), D(t-2).  done[0..G) P, [G..2G) XE, [2G..3G) D.
+#ifndef F3S_OCC
+#define F3S_OCC F3_MEGA_OCC
+#endif
 template <int MODE>
-__global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3s_mega(F3SMega A) {
+__global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* tiles = reinterpret_cast<cplx*>(smem_raw);
   __shared__ int s_item[2];
@@ -237,7 +241,7 @@ __global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3s_mega(F3SMega A) {
   const F3Pol pol = f3_policies();
   const int G = a.G;
   int* done = reinterpret_cast<int*>(a.sync + 1);
-  const int nP = a.gs * F3_N / F3S_PMULT, nE = a.gs * 16 / F3S_EMULT, nD = MODE == F3_APPLY ? 0 : F3_N * F3_DSPLIT;
+  const int nP = a.gs * F3_N / A.pm, nE = a.gs * 16 / A.em, nD = MODE == F3_APPLY ? 0 : F3_N * F3_DSPLIT;
   const int IT = nP + nE + nD, total = (G + 2) * IT;
   int t1 = 0;
   if (threadIdx.x == 0) t1 = atomicAdd(&a.sync->next, 1);
@@ -257,7 +261,7 @@ __global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3s_mega(F3SMega A) {
       if (g < G) {
         if (g >= F3_RING) f3_wait(&done[G + g - F3_RING], nE, a.sync);                 // the Q slot is free
         F3_T(4, 1);
-        for (int k = 0; k < F3S_PMULT; ++k) { if (k) __syncthreads(); f3s_body_p(A, pol, g, r * F3S_PMULT + k, tiles, x); }
+        for (int k = 0; k < A.pm; ++k) { if (k) __syncthreads(); f3s_body_p(A, pol, g, r * A.pm + k, tiles, x); }
         F3_T0();
         f3_signal(&done[g], &a.sync->next, t1); drew = true;
         F3_T(4, 5);
@@ -268,7 +272,7 @@ __global__ void __launch_bounds__(128, F3_MEGA_OCC) k_f3s_mega(F3SMega A) {
         f3_wait(&done[g], nP, a.sync);
         if (MODE != F3_APPLY && g >= F3_RING) f3_wait(&done[2 * G + g - F3_RING], nD, a.sync);   // the X slot is free
         F3_T(4, 2);
-        for (int k = 0; k < F3S_EMULT; ++k) { if (k) __syncthreads(); f3s_body_xe<MODE>(A, pol, g, (r - nP) * F3S_EMULT + k, tiles, red, x); }
+        for (int k = 0; k < A.em; ++k) { if (k) __syncthreads(); f3s_body_xe<MODE>(A, pol, g, (r - nP) * A.em + k, tiles, red, x); }
         F3_T0();
         f3_signal(&done[G + g], &a.sync->next, t1); drew = true;
         F3_T(4, 5);
