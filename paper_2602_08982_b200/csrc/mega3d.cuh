@@ -25,7 +25,9 @@ __device__ unsigned long long g_f3_cycles[8][8];
 #define F3_T(kind, phase) do {} while (0)
 #endif
 #define F3_MEGA_OCC 2
+#ifndef F3_DSPLIT
 #define F3_DSPLIT 2            // D items per x-plane
+#endif
 
 struct F3Sync {                // device counters, zeroed before every launch
   int next;                    // ticket

@@ -91,18 +91,18 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
     }
   }
   F3_T(0, 4);
-  __syncthreads();
+  if (c == 0) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");   // the pair (w, alpha w)
   F3_T(0, 5);
   if (valid) {                                                  // Q_c = alpha (d_y^2 + d_z^2) w + (d_y^2 + d_z^2)(alpha w)
-    cplx* q = a.spec0 + (((size_t)(g % F3_RING) * a.gs + nl) * 2) * M + pl;
+    cplx* q = a.spec0 + (((size_t)(g % F3_RING) * a.gs + nl) * 2 + c) * M + pl;
+    const cplx* T0 = tiles + (2 * c) * TILE;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      const int j = 8 * warp + r, si = j * F3_PITCH + lane, i = j * F3_N + lane;
-      const cplx a0 = tiles[si], a1 = tiles[TILE + si], b0 = tiles[2 * TILE + si], b1 = tiles[3 * TILE + si];
-      st_pol(q + i, cadd(a0, a1), pol.keep);
-      st_pol(q + M + i, cadd(b0, b1), pol.keep);
+    for (int r = 0; r < 16; ++r) {
+      const int j = 16 * t + r, si = j * F3_PITCH + lane;
+      st_pol(q + j * F3_N + lane, cadd(T0[si], T0[TILE + si]), pol.keep);
     }
   }
+  if (c == 0) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");   // tiles free again
   F3_T(0, 6);
 }
 
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
       if (g < G) {
         if (g >= F3_RING) f3_wait(&done[G + g - F3_RING], nE, a.sync);                 // the Q slot is free
         F3_T(4, 1);
-        for (int k = 0; k < A.pm; ++k) { if (k) __syncthreads(); f3s_body_p(A, pol, g, r * A.pm + k, tiles, x); }
+        for (int k = 0; k < A.pm; ++k) { f3s_body_p(A, pol, g, r * A.pm + k, tiles, x); }
         F3_T0();
         f3_signal(&done[g], &a.sync->next, t1); drew = true;
         F3_T(4, 5);
