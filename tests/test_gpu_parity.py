@@ -234,6 +234,32 @@ def test_fast3d_multikernel_fallback(small_fast_chunks, monkeypatch):
     assert "k_f3_pass_c" in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
 
 
+@pytest.mark.parametrize("sep,pm,em", [("0", None, None), ("1", "1", "1"), ("1", "8", "4"), ("1", "2", "2")])
+def test_axis_by_axis_stage_kernel_32cubed(small_fast_chunks, monkeypatch, sep, pm, em):
+    """The default 32^3 Eq. 40 stage kernels (mega3s.cuh: Laplacian axis by axis) for several item sizes, ragged groups
+    of 3 spinors, and the three-pass kernels they replace (WSLDA_SEP=0): H psi and self-consistent steps."""
+    monkeypatch.setenv("WSLDA_SEP", sep)
+    if pm:
+        monkeypatch.setenv("WSLDA_SEP_PM", pm)
+        monkeypatch.setenv("WSLDA_SEP_EM", em)
+    w = wl.cfg4(n_side=32, n_wf=10, kin_form=1, n_steps=3)
+    psi0 = w.spinors()
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi0)
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("delta", "U_a", "rho_a", "nu"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert ("k_f3s_mega_corr" in names) == (sep == "1") and ("k_f3_mega_corr" in names) == (sep == "0")
+
+
 @pytest.mark.parametrize("kin_form", [0, 1])
 def test_pair_line_kernel_32cubed(small_fast_chunks, monkeypatch, kin_form):
     """The opt-in pair-of-threads 32^3 stage kernel (mega32p.cuh, WSLDA_PAIR=1): H psi and self-consistent steps."""
