@@ -109,8 +109,8 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   }
   P.mega = P.fast;
   if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
-  // 32^3 with the Eq. 40 operator: the axis-by-axis stage kernel (mega3s.cuh), whose only ring is Q: large groups
-  P.sep = P.mega && P.N[0] == 32 && f->kin_form == WSLDA_KIN_SYM40;
+  // 32^3: the axis-by-axis stage kernels (mega3s.cuh), whose only ring is Q: large groups
+  P.sep = P.mega && P.N[0] == 32;
   if (const char* e = getenv("WSLDA_SEP")) if (atoi(e) == 0) P.sep = 0;
   P.gs = P.sep ? 32 : 5;
   if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
@@ -368,7 +368,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     if (const char* e = getenv("WSLDA_SEP_PM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4 || v == 8) c->sep_pm = v; }
     if (const char* e = getenv("WSLDA_SEP_EM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4) c->sep_em = v; }
     if (c->sep3) {
-      WS_MEGA_ATTR((k_f3s_mega<F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<F3_RHS>));
+      WS_MEGA_ATTR((k_f3s_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<true, F3_RHS>));
+      WS_MEGA_ATTR((k_f3s_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_RHS>));
     }
 #undef WS_MEGA_ATTR
     c->pair32 = 0;                   // measured slower than one thread per line (127k vs 141k spinor-steps/s): opt-in

@@ -92,14 +92,16 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   void (*k)(F3Mega);
   if (sym) k = mode == F3_APPLY ? k_f3_mega<true, F3_APPLY> : mode == F3_CORR ? k_f3_mega<true, F3_CORR> : k_f3_mega<true, F3_RHS>;
   else k = mode == F3_APPLY ? k_f3_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3_mega<false, F3_CORR> : k_f3_mega<false, F3_RHS>;
-  if (c->sep3 && sym && !c->pair32) {                      // 32^3 Eq. 40: axis-by-axis Laplacian, two passes (mega3s.cuh)
+  if (c->sep3 && !c->pair32) {                             // 32^3: axis-by-axis Laplacian, two passes (mega3s.cuh)
     F3SMega A;
     A.m = a; A.pm = c->sep_pm; A.em = c->sep_em;
     for (int j = 0; j < 32; ++j) { A.k2zy[j] = c->hk2[2][j]; A.k2zy[32 + j] = c->hk2[1][j]; }
-    const int ITs = a.gs * 32 / A.pm + a.gs * 16 / A.em + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
+    const int ITs = a.gs * (sym ? 32 : 16) / A.pm + a.gs * 16 / A.em + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
     const long tot = (long)(a.G + 2) * ITs;
     const int gr = (int)(tot < c->mega_grid ? tot : c->mega_grid);
-    void (*ks)(F3SMega) = mode == F3_APPLY ? k_f3s_mega<F3_APPLY> : mode == F3_CORR ? k_f3s_mega<F3_CORR> : k_f3s_mega<F3_RHS>;
+    void (*ks)(F3SMega);
+    if (sym) ks = mode == F3_APPLY ? k_f3s_mega<true, F3_APPLY> : mode == F3_CORR ? k_f3s_mega<true, F3_CORR> : k_f3s_mega<true, F3_RHS>;
+    else ks = mode == F3_APPLY ? k_f3s_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3s_mega<false, F3_CORR> : k_f3s_mega<false, F3_RHS>;
     LAUNCHN(c, mode == F3_APPLY ? "k_f3s_mega_apply" : mode == F3_CORR ? "k_f3s_mega_corr" : "k_f3s_mega_rhs", ks, gr, 128,
             4 * F3_TILE_BYTES, st, A);
     return;

@@ -1,4 +1,4 @@
-// mega3s.cuh -- the 32^3 Eq. 40 stage kernel with the Laplacian taken axis by axis.
+// mega3s.cuh -- the 32^3 stage kernels (Eq. 40 and Eq. 14 operators) with the Laplacian taken axis by axis.
 //
 // The spectral Laplacian of Eq. 26 is a sum over the axes, lap = d_x^2 + d_y^2 + d_z^2, and each
 // term needs transforms along ITS axis only (forward, times -k_d^2 / N_d, inverse on every line of that axis).  So
@@ -45,13 +45,15 @@ __device__ __forceinline__ void f3s_d2(cplx* x, K2 k2) {
 }
 
 // ---- P: (d_y^2 + d_z^2) of the four fields u, alpha_a u, v, alpha_b v of one (spinor, x-plane), one per warp -----
+// Eq. 14 (SYM = false): the item is two x-planes, one (plane, component) per warp, Q_c = (d_y^2 + d_z^2) w, no pairing.
+template <bool SYM>
 __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, int g, int ip, cplx* tiles, cplx* x) {
   const F3Mega& a = A.m;
-  constexpr int TILE = F3_N * F3_PITCH;
+  constexpr int TILE = F3_N * F3_PITCH, PER = SYM ? F3_N : F3_N / 2;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int nl = ip / F3_N, ix = ip - nl * F3_N, n = g * a.gs + nl;
+  const int nl = ip / PER, rr = ip - nl * PER, ix = SYM ? rr : 2 * rr + (warp >> 1), n = g * a.gs + nl;
   const bool valid = n < a.n;
-  const int c = warp >> 1, t = warp & 1;                       // t = 0: w (times alpha afterwards), t = 1: alpha w
+  const int c = SYM ? warp >> 1 : warp & 1, t = SYM ? warp & 1 : 0;   // t = 0: w (times alpha afterwards), t = 1: alpha w
   const size_t M = (size_t)F3_N * F3_PLANE, pl = (size_t)ix * F3_PLANE;
   cplx* S = tiles + warp * TILE;
   F3_T0();
@@ -64,7 +66,7 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
 #pragma unroll
       for (int j = 0; j < F3_N; ++j) {
         double f = s;
-        if (t) f *= al[j * F3_N + lane];
+        if (SYM && t) f *= al[j * F3_N + lane];
         x[j] = cscale(ld_ca_pol(src + j * F3_N + lane, pol.keep), f);   // (y = j, z = lane); the second pass hits L1 / L2; XE and D re-read it
       }
       if (pass == 0) F3_T(0, 0); else F3_T(0, 2);
@@ -83,6 +85,13 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
         __syncwarp();
       }
     }
+    if (!SYM) {                                                 // straight to the Q ring: nothing to pair with
+      cplx* q = a.spec0 + (((size_t)(g % F3_RING) * a.gs + nl) * 2 + c) * M + pl;
+#pragma unroll
+      for (int j = 0; j < F3_N; ++j) st_pol(q + j * F3_N + lane, cadd(x[j], S[j * F3_PITCH + lane]), pol.keep);
+      __syncwarp();
+      return;
+    }
 #pragma unroll
     for (int j = 0; j < F3_N; ++j) {
       const cplx z = S[j * F3_PITCH + lane];
@@ -90,6 +99,7 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
       S[j * F3_PITCH + lane] = make_double2((x[j].x + z.x) * f, (x[j].y + z.y) * f);
     }
   }
+  if (!SYM) return;
   F3_T(0, 4);
   if (c == 0) asm volatile("bar.sync 1, 64;" ::: "memory"); else asm volatile("bar.sync 2, 64;" ::: "memory");   // the pair (w, alpha w)
   F3_T(0, 5);
@@ -111,7 +121,7 @@ struct F3SRow { cplx u, v, D, q, Qu, Qv, cu, cv; double Aa, Ab; };   // the epil
 // ---- XE: the x-lines of one (spinor, y-row) by a PAIR of warps (lane = z): warp c of the pair differentiates
 // component c (alpha d_x^2 w + d_x^2(alpha w), parked in shared memory); after a pair barrier each warp finishes half of
 // the line for BOTH components, so that psi, the fields, Q and C_part are read once per point ---------------------------
-template <int MODE>
+template <bool SYM, int MODE>
 __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, int g, int ie, cplx* park, double* red, cplx* x) {
   const F3Mega& a = A.m;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -132,7 +142,7 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
     const cplx* pc = c ? pv : pu;
     const double* al = a.F.alpha[c] + off;
 #pragma unroll 1
-    for (int t = 0; t < 2; ++t) {                               // t = 0: alpha d_x^2 w, t = 1: d_x^2 (alpha w)
+    for (int t = 0; t < (SYM ? 2 : 1); ++t) {                   // t = 0: alpha d_x^2 w (Eq. 14: d_x^2 w), t = 1: d_x^2 (alpha w)
 #pragma unroll
       for (int j = 0; j < F3_N; ++j) {
         double f = s;
@@ -144,7 +154,7 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
       F3_T(1, 1);
       if (t == 0) {
 #pragma unroll
-        for (int j = 0; j < F3_N; ++j) P[j * 128] = cscale(x[j], al[(size_t)j * F3_PLANE]);
+        for (int j = 0; j < F3_N; ++j) P[j * 128] = SYM ? cscale(x[j], al[(size_t)j * F3_PLANE]) : x[j];
       } else {
 #pragma unroll
         for (int j = 0; j < F3_N; ++j) { const cplx z = P[j * 128]; P[j * 128] = cadd(x[j], z); }
@@ -166,7 +176,7 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
       for (int r = 0; r < 2; ++r) {
         const size_t i = (size_t)(j0 + r) * F3_PLANE;
         b[r].u = pu[i]; b[r].v = pv[i]; b[r].q = pk[i]; b[r].D = pk[M + i];
-        if (kp2 != 0.0) { const cplx t = pk[2 * M + i]; b[r].Aa = t.x; b[r].Ab = t.y; } else { b[r].Aa = b[r].Ab = 0.0; }
+        if (SYM && kp2 != 0.0) { const cplx t = pk[2 * M + i]; b[r].Aa = t.x; b[r].Ab = t.y; } else { b[r].Aa = b[r].Ab = 0.0; }
         b[r].Qu = ld_pol(Qu + i, pol.drop); b[r].Qv = ld_pol(Qu + M + i, pol.drop);    // last use of Q
         if (MODE == F3_CORR) { b[r].cu = ld_pol(cu + i, pol.drop); b[r].cv = ld_pol(cu + M + i, pol.drop); }   // read once
       }
@@ -177,9 +187,10 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
         const size_t i = (size_t)(j0 + r) * F3_PLANE;
         const cplx u = cscale(b[r].u, s), v = cscale(b[r].v, s);
         const cplx Lu = cadd(Pu[(j0 + r) * 128], b[r].Qu), Lv = cadd(Pv[(j0 + r) * 128], b[r].Qv);
-        const double ha = 0.5 * kp2 * b[r].Aa, hb = 0.5 * kp2 * b[r].Ab;
-        const cplx Ku = make_double2(-0.25 * Lu.x + ha * u.x, -0.25 * Lu.y + ha * u.y);   // Eq. 40; +(lap alpha) w / 4 sits in q
-        const cplx Kv = make_double2(-0.25 * Lv.x + hb * v.x, -0.25 * Lv.y + hb * v.y);
+        const double ha = SYM ? 0.5 * kp2 * b[r].Aa : 0.5 * kp2, hb = SYM ? 0.5 * kp2 * b[r].Ab : 0.5 * kp2;
+        constexpr double kf = SYM ? -0.25 : -0.5;                                           // Eq. 40 (its +(lap alpha) w / 4 sits in q) | Eq. 14
+        const cplx Ku = make_double2(kf * Lu.x + ha * u.x, kf * Lu.y + ha * u.y);
+        const cplx Kv = make_double2(kf * Lv.x + hb * v.x, kf * Lv.y + hb * v.y);
         const cplx D = b[r].D;
         const cplx Hu = cadd(Ku, cadd(cscale(u, b[r].q.x), cmul(D, v)));                  // Eqs. 5, 15
         const cplx Hv = csub(cmul(cconj(D), u), cadd(Kv, cscale(v, b[r].q.y)));
@@ -230,7 +241,7 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
 #ifndef F3S_OCC
 #define F3S_OCC F3_MEGA_OCC
 #endif
-template <int MODE>
+template <bool SYM, int MODE>
 __global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* tiles = reinterpret_cast<cplx*>(smem_raw);
@@ -241,7 +252,7 @@ __global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
   const F3Pol pol = f3_policies();
   const int G = a.G;
   int* done = reinterpret_cast<int*>(a.sync + 1);
-  const int nP = a.gs * F3_N / A.pm, nE = a.gs * 16 / A.em, nD = MODE == F3_APPLY ? 0 : F3_N * F3_DSPLIT;
+  const int nP = a.gs * (SYM ? F3_N : F3_N / 2) / A.pm, nE = a.gs * 16 / A.em, nD = MODE == F3_APPLY ? 0 : F3_N * F3_DSPLIT;
   const int IT = nP + nE + nD, total = (G + 2) * IT;
   int t1 = 0;
   if (threadIdx.x == 0) t1 = atomicAdd(&a.sync->next, 1);
@@ -261,7 +272,7 @@ __global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
       if (g < G) {
         if (g >= F3_RING) f3_wait(&done[G + g - F3_RING], nE, a.sync);                 // the Q slot is free
         F3_T(4, 1);
-        for (int k = 0; k < A.pm; ++k) { f3s_body_p(A, pol, g, r * A.pm + k, tiles, x); }
+        for (int k = 0; k < A.pm; ++k) { f3s_body_p<SYM>(A, pol, g, r * A.pm + k, tiles, x); }
         F3_T0();
         f3_signal(&done[g], &a.sync->next, t1); drew = true;
         F3_T(4, 5);
@@ -272,7 +283,7 @@ __global__ void __launch_bounds__(128, F3S_OCC) k_f3s_mega(F3SMega A) {
         f3_wait(&done[g], nP, a.sync);
         if (MODE != F3_APPLY && g >= F3_RING) f3_wait(&done[2 * G + g - F3_RING], nD, a.sync);   // the X slot is free
         F3_T(4, 2);
-        for (int k = 0; k < A.em; ++k) { if (k) __syncthreads(); f3s_body_xe<MODE>(A, pol, g, (r - nP) * A.em + k, tiles, red, x); }
+        for (int k = 0; k < A.em; ++k) { if (k) __syncthreads(); f3s_body_xe<SYM, MODE>(A, pol, g, (r - nP) * A.em + k, tiles, red, x); }
         F3_T0();
         f3_signal(&done[G + g], &a.sync->next, t1); drew = true;
         F3_T(4, 5);
