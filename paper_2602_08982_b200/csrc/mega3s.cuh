@@ -30,18 +30,25 @@ struct F3SMega {
   double k2zy[64];               // k_z^2 (0..31) then k_y^2 (32..63), natural order (kernel parameters: constant bank)
 };
 
-// second derivative along the register index: x <- IFFT( -k2[j] / 32 * FFT(x) ); the inverse is conj(FFT(conj .))
+// second derivative along the register index: x <- s * IFFT( -k2[j] / 32 * FFT(x) ); the inverse is conj(FFT(conj .)).
+// The spinor's scale s rides on the k-space factor and the closing conjugation is a sign-bit flip (no FP64 issue slot).
+__device__ __forceinline__ double f3s_flip(double v) { return __hiloint2double(__double2hiint(v) ^ (int)0x80000000u, __double2loint(v)); }
 template <class K2>
-__device__ __forceinline__ void f3s_d2(cplx* x, K2 k2) {
+__device__ __forceinline__ void f3s_d2(cplx* x, K2 k2, double s) {
+  const double sm = -0.03125 * s;
 #pragma unroll 1
   for (int dir = 0; dir < 2; ++dir) {
     fft_reg<F3_N, false>(x);
+    if (dir == 0) {
 #pragma unroll
-    for (int j = 0; j < F3_N; ++j) {
-      const double f = dir ? 1.0 : -k2(j) * 0.03125;
-      x[j] = make_double2(x[j].x * f, -x[j].y * f);
+      for (int j = 0; j < F3_N; ++j) {
+        const double f = k2(j) * sm;
+        x[j] = make_double2(x[j].x * f, -x[j].y * f);
+      }
     }
   }
+#pragma unroll
+  for (int j = 0; j < F3_N; ++j) x[j].y = f3s_flip(x[j].y);
 }
 
 // ---- P: (d_y^2 + d_z^2) of the four fields u, alpha_a u, v, alpha_b v of one (spinor, x-plane), one per warp -----
@@ -63,11 +70,12 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
     const double s = a.scale ? a.scale[n] : 1.0;
 #pragma unroll 1
     for (int pass = 0; pass < 2; ++pass) {
+      if (SYM && t) {
 #pragma unroll
-      for (int j = 0; j < F3_N; ++j) {
-        double f = s;
-        if (SYM && t) f *= al[j * F3_N + lane];
-        x[j] = cscale(ld_ca_pol(src + j * F3_N + lane, pol.keep), f);   // (y = j, z = lane); the second pass hits L1 / L2; XE and D re-read it
+        for (int j = 0; j < F3_N; ++j) x[j] = cscale(ld_ca_pol(src + j * F3_N + lane, pol.keep), al[j * F3_N + lane]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < F3_N; ++j) x[j] = ld_ca_pol(src + j * F3_N + lane, pol.keep);   // (y = j, z = lane); the second pass hits L1 / L2; XE and D re-read it
       }
       if (pass == 0) F3_T(0, 0); else F3_T(0, 2);
       if (pass == 0) {                                          // z-lines: transpose, differentiate, transpose back
@@ -77,7 +85,7 @@ __device__ __forceinline__ void f3s_body_p(const F3SMega& A, const F3Pol& pol, i
 #pragma unroll
         for (int j = 0; j < F3_N; ++j) x[j] = S[lane * F3_PITCH + j];
       }
-      f3s_d2(x, [&](int j) { return A.k2zy[pass * 32 + j]; });
+      f3s_d2(x, [&](int j) { return A.k2zy[pass * 32 + j]; }, s);
       if (pass == 0) F3_T(0, 1); else F3_T(0, 3);
       if (pass == 0) {
 #pragma unroll
@@ -143,14 +151,15 @@ __device__ __forceinline__ void f3s_body_xe(const F3SMega& A, const F3Pol& pol, 
     const double* al = a.F.alpha[c] + off;
 #pragma unroll 1
     for (int t = 0; t < (SYM ? 2 : 1); ++t) {                   // t = 0: alpha d_x^2 w (Eq. 14: d_x^2 w), t = 1: d_x^2 (alpha w)
+      if (t) {
 #pragma unroll
-      for (int j = 0; j < F3_N; ++j) {
-        double f = s;
-        if (t) f *= al[(size_t)j * F3_PLANE];
-        x[j] = cscale(pc[(size_t)j * F3_PLANE], f);
+        for (int j = 0; j < F3_N; ++j) x[j] = cscale(pc[(size_t)j * F3_PLANE], al[(size_t)j * F3_PLANE]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < F3_N; ++j) x[j] = pc[(size_t)j * F3_PLANE];
       }
       F3_T(1, 0);
-      f3s_d2(x, [&](int j) { return a.kx2[j]; });
+      f3s_d2(x, [&](int j) { return a.kx2[j]; }, s);
       F3_T(1, 1);
       if (t == 0) {
 #pragma unroll
