@@ -103,7 +103,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_fast = o; P.fast_spec_bytes = P.fast_part_bytes = P.fast_stream_bytes = 0;
   if (P.fast) {
     P.fast_spec_bytes = align_up((size_t)P.fc * 2 * M * 16);
-    P.fast_part_bytes = align_up((size_t)F3_NPART * P.fc * P.N[0] * 8) + align_up((size_t)P.fc * P.nblk * 8);
+    P.fast_part_bytes = align_up((size_t)F3_NPART * P.fc * P.N[0] * 8) + align_up((size_t)P.fc * P.nblk * 8) + align_up((size_t)P.fc * 4);
     P.fast_stream_bytes = 3 * P.fast_spec_bytes + P.fast_part_bytes + align_up((size_t)4 * M * 8);
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
@@ -181,6 +181,7 @@ struct wslda_ctx {
   int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
   int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
   double *f_part[4], *f_partn[4], *f_acc[4];
+  int* f_cnt[4];                   // per-spinor arrival counters of k_f3_combine (self-resetting)
   double* raw;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
   cplx *delta, *dext;
@@ -325,10 +326,13 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       c->f_spec0[q] = (cplx*)b; c->f_spec1[q] = (cplx*)(b + P.fast_spec_bytes); c->f_X[q] = (cplx*)(b + 2 * P.fast_spec_bytes);
       b += 3 * P.fast_spec_bytes;
       c->f_part[q] = (double*)b; c->f_partn[q] = (double*)(b + align_up((size_t)F3_NPART * P.fc * P.N[0] * 8));
+      c->f_cnt[q] = (int*)((char*)c->f_partn[q] + align_up((size_t)P.fc * P.nblk * 8));
+      cudaMemset(c->f_cnt[q], 0, (size_t)P.fc * 4);
       c->f_acc[q] = (double*)(b + P.fast_part_bytes);
       if (q > 0 || P.ns > 1) cudaStreamCreateWithFlags(&c->aux[q], cudaStreamNonBlocking);
       cudaEventCreateWithFlags(&c->ev_join[q], cudaEventDisableTiming);
     }
+    cudaDeviceSynchronize();                               // the counters are zero before any stream of the caller runs
     cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
     cudaFuncSetAttribute(k_f3_pass_a<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
     cudaFuncSetAttribute(k_f3_pass_a<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);

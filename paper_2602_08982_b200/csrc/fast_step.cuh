@@ -225,9 +225,7 @@ static void f3_stage1(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int
   for (int j = 0; j < 5; ++j) if (h.f[j]) h.f[j] += off;
   WORK(c, 32.0 * P.M * cnt * (1 + c->m + 2), 0);
   LAUNCH(c, k_f3_combine, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, s.phi + off, h, s.cpart + off, s.k, P.M,
-         c->f.normalize ? c->f_partn[q] : (double*)nullptr, P.nblk);
-  if (c->f.normalize)
-    LAUNCH(c, k_from_partials, nb(cnt * 32, 128), 128, 0, st, c->f_partn[q], P.nblk, (int64_t)cnt, c->dV, 1, c->scale + n0, (double*)nullptr);
+         c->f.normalize ? c->f_partn[q] : (double*)nullptr, P.nblk, c->f_cnt[q], c->dV, c->scale + n0);
 }
 // Alg. 2 steps 3-4, 8: phi_new = C_part + c0 dt f(P), normalised, written over P (+ its densities)
 static void f3_stage2(wslda_ctx* c, const F3Step& s, int q, cudaStream_t st, int64_t n0, int cnt, int do_dens, int first) {

@@ -38,9 +38,12 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_abm_combine(cplx* phi, HistPt
 // The same predictor sweep for the fused 3-D path (chunks of a few dozen MB on concurrent streams): the history and
 // phi are read for the last time in this stage (L2 evict_first), C_part is not needed before the next stage
 // (evict_first), while P is re-read by the density kernel of the same chunk and must stay in L2 (evict_last).
+// The CTA that completes a spinor's partial sums (a self-resetting arrival counter per spinor) turns them into
+// scale_n = 1 / sqrt(dV sum |P|^2) in the fixed order of k_from_partials: no separate launch per chunk.
 __global__ void __launch_bounds__(WS_PT_THREADS) k_f3_combine(cplx* phi, HistPtrs h, cplx* cpart, AbmCoef k, int64_t M,
-                                                              double* part, int nblk) {
+                                                              double* part, int nblk, int* arrived, double dV, double* scale) {
   __shared__ double sh[32];
+  __shared__ int s_last;
   const F3Pol pol = f3_policies();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, n = blockIdx.y;
   double acc = 0.0;
@@ -67,7 +70,20 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_f3_combine(cplx* phi, HistPtr
       acc += cabs2(p);
     }
   }
-  if (part) { double r = block_sum(acc, sh); if (threadIdx.x == 0) part[n * nblk + blockIdx.x] = r; }
+  if (!part) return;
+  const double r = block_sum(acc, sh);
+  if (threadIdx.x == 0) {
+    part[n * nblk + blockIdx.x] = r;
+    __threadfence();
+    s_last = atomicAdd(arrived + n, 1) == nblk - 1;
+  }
+  __syncthreads();
+  if (!s_last || threadIdx.x >= 32) return;
+  __threadfence();
+  double s = 0.0;
+  for (int b = threadIdx.x; b < nblk; b += 32) s += __ldcg(part + n * nblk + b);
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x == 0) { scale[n] = 1.0 / sqrt(s * dV); arrived[n] = 0; }
 }
 
 __global__ void __launch_bounds__(WS_PT_THREADS) k_norm_partials(const cplx* psi, int64_t M, double* part, int nblk) {
