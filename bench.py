@@ -23,7 +23,6 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 import workloads as wl  # noqa: E402
 
@@ -121,10 +120,20 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def make_gpu(w):
+    """A CUDA context configured from the workload (product only: neither the oracle nor the test harness is imported)."""
+    import paper_2602_08982_b200 as ws
+    return wl.configure(ws.Context(w.mode, w.dims, w.dx, w.n_wf, **wl.context_kwargs(w)), w)
+
+
+def make_oracle(w):
+    import oracle as orc
+    return wl.configure(orc.Oracle(w.mode, w.dims, w.dx, w.n_wf, **wl.context_kwargs(w)), w)
+
+
 def time_oracle(w, budget_s=20.0, steps=2):
     """The oracle as it stands on the host cores: abm steps on the first n_sub spinors of the workload."""
-    import oracle as orc
-    from harness import make_oracle
+    import oracle as orc                     # the only legs that touch oracle/: cpu_baseline and --impl reference
     threads = orc.num_threads()
     n_sub = min(w.n_wf, max(threads, 1) * 2)
     best = None
@@ -155,7 +164,6 @@ def run_reference(args):
         return
     w, desc = make_workload(args.config, args.n_wf)
     import oracle as orc
-    from harness import make_oracle
     orc.build()
     cal, _ = time_oracle(w, budget_s=4.0, steps=1)                 # calibration: spinor-steps/s
     total = args.steps + args.warmup
@@ -204,7 +212,6 @@ def run_gpu(args):
     import torch
     import torch.distributed as dist
     import paper_2602_08982_b200 as ws
-    from harness import make_gpu
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))

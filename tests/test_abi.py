@@ -60,3 +60,16 @@ def test_product_never_imports_the_oracle():
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, fn)).read()
                 assert "import oracle" not in txt and "wslda_oracle" not in txt, fn
+
+
+def test_bench_gpu_arm_does_not_pull_in_the_oracle_or_the_tests():
+    """Importing bench.py (and building its GPU-arm helpers) must leave oracle/ and tests/ untouched: the oracle is
+    imported lazily by the cpu_baseline / --impl reference legs only."""
+    import subprocess
+    import sys
+    code = ("import sys, bench; bench.make_workload('cfg1'); "
+            "bad = [m for m in sys.modules if m == 'oracle' or m.startswith('oracle.') or m == 'harness']; "
+            "assert not bad, bad; assert not any(p.rstrip('/').endswith('tests') for p in sys.path), sys.path")
+    subprocess.run([sys.executable, "-c", code], cwd=ROOT, check=True)
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert "import harness" not in src and "from harness" not in src and '"tests"' not in src

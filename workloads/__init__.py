@@ -350,3 +350,30 @@ def random_spinors(seed, n_wf, shape, dV=1.0):
     psi = z[..., 0] + 1j * z[..., 1]
     nrm = np.sqrt(np.sum(np.abs(psi) ** 2, axis=tuple(range(1, psi.ndim)), keepdims=True) * dV)
     return psi / nrm
+
+
+# ---- context plumbing: hand a Workload's inputs to a context object (the oracle's or the CUDA library's; both expose the
+# same setters).  Argument marshalling only -- used by tests/harness.py, bench.py and __graft_entry__.smoke().
+def context_kwargs(w: "Workload", over=None) -> dict:
+    kw = dict(func_id=w.func_id, force_a1=w.force_a1, spin_symmetric=w.spin_symmetric, kin_form=w.kin_form,
+              ab_order=w.ab_order, am_order=w.am_order, subtract_mean_energy=w.subtract_mean_energy,
+              normalize=w.normalize, four_pi_as=w.four_pi_as, E_cut=w.E_cut, lambda_mode=w.lambda_mode)
+    kw.update(over or {})
+    return kw
+
+
+def configure(c, w: "Workload", n_wf: int | None = None):
+    """Set chemical potentials, the mode table (clipped to the first n_wf spinors), weights, external and fixed fields."""
+    n_wf = w.n_wf if n_wf is None else n_wf
+    c.set_mu(*w.mu)
+    if w.kperp is not None:
+        c.set_modes(w.kperp, w.mult, np.minimum(np.asarray(w.first), n_wf))
+    c.set_weights(np.asarray(w.w_a[:n_wf]), np.asarray(w.w_b[:n_wf]))
+    if w.vext_a is not None or w.delta_ext is not None:
+        shp = w.shape
+        va = None if w.vext_a is None else np.broadcast_to(w.vext_a.reshape(shp), shp).copy()
+        vb = None if w.vext_b is None else np.broadcast_to(w.vext_b.reshape(shp), shp).copy()
+        c.set_external(va, vb, w.delta_ext)
+    if w.fixed:
+        c.set_potentials(**w.fixed)
+    return c
