@@ -12,10 +12,8 @@
 #include "fast3d.cuh"
 #include "mega3d.cuh"
 #include "mega3s.cuh"
-#include "cluster3d.cuh"
+#include "mega3t.cuh"
 #include "mega64.cuh"
-#include "mega64s.cuh"
-#include "mega32p.cuh"
 #include "kernels.cuh"
 
 struct Plan {
@@ -119,9 +117,9 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_mega = o; P.mega_ring_bytes = P.mega_part_bytes = P.mega_acc_bytes = P.mega_sync_bytes = P.mega_pack_bytes = 0;
   if (P.mega) {
     P.mega_ring_bytes = align_up((size_t)F3_RING * P.gs * 2 * M * 16);
-    P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * P.N[0] * 8);
+    P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * (P.N[0] < 64 ? 64 : P.N[0]) * 8);   // mega3t: 64 partial sums per spinor
     P.mega_acc_bytes = align_up((size_t)F3_RING * 4 * M * 8);
-    P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)4 * P.mG * sizeof(int));
+    P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)5 * n_wf * sizeof(int));      // done[4][G <= n_wf] + one arrival counter per spinor
     P.mega_pack_bytes = align_up((size_t)M * 48);
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
@@ -175,11 +173,13 @@ struct wslda_ctx {
   double *s_part, *s_acc, *s_partn;
   F3Sync* s_sync;
   int mega_grid;
-  int f6_version;                  // 64^3 tiling: 1 = two planes per 256-thread CTA, 2 = one plane per 128-thread CTA
-  int c3, c3_grid;                 // 32^3: H psi inside one thread-block cluster (cluster3d.cuh); grid = clusters x 8
   int sep_pm, sep_em;              // mega3s.cuh: x-planes per P item, row pairs per XE item
   int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
-  int pair32;                      // 32^3: pair-of-threads lines (mega32p.cuh) instead of one thread per line
+  int t3, t3_gs, t3_r, t3_ring, t3_lag, t3_grid;    // 32^3 Eq. 40: warp-specialised TMA-fed stage kernel (mega3t.cuh): spinors per group, per heavy super-item
+  T3Maps t3_maps;                  // tensor maps of the arrays the library owns (QL ring, alpha); psi is encoded per launch
+  int spin_limit;                  // bound of the device-side dependency waits (polls of 200 ns)
+  int* err_host;                   // pinned: error word of the last persistent launch (copied back asynchronously)
+  int sticky;                      // a launch could not be made or a device-side wait timed out: every later call fails
   double *f_part[4], *f_partn[4], *f_acc[4];
   int* f_cnt[4];                   // per-spinor arrival counters of k_f3_combine (self-resetting)
   double* raw;
@@ -203,6 +203,13 @@ static wslda_status fail(wslda_ctx* c, wslda_status s, const char* msg) {
   return s;
 }
 static wslda_status cuda_check(wslda_ctx* c, const char* where) {
+  // device-side dependency waits are bounded; a wait that ran out flags the launch, and the flag travels to pinned host
+  // memory behind the launch (asynchronously: it is seen by the first call made after that copy has completed)
+  if (c && c->err_host && *c->err_host && !c->sticky) {
+    c->sticky = 1;
+    snprintf(c->err, 256, "a device-side dependency wait timed out in a persistent stage kernel: results since then are invalid");
+  }
+  if (c && c->sticky) return WSLDA_ECUDA;
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) return WSLDA_OK;
   snprintf(c ? c->err : g_err, 256, "CUDA error at %s: %s", where, cudaGetErrorString(e));
@@ -267,6 +274,10 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   c->prof_ev = new std::vector<cudaEvent_t>(); c->prof_name = new std::vector<const char*>();
   c->prof_work = new std::vector<double>();
   c->m = f->ab_order > f->am_order - 1 ? f->ab_order : f->am_order - 1;
+  c->spin_limit = 1 << 25;           // ~7 s of polling: far beyond any step, short enough to report a stall
+  if (const char* e = getenv("WSLDA_SPIN_LIMIT")) { int v = atoi(e); if (v > 0) c->spin_limit = v; }
+  cudaHostAlloc((void**)&c->err_host, sizeof(int), cudaHostAllocDefault);
+  if (c->err_host) *c->err_host = 0;
   c->dV = 1.0; c->Lperp = 1.0;
   for (int d = 0; d < 3; ++d) {
     c->dx[d] = dx[d];
@@ -340,21 +351,6 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
     cudaFuncSetAttribute(k_f3_pass_c<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (F3_TILE_BYTES + F3_PLANE * 16));
   }
-  c->c3 = 0; c->c3_grid = 0;
-  if (const char* e = getenv("WSLDA_CLUSTER")) c->c3 = atoi(e) != 0 && P.fast && P.N[0] == 32;
-  if (c->c3) {
-    int ncl = 0;
-#define WS_C3_ATTR(K) do { cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, C3_SMEM); \
-      cudaLaunchConfig_t lc = {}; lc.gridDim = dim3(C3_CS * 64); lc.blockDim = dim3(C3_NT); lc.dynamicSmemBytes = C3_SMEM; \
-      int v = 0; if (cudaOccupancyMaxActiveClusters(&v, K, &lc) == cudaSuccess && v > 0 && (ncl == 0 || v < ncl)) ncl = v; } while (0)
-    WS_C3_ATTR((k_c3_hpsi<true, F3_APPLY>)); WS_C3_ATTR((k_c3_hpsi<true, F3_CORR>)); WS_C3_ATTR((k_c3_hpsi<true, F3_RHS>));
-    WS_C3_ATTR((k_c3_hpsi<false, F3_APPLY>)); WS_C3_ATTR((k_c3_hpsi<false, F3_CORR>)); WS_C3_ATTR((k_c3_hpsi<false, F3_RHS>));
-#undef WS_C3_ATTR
-    cudaGetLastError();
-    if (ncl <= 0) ncl = 16;
-    if (const char* e = getenv("WSLDA_CLUSTERS")) { int v = atoi(e); if (v > 0) ncl = v; }
-    c->c3_grid = ncl * C3_CS;
-  }
   if (P.mega) {
     char* b = base + P.off_mega;
     c->m_spec0 = (cplx*)b; c->m_spec1 = (cplx*)(b + P.mega_ring_bytes); c->m_X = (cplx*)(b + 2 * P.mega_ring_bytes);
@@ -376,19 +372,31 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       WS_MEGA_ATTR((k_f3s_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_RHS>));
     }
 #undef WS_MEGA_ATTR
-    c->pair32 = 0;                   // measured slower than one thread per line (127k vs 141k spinor-steps/s): opt-in
-    if (const char* e = getenv("WSLDA_PAIR")) c->pair32 = atoi(e) != 0 && P.N[0] == 32;
-    if (c->pair32) {
-      cudaFuncSetAttribute(k_f5_mega<true, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-      cudaFuncSetAttribute(k_f5_mega<true, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-      cudaFuncSetAttribute(k_f5_mega<true, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-      cudaFuncSetAttribute(k_f5_mega<false, F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-      cudaFuncSetAttribute(k_f5_mega<false, F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-      cudaFuncSetAttribute(k_f5_mega<false, F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * F3_TILE_BYTES);
-    }
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
     c->mega_grid = best * sms;
+    // opt-in (measured slower than the mega3s kernels at configs[3]: DESIGN.md 6.5); WSLDA_T3=1 selects it
+    c->t3 = 0;
+    if (const char* e = getenv("WSLDA_T3")) c->t3 = atoi(e) != 0 && P.sep && f->kin_form == WSLDA_KIN_SYM40;
+    c->t3_gs = 8; c->t3_r = 2; c->t3_grid = sms;
+    if (const char* e = getenv("WSLDA_T3_GROUP")) { int v = atoi(e); if (v > 0 && v <= P.gs) c->t3_gs = v; }
+    if (const char* e = getenv("WSLDA_T3_BLOCK")) { int v = atoi(e); if (v > 1) c->t3_r = v; }
+    if (c->t3_gs > P.gs) c->t3_gs = P.gs;
+    while (c->t3_gs % c->t3_r) --c->t3_r;
+    if (const char* e = getenv("WSLDA_T3_CTAS")) { int v = atoi(e); if (v > 0 && v <= sms) c->t3_grid = v; }
+    c->t3_lag = 5; c->t3_ring = 20;                      // ring depth in blocks of r spinors (> 2 lag + the D items' delay)
+    if (const char* e = getenv("WSLDA_T3_LAG")) { int v = atoi(e); if (v > 0) c->t3_lag = v; }
+    if (const char* e = getenv("WSLDA_T3_RING")) { int v = atoi(e); if (v > 1) c->t3_ring = v; }
+    if ((int64_t)c->t3_ring * c->t3_r > (int64_t)F3_RING * P.gs) c->t3_ring = (int)((int64_t)F3_RING * P.gs / c->t3_r);
+    { const int bpg = c->t3_gs / c->t3_r; if (c->t3_ring < 2 * bpg) c->t3_ring = 2 * bpg; }   // a group's blocks + the next group's
+    if (c->t3) {
+      bool ok = t3_encode_cplx(nullptr, &c->t3_maps.qlX, c->m_spec0, (size_t)c->t3_ring * c->t3_r * 2) &&
+                t3_encode_alpha(&c->t3_maps.alP, &c->t3_maps.alX, c->alpha_a, (size_t)((char*)c->alpha_b - (char*)c->alpha_a));
+      ok = ok && cudaFuncSetAttribute(k_t3_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_BYTES) == cudaSuccess &&
+           cudaFuncSetAttribute(k_t3_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_BYTES) == cudaSuccess &&
+           cudaFuncSetAttribute(k_t3_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_BYTES) == cudaSuccess;
+      if (!ok) { cudaGetLastError(); c->t3 = 0; }            // no TMA encoder / not enough shared memory: the mega3s kernels serve
+    }
     if (const char* e = getenv("WSLDA_MEGA_CTAS")) { int v = atoi(e); if (v > 0) c->mega_grid = v; }
   }
   if (P.f6) {
@@ -403,11 +411,6 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f6_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
     cudaFuncSetAttribute(k_f6_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
-    cudaFuncSetAttribute(k_f6s_mega<F3_APPLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
-    cudaFuncSetAttribute(k_f6s_mega<F3_CORR>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
-    cudaFuncSetAttribute(k_f6s_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, F6_TILE * 16);
-    c->f6_version = 1;               // measured: 11.5k (two planes per CTA) vs 10.0k (one plane per CTA) spinor-steps/s
-    if (const char* e = getenv("WSLDA_MEGA64_V")) c->f6_version = atoi(e) == 2 ? 2 : 1;
   }
   if (P.oc) c->oc_dpart = (double*)(base + P.off_oc);
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
@@ -500,6 +503,7 @@ extern "C" wslda_status wslda_ctx_destroy(wslda_ctx* c) {
   }
   for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e);
   delete c->prof_ev; delete c->prof_name; delete c->prof_work;
+  if (c->err_host) cudaFreeHost(c->err_host);
   free(c);
   return WSLDA_OK;
 }

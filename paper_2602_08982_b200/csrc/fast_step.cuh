@@ -25,20 +25,6 @@ static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk,
   const bool sym = c->f.kin_form == WSLDA_KIN_SYM40;
   const int nspec = sym ? 2 : 1;
   const double fl_plane = 5.0 * M * 10.0 * 2 * cnt * nspec, fl_x = 5.0 * M * P.lg[0] * 2.0 * 2 * cnt * nspec;
-  if (c->c3) {                                             // the three passes inside one thread-block cluster per spinor
-    C3Args k;
-    k.psi = psi_chunk; k.scale = scale_chunk; k.kperp2 = c->kperp2 + n0; k.F = f3_fields(c);
-    k.ky2 = c->k2n[1]; k.kz2 = c->k2n[2];
-    for (int j = 0; j < 32; ++j) k.kx2[j] = c->hk2[0][j];
-    k.invM = c->L.invM; k.kappa = kappa; k.out = out; k.cpart = cpart; k.part = c->f_part[q]; k.cnt = cnt;
-    const int want = cnt * C3_CS, grid = want < c->c3_grid ? want : c->c3_grid;
-    WORK(c, (mode == F3_RHS ? 32.0 : 64.0) * M * cnt, 2 * fl_plane + fl_x);
-    void (*kc)(C3Args);
-    if (sym) kc = mode == F3_APPLY ? k_c3_hpsi<true, F3_APPLY> : mode == F3_CORR ? k_c3_hpsi<true, F3_CORR> : k_c3_hpsi<true, F3_RHS>;
-    else kc = mode == F3_APPLY ? k_c3_hpsi<false, F3_APPLY> : mode == F3_CORR ? k_c3_hpsi<false, F3_CORR> : k_c3_hpsi<false, F3_RHS>;
-    LAUNCHN(c, "k_c3_hpsi", kc, grid, C3_NT, C3_SMEM, st, k);
-    return;
-  }
   F3PassA a;
   a.psi = psi_chunk; a.scale = scale_chunk; a.alpha[0] = c->alpha_a; a.alpha[1] = c->alpha_b;
   a.spec0 = c->f_spec0[q]; a.spec1 = c->f_spec1[q]; a.n_items = cnt * 2 * NX; a.NX = NX;
@@ -66,8 +52,9 @@ static void f3_hpsi(wslda_ctx* c, int q, cudaStream_t st, const cplx* psi_chunk,
 
 // One persistent dataflow launch (mega3d.cuh) over spinors [n0, n0 + n) of the caller's buffers:
 // APPLY: out = H psi (+ eps via k_f3_scal); CORR: psi buffer <- phi_new (normalised) + densities; RHS: out = f(psi).
+static bool f3_uses_t3(const wslda_ctx* c) { return c->t3 && c->f.kin_form == WSLDA_KIN_SYM40; }
 static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, const double* scale, int64_t n0, int64_t n,
-                    cplx* out, const cplx* cpart, double kappa, int do_dens) {
+                    cplx* out, const cplx* cpart, double kappa, int do_dens, double* eps_user = nullptr) {
   const Plan& P = c->P;
   const bool sym = c->f.kin_form == WSLDA_KIN_SYM40;
   F3Mega a;
@@ -92,7 +79,23 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   void (*k)(F3Mega);
   if (sym) k = mode == F3_APPLY ? k_f3_mega<true, F3_APPLY> : mode == F3_CORR ? k_f3_mega<true, F3_CORR> : k_f3_mega<true, F3_RHS>;
   else k = mode == F3_APPLY ? k_f3_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3_mega<false, F3_CORR> : k_f3_mega<false, F3_RHS>;
-  if (c->sep3 && !c->pair32) {                             // 32^3: axis-by-axis Laplacian, two passes (mega3s.cuh)
+  if (f3_uses_t3(c)) {                                     // 32^3 Eq. 40: warp-specialised, TMA-fed (mega3t.cuh)
+    T3Maps maps = c->t3_maps;
+    if (!t3_encode_cplx(&maps.psiP, &maps.psiX, psi, (size_t)2 * n)) { snprintf(c->err, 256, "cuTensorMapEncodeTiled failed (psi)"); c->sticky = 1; return; }
+    T3Mega A;
+    A.m = a; A.m.sync = nullptr; A.sync = (T3Sync*)c->m_sync; A.sn_out = c->scale2 + n0;
+    A.m.eps_out = c->eps + n0; A.eps_user = eps_user;
+    for (int j = 0; j < 32; ++j) { A.k2all[j] = c->hk2[2][j]; A.k2all[32 + j] = c->hk2[1][j]; A.k2all[64 + j] = c->hk2[0][j]; }
+    A.gs = c->t3_gs; A.r = c->t3_r; A.R = c->t3_ring; A.RA = F3_RING; A.lag = c->t3_lag; A.G = (int)((n + A.gs - 1) / A.gs); A.spin_limit = c->spin_limit;
+    A.m.gs = A.gs; A.m.G = A.G;
+    cudaMemsetAsync(c->m_sync, 0, sizeof(T3Sync) + ((size_t)3 * ((n + A.r - 1) / A.r) + (size_t)2 * A.G) * sizeof(int), st);
+    void (*kt)(T3Maps, T3Mega) = mode == F3_APPLY ? k_t3_mega<F3_APPLY> : mode == F3_CORR ? k_t3_mega<F3_CORR> : k_t3_mega<F3_RHS>;
+    LAUNCHN(c, mode == F3_APPLY ? "k_t3_mega_apply" : mode == F3_CORR ? "k_t3_mega_corr" : "k_t3_mega_rhs", kt, c->t3_grid, T3_THREADS,
+            T3_SMEM_BYTES, st, maps, A);
+    cudaMemcpyAsync(c->err_host, &A.sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);      // read at the next API call
+    return;
+  }
+  if (c->sep3) {                             // 32^3: axis-by-axis Laplacian, two passes (mega3s.cuh)
     F3SMega A;
     A.m = a; A.pm = c->sep_pm; A.em = c->sep_em;
     for (int j = 0; j < 32; ++j) { A.k2zy[j] = c->hk2[2][j]; A.k2zy[32 + j] = c->hk2[1][j]; }
@@ -104,17 +107,12 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
     else ks = mode == F3_APPLY ? k_f3s_mega<false, F3_APPLY> : mode == F3_CORR ? k_f3s_mega<false, F3_CORR> : k_f3s_mega<false, F3_RHS>;
     LAUNCHN(c, mode == F3_APPLY ? "k_f3s_mega_apply" : mode == F3_CORR ? "k_f3s_mega_corr" : "k_f3s_mega_rhs", ks, gr, 128,
             4 * F3_TILE_BYTES, st, A);
-    return;
-  }
-  if (c->pair32) {                                         // 32^3: pair-of-threads lines, 256-thread CTAs
-    if (sym) k = mode == F3_APPLY ? k_f5_mega<true, F3_APPLY> : mode == F3_CORR ? k_f5_mega<true, F3_CORR> : k_f5_mega<true, F3_RHS>;
-    else k = mode == F3_APPLY ? k_f5_mega<false, F3_APPLY> : mode == F3_CORR ? k_f5_mega<false, F3_CORR> : k_f5_mega<false, F3_RHS>;
-    LAUNCHN(c, mode == F3_APPLY ? "k_f5_mega_apply" : mode == F3_CORR ? "k_f5_mega_corr" : "k_f5_mega_rhs", k, grid, F5_THREADS,
-            4 * F3_TILE_BYTES, st, a);
+    cudaMemcpyAsync(c->err_host, &c->m_sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);
     return;
   }
   LAUNCHN(c, mode == F3_APPLY ? "k_f3_mega_apply" : mode == F3_CORR ? "k_f3_mega_corr" : "k_f3_mega_rhs", k, grid, 128,
           4 * F3_TILE_BYTES, st, a);
+  cudaMemcpyAsync(c->err_host, &c->m_sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);
 }
 
 // ---- 64^3 (mega64.cuh) -------------------------------------------------------------------------------------------
@@ -145,18 +143,13 @@ static void f6_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   const double M = (double)P.M;
   WORK(c, M * n * (mode == F3_CORR ? 96.0 : 64.0), 5.0 * M * 18.0 * 2.0 * 2 * 2 * n);
   const char* name = mode == F3_APPLY ? "k_f6_mega_apply" : mode == F3_CORR ? "k_f6_mega_corr" : "k_f6_mega_rhs";
-  if (c->f6_version == 2) {                                // one plane per 128-thread CTA, two CTAs per SM
-    const int IT = 4 * F6_N + (mode == F3_APPLY ? 0 : (int)F6S_ND);
-    const long total = (long)(a.G + 5) * IT;
-    const int grid = (int)(total < 296 ? total : 296);
-    void (*k)(F6Mega) = mode == F3_APPLY ? k_f6s_mega<F3_APPLY> : mode == F3_CORR ? k_f6s_mega<F3_CORR> : k_f6s_mega<F3_RHS>;
-    LAUNCHN(c, name, k, grid, F6S_THREADS, F6_TILE * 16, st, a);
-  } else {
+  {
     const int IT = F6_N / 2 + F6_N / 2 + F6_N + (mode == F3_APPLY ? 0 : F6_ND);
     const long total = (long)(a.G + 4) * IT;
     const int grid = (int)(total < 148 ? total : 148);
     void (*k)(F6Mega) = mode == F3_APPLY ? k_f6_mega<F3_APPLY> : mode == F3_CORR ? k_f6_mega<F3_CORR> : k_f6_mega<F3_RHS>;
     LAUNCHN(c, name, k, grid, F6_THREADS, 2 * F6_TILE * 16, st, a);
+    if (c->err_host) cudaMemcpyAsync(c->err_host, &c->s_sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);
   }
 }
 
@@ -179,7 +172,12 @@ static wslda_status f3_apply_h(wslda_ctx* c, const cplx* psi, cplx* hpsi, double
     }
     return cuda_check(c, "apply_h");
   }
-  if (c->P.mega && !c->c3 && n_count > 0) {
+  if (c->P.mega && n_count > 0 && f3_uses_t3(c)) {           // eps_n comes out of the stage kernel itself
+    f3_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0,
+            eps_dev ? eps_dev + n_first : nullptr);
+    return cuda_check(c, "apply_h");
+  }
+  if (c->P.mega && n_count > 0) {
     f3_mega(c, st, F3_APPLY, psi + 2 * n_first * M, nullptr, n_first, n_count, hpsi + 2 * n_first * M, nullptr, 0.0, 0);
     F3Scal s;
     s.part = c->m_part; s.cnt = (int)n_count; s.NX = c->P.N[0]; s.mode = F3_APPLY; s.use_shift = 1; s.normalize = 0;
@@ -270,7 +268,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
   const int used = (int)(n_chunks < ns ? n_chunks : ns);
   auto cnt_of = [&](int64_t k) { return (int)((n_wf - k * fc < fc) ? n_wf - k * fc : fc); };
   const bool fixed = c->f.func_id == WSLDA_FUNC_FIXED;
-  if (P.mega && !c->c3) {                                // stage 1 in chunks, stages 2 and 3 as persistent dataflow kernels
+  if (P.mega) {                                // stage 1 in chunks, stages 2 and 3 as persistent dataflow kernels
     f3_fork(c, s);
     for (int64_t k = 0; k < n_chunks; ++k) {
       const int q = (int)(k % ns); cudaStream_t st = f3_stream(c, s, q);
@@ -288,7 +286,8 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
     if (!fixed) { f3_dens_final(c, used, s.user); potentials(c, s.user); }
     f3_mega(c, s.user, F3_CORR, s.phi, c->f.normalize ? c->scale : nullptr, 0, n_wf, s.phi, s.cpart, s.c0dt, !fixed);
     if (!fixed) {
-      const int slots = (int)(c->P.mG < F3_RING ? c->P.mG : F3_RING);
+      const int64_t mG = f3_uses_t3(c) ? (n_wf + c->t3_gs - 1) / c->t3_gs : c->P.mG;
+      const int slots = (int)(mG < F3_RING ? mG : F3_RING);
       LAUNCH(c, k_f3_dens_final, nb(4 * P.M, 256), 256, 0, s.user, c->m_acc, slots, (int64_t)(4 * P.M), P.M, c->raw);
       potentials(c, s.user);
     }

@@ -120,7 +120,7 @@ __device__ __forceinline__ void f3_wait(int* ctr, int target, F3Sync* sy) {
     int spins = 0;
     while (f3_ld_acquire(ctr) < target) {
       __nanosleep(200);
-      if (++spins > (1 << 23)) { sy->error = 1; break; }
+      if (++spins > (1 << 25)) { sy->error = 1; break; }       // ~7 s; the host reads the flag after the launch (ctx.cuh cuda_check)
     }
   }
   __syncthreads();

@@ -260,49 +260,6 @@ def test_axis_by_axis_stage_kernel_32cubed(small_fast_chunks, monkeypatch, sep, 
     assert ("k_f3s_mega_corr" in names) == (sep == "1") and ("k_f3_mega_corr" in names) == (sep == "0")
 
 
-@pytest.mark.parametrize("kin_form", [0, 1])
-def test_pair_line_kernel_32cubed(small_fast_chunks, monkeypatch, kin_form):
-    """The opt-in pair-of-threads 32^3 stage kernel (mega32p.cuh, WSLDA_PAIR=1): H psi and self-consistent steps."""
-    monkeypatch.setenv("WSLDA_PAIR", "1")
-    w = wl.cfg4(n_side=32, n_wf=10, kin_form=kin_form, n_steps=3)
-    psi0 = w.spinors()
-    o, g = make_oracle(w), make_gpu(w)
-    ref, eref = o.apply_h(psi0)
-    h, e = g.apply_h(to_gpu(psi0))
-    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
-    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
-    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
-    for f in ("delta", "U_a", "rho_a", "nu"):
-        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
-    import torch
-    phi = to_gpu(psi0)
-    hist = [torch.zeros_like(phi) for _ in range(g.m)]
-    hist = g.abm_init(phi, hist, w.dt, 0)
-    assert any(k.startswith("k_f5") for k in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt)))
-
-
-@pytest.mark.parametrize("kin_form", [0, 1])
-def test_cluster_kernel_32cubed(small_fast_chunks, monkeypatch, kin_form):
-    """The thread-block-cluster H psi kernel (cluster3d.cuh, WSLDA_CLUSTER=1): the 3-D transforms stay in the
-    distributed shared memory of 8 CTAs.  H psi and self-consistent steps, ragged chunks."""
-    monkeypatch.setenv("WSLDA_CLUSTER", "1")
-    w = wl.cfg4(n_side=32, n_wf=10, kin_form=kin_form, n_steps=3)
-    psi0 = w.spinors()
-    o, g = make_oracle(w), make_gpu(w)
-    ref, eref = o.apply_h(psi0)
-    h, e = g.apply_h(to_gpu(psi0))
-    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
-    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
-    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
-    for f in ("delta", "U_a", "rho_a", "nu"):
-        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
-    import torch
-    phi = to_gpu(psi0)
-    hist = [torch.zeros_like(phi) for _ in range(g.m)]
-    hist = g.abm_init(phi, hist, w.dt, 0)
-    assert "k_c3_hpsi" in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
-
-
 @pytest.mark.parametrize("case", ["fixed_sym40", "fixed_laplace_noshift", "bdg", "slda_trap_32", "fixed_ab5am5_nonorm"])
 def test_fast3d_abm_matches_oracle(small_fast_chunks, case):
     if case == "fixed_sym40":
@@ -398,11 +355,8 @@ def test_mega64_apply_h():
     assert relerr(h2[1:3], ref[1:3]) < TOL_H and not h2[:1].any()
 
 
-@pytest.mark.parametrize("case", ["cfg5_fixed", "slda_selfconsistent", "cfg5_fixed_one_plane_per_cta"])
-def test_mega64_abm_matches_oracle(case, monkeypatch):
-    if case.endswith("one_plane_per_cta"):
-        monkeypatch.setenv("WSLDA_MEGA64_V", "2")            # the opt-in tiling of mega64s.cuh
-        case = "cfg5_fixed"
+@pytest.mark.parametrize("case", ["cfg5_fixed", "slda_selfconsistent"])
+def test_mega64_abm_matches_oracle(case):
     if case == "cfg5_fixed":
         w = wl.cfg5(n_wf=7, n_steps=3)                       # configs[4] recipe: h_a != h_b, fixed smooth fields
     else:
