@@ -18,6 +18,10 @@
  *    stream) and returns a status; argument errors return WSLDA_EINVAL before any launch; lattice sizes
  *    that are not powers of two >= 2 return WSLDA_EUNSUPPORTED (the paper needs even sizes);
  *    a CUDA error is reported as WSLDA_ECUDA.  wslda_last_error() gives a text for the last failure.
+ *  - the persistent stage kernels wait on device-side completion counters with a bound (wslda_tuning.spin_limit);
+ *    a wait that runs out flags its launch, the flag is copied to the host behind the launch, and from the first
+ *    call that sees it on every call returns WSLDA_ECUDA ("dependency wait timed out"): results are never
+ *    silently wrong, but the report can lag the faulty launch by one call.
  *  - there is no CPU fallback: without a CUDA device every compute call fails with WSLDA_ECUDA.
  */
 #ifndef WSLDA_H
@@ -66,6 +70,33 @@ enum { WSLDA_F_RHO_A = 0, WSLDA_F_RHO_B = 1, WSLDA_F_TAU_A = 2, WSLDA_F_TAU_B = 
 /* which_mask bits of wslda_densities (Eqs. 7a-g) */
 enum { WSLDA_D_RHO = 1u, WSLDA_D_NU = 2u, WSLDA_D_TAU = 4u, WSLDA_D_J = 8u, WSLDA_D_ALL = 15u };
 
+/* Optional tuning of the kernel selection and of the tile / group sizes.  Process-wide: it is read by
+ * wslda_workspace_bytes and wslda_ctx_create (contexts that exist keep what they were created with), so set it
+ * before sizing the workspace.  A zero field means "library default"; NULL restores all defaults.  None of the
+ * fields changes WHAT is computed -- every selectable path is parity-tested against the oracle -- only which
+ * kernels compute it (DESIGN.md section 6 says which path serves which lattice and why it is the default). */
+typedef struct {
+  int disable_fused3d;      /* 1: never use the fused Ny = Nz = 32 kernels (general path everywhere)               */
+  int disable_persistent;   /* 1: fused 3-D: chunk pipeline of three passes instead of the persistent stage kernels */
+  int disable_axis_split;   /* 1: 32^3: three-pass persistent kernel (mega3d) instead of the axis-by-axis one       */
+  int enable_tma_stage;     /* 1: 32^3, Eq. 40: the TMA-fed warp-specialised stage kernel (mega3t; measured slower) */
+  int disable_mega64;       /* 1: 64^3: general path instead of the persistent 64^3 kernels                         */
+  int disable_onchip;       /* 1: lattices <= 4096 points: general path instead of the fused on-chip stages         */
+  int fused_chunk;          /* spinors per chunk of the fused 3-D stage 1 / chunk pipeline (default 32)             */
+  int fused_streams;        /* concurrent chunk streams, 1..4 (default 3)                                           */
+  int group;                /* spinors per group of the persistent kernels, 1..32 (default 32 at 32^3, else 5)      */
+  int p_planes, x_rows;     /* mega3s: x-planes per P item (1, 2, 4, 8; default 4), row pairs per XE item (1, 2, 4; default 2) */
+  int persistent_ctas;      /* cap on the persistent grids (default: all SMs x resident CTAs)                       */
+  int onchip_ctas;          /* cap on the on-chip stage grids                                                       */
+  double chunk_mb;          /* general path: MB of spinors per chunk (default 16)                                   */
+  int fft_radix;            /* general on-chip transform: 4 or 8 (default 8)                                        */
+  int spin_limit;           /* bound of the device-side dependency waits, in polls of 200 ns (default 2^25, about 7 s);
+                               a wait that runs out makes every later call return WSLDA_ECUDA                       */
+  int tma_group, tma_block, tma_ring, tma_lag;   /* mega3t: spinors per group (8), per block (2), ring depth in blocks (20),
+                               ticks between the P, X, E items of a block (5)                                       */
+} wslda_tuning;
+wslda_status wslda_set_tuning(const wslda_tuning* t);
+
 /* Bytes of device workspace wslda_ctx_create needs for this problem (pure host computation; 0 on bad
  * arguments).  dims/dx: host arrays of 3 (Nx,Ny,Nz / dx,dy,dz); non-held axes only enter L_perp (Eqs. 29a, 30a). */
 size_t wslda_workspace_bytes(const int dims[3], wslda_mode mode, int64_t n_wf, const wslda_functional* f);
@@ -80,12 +111,17 @@ wslda_status wslda_ctx_destroy(wslda_ctx* ctx);
 
 /* Transverse modes (quasi-1D/2D; substitutions PAPER.md:413-419, 444-448).  Host arrays: kperp[2*m+{0,1}],
  * multiplicity mult[m], and mode m owns spinors [first[m], first[m+1]); first[0] = 0, first[n_modes] = n_wf. */
-wslda_status wslda_set_modes(wslda_ctx*, int n_modes, const double* kperp, const double* mult, const int64_t* first);
+wslda_status wslda_set_modes(wslda_ctx*, int n_modes, const double* kperp, const double* mult, const int64_t* first,
+                             void* cuda_stream);
 /* Frozen occupation weights f_beta(E_n), f_beta(-E_n); device arrays of n_wf doubles (copied). */
-wslda_status wslda_set_weights(wslda_ctx*, const double* w_a_dev, const double* w_b_dev);
+wslda_status wslda_set_weights(wslda_ctx*, const double* w_a_dev, const double* w_b_dev, void* cuda_stream);
+/* Chemical potentials: host scalars, read when a later call is enqueued. */
 wslda_status wslda_set_mu(wslda_ctx*, double mu_a, double mu_b);
 /* External fields (device, nullable = zero): V_ext_sigma real [M], Delta_ext complex [M]. Copied. */
-wslda_status wslda_set_external(wslda_ctx*, const double* vext_a_dev, const double* vext_b_dev, const void* delta_ext_dev);
+wslda_status wslda_set_external(wslda_ctx*, const double* vext_a_dev, const double* vext_b_dev, const void* delta_ext_dev,
+                                void* cuda_stream);
+/* The three setters above copy on the given stream (stream-ordered like every compute call; the host arrays of
+ * wslda_set_modes may be freed as soon as it returns). */
 /* Fixed potentials (FUNC_FIXED and tests): device arrays alpha_sigma, U_sigma real [M], Delta complex [M];
  * copied; Laplacian of alpha_sigma (Eq. 40) is recomputed spectrally. */
 wslda_status wslda_set_potentials(wslda_ctx*, const double* alpha_a_dev, const double* alpha_b_dev,

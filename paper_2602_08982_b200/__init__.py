@@ -35,6 +35,29 @@ class Functional(C.Structure):
                 ("rho_floor", C.c_double)]
 
 
+class Tuning(C.Structure):
+    _fields_ = [("disable_fused3d", C.c_int), ("disable_persistent", C.c_int), ("disable_axis_split", C.c_int),
+                ("enable_tma_stage", C.c_int), ("disable_mega64", C.c_int), ("disable_onchip", C.c_int),
+                ("fused_chunk", C.c_int), ("fused_streams", C.c_int), ("group", C.c_int), ("p_planes", C.c_int),
+                ("x_rows", C.c_int), ("persistent_ctas", C.c_int), ("onchip_ctas", C.c_int), ("chunk_mb", C.c_double),
+                ("fft_radix", C.c_int), ("spin_limit", C.c_int), ("tma_group", C.c_int), ("tma_block", C.c_int),
+                ("tma_ring", C.c_int), ("tma_lag", C.c_int)]
+
+
+def set_tuning(**kw):
+    """Process-wide kernel selection / tile sizes for contexts created afterwards (wslda_set_tuning); no arguments
+    restores the defaults."""
+    if not kw:
+        lib().wslda_set_tuning(None)
+        return
+    t = Tuning()
+    for k, v in kw.items():
+        if not hasattr(t, k):
+            raise TypeError(f"unknown tuning field {k}")
+        setattr(t, k, v)
+    lib().wslda_set_tuning(C.byref(t))
+
+
 FIELD = dict(rho_a=0, rho_b=1, tau_a=2, tau_b=3, nu=4, ja_x=5, ja_y=6, ja_z=7, jb_x=8, jb_y=9, jb_z=10,
              alpha_a=16, alpha_b=17, U_a=18, U_b=19, delta=20, lap_alpha_a=21, lap_alpha_b=22, lambda_c=23,
              g_eff=24, V_a=25, V_b=26)
@@ -44,7 +67,7 @@ SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "ws
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
-           "wslda_profile_report", "wslda_set_reduce_hook"]
+           "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning"]
 REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 _lib = None
@@ -54,18 +77,17 @@ def lib():
     """Load libwslda.so (building it if the sources are newer); raises if that fails."""
     global _lib
     if _lib is None:
-        if not os.path.exists(_SO):
-            build()
+        build()                                   # no-op when libwslda.so is newer than every source
         L = C.CDLL(_SO)
         L.wslda_workspace_bytes.restype = C.c_size_t
         L.wslda_workspace_bytes.argtypes = [C.POINTER(C.c_int), C.c_int, C.c_int64, C.POINTER(Functional)]
         L.wslda_ctx_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.POINTER(C.c_double), C.c_int,
                                        C.c_int64, C.POINTER(Functional), C.c_void_p, C.c_size_t]
         L.wslda_ctx_destroy.argtypes = [C.c_void_p]
-        L.wslda_set_modes.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
-        L.wslda_set_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_modes.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_weights.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_set_mu.argtypes = [C.c_void_p, C.c_double, C.c_double]
-        L.wslda_set_external.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_set_external.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_set_potentials.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.wslda_get_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.wslda_set_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
@@ -78,6 +100,7 @@ def lib():
         L.wslda_abm_step_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p,
                                           C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
         L.wslda_set_reduce_hook.argtypes = [C.c_void_p, REDUCE_HOOK, C.c_void_p]
+        L.wslda_set_tuning.argtypes = [C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
         L.wslda_profile_report.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.wslda_launch_count.restype = C.c_int64
@@ -137,8 +160,8 @@ class Context:
         self.m = lib().wslda_history_length(self.ctx)
 
     def __del__(self):
-        if getattr(self, "ctx", None):
-            lib().wslda_ctx_destroy(self.ctx)
+        if getattr(self, "ctx", None) and _lib is not None:      # at interpreter exit the module may already be torn down
+            _lib.wslda_ctx_destroy(self.ctx)
             self.ctx = None
 
     # -- helpers
@@ -149,13 +172,25 @@ class Context:
     def _stream(self):
         return C.c_void_p(self.torch.cuda.current_stream().cuda_stream)
 
-    def _dev(self, a, dtype):
+    def _dev(self, a, dtype, numel=None):
         t = self.torch
         if a is None:
             return None
         if not isinstance(a, t.Tensor):
             a = t.as_tensor(a)
-        return a.to(device="cuda", dtype=dtype).contiguous()
+        a = a.to(device="cuda", dtype=dtype).contiguous()
+        if numel is not None and a.numel() != numel:
+            raise WsldaError(f"expected {numel} elements, got {a.numel()}")
+        return a
+
+    def _spinors(self, x, what):
+        """The library reads raw pointers: refuse anything that is not a contiguous complex128 CUDA tensor of the
+        whole-batch shape [n_wf, 2, *held_dims] (a slice, a float32 or a host tensor would be read out of bounds)."""
+        t = self.torch
+        want = (self.n_wf, 2) + self.shape
+        if not (isinstance(x, t.Tensor) and x.is_cuda and x.dtype == t.complex128 and x.is_contiguous() and tuple(x.shape) == want):
+            raise WsldaError(f"{what}: need a contiguous complex128 CUDA tensor of shape {want}")
+        return x
 
     @staticmethod
     def _ptr(t):
@@ -167,25 +202,29 @@ class Context:
         kperp = np.ascontiguousarray(kperp, dtype=np.float64)
         mult = np.ascontiguousarray(mult, dtype=np.float64)
         first = np.ascontiguousarray(first, dtype=np.int64)
-        self._chk(lib().wslda_set_modes(self.ctx, len(mult), kperp.ctypes.data, mult.ctypes.data, first.ctypes.data),
-                  "set_modes")
+        if kperp.size != 2 * len(mult) or len(first) != len(mult) + 1:
+            raise WsldaError("set_modes: need kperp[n_modes][2], mult[n_modes], first[n_modes + 1]")
+        self._chk(lib().wslda_set_modes(self.ctx, len(mult), kperp.ctypes.data, mult.ctypes.data, first.ctypes.data,
+                                        self._stream()), "set_modes")
 
     def set_weights(self, w_a, w_b):
         t = self.torch
-        a, b = self._dev(w_a, t.float64), self._dev(w_b, t.float64)
-        self._chk(lib().wslda_set_weights(self.ctx, self._ptr(a), self._ptr(b)), "set_weights")
+        a, b = self._dev(w_a, t.float64, self.n_wf), self._dev(w_b, t.float64, self.n_wf)
+        self._chk(lib().wslda_set_weights(self.ctx, self._ptr(a), self._ptr(b), self._stream()), "set_weights")
+        t.cuda.current_stream().synchronize()            # a, b are temporaries: keep them alive until the copy is done
 
     def set_mu(self, mu_a, mu_b):
         self._chk(lib().wslda_set_mu(self.ctx, float(mu_a), float(mu_b)), "set_mu")
 
     def set_external(self, vext_a=None, vext_b=None, delta_ext=None):
         t = self.torch
-        a, b, d = self._dev(vext_a, t.float64), self._dev(vext_b, t.float64), self._dev(delta_ext, t.complex128)
-        self._chk(lib().wslda_set_external(self.ctx, self._ptr(a), self._ptr(b), self._ptr(d)), "set_external")
+        a, b, d = self._dev(vext_a, t.float64, self.M), self._dev(vext_b, t.float64, self.M), self._dev(delta_ext, t.complex128, self.M)
+        self._chk(lib().wslda_set_external(self.ctx, self._ptr(a), self._ptr(b), self._ptr(d), self._stream()), "set_external")
+        t.cuda.current_stream().synchronize()
 
     def set_potentials(self, alpha_a, alpha_b, U_a, U_b, delta):
         t = self.torch
-        args = [self._dev(x, t.float64) for x in (alpha_a, alpha_b, U_a, U_b)] + [self._dev(delta, t.complex128)]
+        args = [self._dev(x, t.float64, self.M) for x in (alpha_a, alpha_b, U_a, U_b)] + [self._dev(delta, t.complex128, self.M)]
         self._chk(lib().wslda_set_potentials(self.ctx, *[self._ptr(x) for x in args], self._stream()), "set_potentials")
         t.cuda.current_stream().synchronize()
 
@@ -207,16 +246,21 @@ class Context:
     def apply_h(self, psi, hpsi=None, eps=None, n_first=0, n_count=None):
         t = self.torch
         n_count = self.n_wf - n_first if n_count is None else n_count
+        self._spinors(psi, "apply_h psi")
         if hpsi is None:
             hpsi = t.zeros_like(psi)
         if eps is None:
             eps = t.zeros(self.n_wf, dtype=t.float64, device="cuda")
+        self._spinors(hpsi, "apply_h hpsi")
+        if not (eps.is_cuda and eps.dtype == t.float64 and eps.is_contiguous() and eps.numel() == self.n_wf):
+            raise WsldaError("apply_h eps: need a contiguous float64 CUDA tensor of n_wf elements")
         self._chk(lib().wslda_apply_h(self.ctx, self._ptr(psi), self._ptr(hpsi), self._ptr(eps), n_first, n_count,
                                       self._stream()), "apply_h")
         return hpsi, eps
 
     def densities(self, psi, n_first=0, n_count=None, which=D_ALL, accumulate=0):
         n_count = self.n_wf - n_first if n_count is None else n_count
+        self._spinors(psi, "densities psi")
         self._chk(lib().wslda_densities(self.ctx, self._ptr(psi), n_first, n_count, which, accumulate, self._stream()),
                   "densities")
 
@@ -224,7 +268,10 @@ class Context:
         self._chk(lib().wslda_update_potentials(self.ctx, self._stream()), "update_potentials")
 
     def _hist(self, f_hist):
-        assert len(f_hist) == self.m, f"need {self.m} history buffers"
+        if len(f_hist) != self.m:
+            raise WsldaError(f"need {self.m} history buffers")
+        for x in f_hist:
+            self._spinors(x, "history buffer")
         return (C.c_void_p * self.m)(*[x.data_ptr() for x in f_hist])
 
     @staticmethod
@@ -233,17 +280,25 @@ class Context:
         return [by[p] for p in ptrs]
 
     def abm_init(self, phi, f_hist, dt, selfstart=1):
+        self._spinors(phi, "abm_init phi")
         ptrs = self._hist(f_hist)
         self._chk(lib().wslda_abm_init(self.ctx, self._ptr(phi), ptrs, float(dt), int(selfstart), self._stream()), "abm_init")
         return self._reorder(f_hist, list(ptrs))
 
     def abm_step(self, phi, f_hist, dt):
+        self._spinors(phi, "abm_step phi")
         ptrs = self._hist(f_hist)
         self._chk(lib().wslda_abm_step(self.ctx, self._ptr(phi), ptrs, float(dt), self._stream()), "abm_step")
         return self._reorder(f_hist, list(ptrs))
 
     def abm_step_host(self, phi_host, f_hist_host, phi, f_hist, dt):
         """End-to-end step from (pinned) host tensors; returns the permuted (host, device) history lists."""
+        t = self.torch
+        want = (self.n_wf, 2) + self.shape
+        for x in [phi_host] + list(f_hist_host):
+            if x.is_cuda or x.dtype != t.complex128 or not x.is_contiguous() or tuple(x.shape) != want:
+                raise WsldaError(f"abm_step_host: host buffers must be contiguous complex128 CPU tensors of shape {want}")
+        self._spinors(phi, "abm_step_host phi")
         hp = (C.c_void_p * self.m)(*[x.data_ptr() for x in f_hist_host])
         dp = self._hist(f_hist)
         self._chk(lib().wslda_abm_step_host(self.ctx, C.c_void_p(phi_host.data_ptr()), hp, self._ptr(phi), dp, float(dt),

@@ -39,6 +39,13 @@ struct Plan {
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
+// process-wide tuning (wslda_set_tuning); all zeros = the library's defaults
+static wslda_tuning g_tune = {};
+extern "C" wslda_status wslda_set_tuning(const wslda_tuning* t) {
+  if (t) g_tune = *t; else g_tune = wslda_tuning{};
+  return WSLDA_OK;
+}
+
 static int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -59,7 +66,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.n_wf = n_wf;
   const int64_t M = P.M;
   double chunk_mb = 16.0;
-  if (const char* e = getenv("WSLDA_CHUNK_MB")) { double v = atof(e); if (v > 0) chunk_mb = v; }
+  if (g_tune.chunk_mb > 0) chunk_mb = g_tune.chunk_mb;
   int64_t cn = (int64_t)(chunk_mb * 1048576.0 / (32.0 * (double)M));
   if (cn < 1) cn = 1;
   if (cn > n_wf) cn = n_wf;
@@ -93,10 +100,10 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
            f->kin_form != WSLDA_KIN_DIVGRAD;
-  if (const char* e = getenv("WSLDA_FAST")) if (atoi(e) == 0) P.fast = 0;
+  if (g_tune.disable_fused3d) P.fast = 0;
   P.fc = 32; P.ns = 3;
-  if (const char* e = getenv("WSLDA_FAST_CHUNK")) { int v = atoi(e); if (v > 0) P.fc = v; }
-  if (const char* e = getenv("WSLDA_FAST_STREAMS")) { int v = atoi(e); if (v > 0 && v <= 4) P.ns = v; }
+  if (g_tune.fused_chunk > 0) P.fc = g_tune.fused_chunk;
+  if (g_tune.fused_streams > 0 && g_tune.fused_streams <= 4) P.ns = g_tune.fused_streams;
   if (P.fc > n_wf) P.fc = (int)n_wf;
   P.off_fast = o; P.fast_spec_bytes = P.fast_part_bytes = P.fast_stream_bytes = 0;
   if (P.fast) {
@@ -106,12 +113,12 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     o += (size_t)P.ns * P.fast_stream_bytes;
   }
   P.mega = P.fast;
-  if (const char* e = getenv("WSLDA_MEGA")) if (atoi(e) == 0) P.mega = 0;
+  if (g_tune.disable_persistent) P.mega = 0;
   // 32^3: the axis-by-axis stage kernels (mega3s.cuh), whose only ring is Q: large groups
   P.sep = P.mega && P.N[0] == 32;
-  if (const char* e = getenv("WSLDA_SEP")) if (atoi(e) == 0) P.sep = 0;
+  if (g_tune.disable_axis_split) P.sep = 0;
   P.gs = P.sep ? 32 : 5;
-  if (const char* e = getenv("WSLDA_MEGA_GROUP")) { int v = atoi(e); if (v > 0 && v <= 32) P.gs = v; }
+  if (g_tune.group > 0 && g_tune.group <= 32) P.gs = g_tune.group;
   if (P.gs > n_wf) P.gs = (int)n_wf;
   P.mG = (int)((n_wf + P.gs - 1) / P.gs);
   P.off_mega = o; P.mega_ring_bytes = P.mega_part_bytes = P.mega_acc_bytes = P.mega_sync_bytes = P.mega_pack_bytes = 0;
@@ -124,7 +131,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
   P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40;
-  if (const char* e = getenv("WSLDA_MEGA64")) if (atoi(e) == 0) P.f6 = 0;
+  if (g_tune.disable_mega64) P.f6 = 0;
   P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = P.f6_partn_bytes = 0;
   if (P.f6) {
     P.f6_ring_bytes = align_up((size_t)F6_RING * M * 16);
@@ -136,11 +143,11 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
   P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
-  if (const char* e = getenv("WSLDA_ONCHIP")) if (atoi(e) == 0) P.oc = 0;
+  if (g_tune.disable_onchip) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
   { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
   { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS, cap = M <= 512 ? 296 : 148; P.oc_grid = (int)(nb_ < cap ? nb_ : cap); }
-  if (const char* e = getenv("WSLDA_ONCHIP_CTAS")) { int v = atoi(e); if (v > 0 && v < P.oc_grid) P.oc_grid = v; }
+  if (g_tune.onchip_ctas > 0 && g_tune.onchip_ctas < P.oc_grid) P.oc_grid = g_tune.onchip_ctas;
   P.off_oc = o; P.oc_dpart_bytes = 0;
   if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes; }
   P.total = o;
@@ -157,7 +164,7 @@ struct wslda_ctx {
   int lambda_valid;
   wslda_reduce_hook reduce_hook;   // multi-GPU: in-place sum over ranks of the density block (nullable)
   void* reduce_user;
-  int raw_local;                   // the density block holds this rank's partial sums (not yet reduced)
+  unsigned raw_local;              // WSLDA_D_* groups of the density block that hold this rank's partial sums (not yet reduced)
   double *kperp2, *cpref, *w_a, *w_b, *scale, *eps, *scale2;
   double* k2n[3];                  // k_d^2 in natural index order
   double hk2[3][64];               // host copy (kernel parameters)
@@ -237,7 +244,7 @@ static inline void prof_end(wslda_ctx* c, cudaStream_t st) { cudaEventRecord((*c
 #define WORK(c, bytes, flops) do { (c)->work_bytes = (double)(bytes); (c)->work_flops = (double)(flops); } while (0)
 
 // stored position p of the in-place DIF transform (radix 8 from L = n down, then the remaining 4 or 2) <-> frequency index
-static int ws_fft_radix() { const char* e = getenv("WSLDA_FFT_RADIX"); return (e && atoi(e) == 4) ? 4 : 8; }
+static int ws_fft_radix() { return g_tune.fft_radix == 4 ? 4 : 8; }
 static void scrambled_freq(int n, std::vector<int>& fr) {
   fr.resize(n);
   const int maxr = ws_fft_radix();
@@ -275,7 +282,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   c->prof_work = new std::vector<double>();
   c->m = f->ab_order > f->am_order - 1 ? f->ab_order : f->am_order - 1;
   c->spin_limit = 1 << 25;           // ~7 s of polling: far beyond any step, short enough to report a stall
-  if (const char* e = getenv("WSLDA_SPIN_LIMIT")) { int v = atoi(e); if (v > 0) c->spin_limit = v; }
+  if (g_tune.spin_limit > 0) c->spin_limit = g_tune.spin_limit;
+  cudaMemcpyToSymbol(g_f3_spin_limit, &c->spin_limit, sizeof(int));
   cudaHostAlloc((void**)&c->err_host, sizeof(int), cudaHostAllocDefault);
   if (c->err_host) *c->err_host = 0;
   c->dV = 1.0; c->Lperp = 1.0;
@@ -365,8 +373,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     WS_MEGA_ATTR((k_f3_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<true, F3_RHS>));
     WS_MEGA_ATTR((k_f3_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3_mega<false, F3_RHS>));
     c->sep3 = P.sep; c->sep_pm = 4; c->sep_em = 2;     // measured: (1,1) 152k, (2,1) 155k, (4,2) 158k spinor-steps/s at 32 per group
-    if (const char* e = getenv("WSLDA_SEP_PM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4 || v == 8) c->sep_pm = v; }
-    if (const char* e = getenv("WSLDA_SEP_EM")) { int v = atoi(e); if (v == 1 || v == 2 || v == 4) c->sep_em = v; }
+    { const int v = g_tune.p_planes; if (v == 1 || v == 2 || v == 4 || v == 8) c->sep_pm = v; }
+    { const int v = g_tune.x_rows; if (v == 1 || v == 2 || v == 4) c->sep_em = v; }
     if (c->sep3) {
       WS_MEGA_ATTR((k_f3s_mega<true, F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<true, F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<true, F3_RHS>));
       WS_MEGA_ATTR((k_f3s_mega<false, F3_APPLY>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_CORR>)); WS_MEGA_ATTR((k_f3s_mega<false, F3_RHS>));
@@ -377,16 +385,16 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->mega_grid = best * sms;
     // opt-in (measured slower than the mega3s kernels at configs[3]: DESIGN.md 6.5); WSLDA_T3=1 selects it
     c->t3 = 0;
-    if (const char* e = getenv("WSLDA_T3")) c->t3 = atoi(e) != 0 && P.sep && f->kin_form == WSLDA_KIN_SYM40;
+    c->t3 = g_tune.enable_tma_stage && P.sep && f->kin_form == WSLDA_KIN_SYM40;
     c->t3_gs = 8; c->t3_r = 2; c->t3_grid = sms;
-    if (const char* e = getenv("WSLDA_T3_GROUP")) { int v = atoi(e); if (v > 0 && v <= P.gs) c->t3_gs = v; }
-    if (const char* e = getenv("WSLDA_T3_BLOCK")) { int v = atoi(e); if (v > 1) c->t3_r = v; }
+    if (g_tune.tma_group > 0 && g_tune.tma_group <= P.gs) c->t3_gs = g_tune.tma_group;
+    if (g_tune.tma_block > 1) c->t3_r = g_tune.tma_block;
     if (c->t3_gs > P.gs) c->t3_gs = P.gs;
     while (c->t3_gs % c->t3_r) --c->t3_r;
-    if (const char* e = getenv("WSLDA_T3_CTAS")) { int v = atoi(e); if (v > 0 && v <= sms) c->t3_grid = v; }
+    if (g_tune.persistent_ctas > 0 && g_tune.persistent_ctas <= sms) c->t3_grid = g_tune.persistent_ctas;
     c->t3_lag = 5; c->t3_ring = 20;                      // ring depth in blocks of r spinors (> 2 lag + the D items' delay)
-    if (const char* e = getenv("WSLDA_T3_LAG")) { int v = atoi(e); if (v > 0) c->t3_lag = v; }
-    if (const char* e = getenv("WSLDA_T3_RING")) { int v = atoi(e); if (v > 1) c->t3_ring = v; }
+    if (g_tune.tma_lag > 0) c->t3_lag = g_tune.tma_lag;
+    if (g_tune.tma_ring > 1) c->t3_ring = g_tune.tma_ring;
     if ((int64_t)c->t3_ring * c->t3_r > (int64_t)F3_RING * P.gs) c->t3_ring = (int)((int64_t)F3_RING * P.gs / c->t3_r);
     { const int bpg = c->t3_gs / c->t3_r; if (c->t3_ring < 2 * bpg) c->t3_ring = 2 * bpg; }   // a group's blocks + the next group's
     if (c->t3) {
@@ -397,7 +405,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
            cudaFuncSetAttribute(k_t3_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, T3_SMEM_BYTES) == cudaSuccess;
       if (!ok) { cudaGetLastError(); c->t3 = 0; }            // no TMA encoder / not enough shared memory: the mega3s kernels serve
     }
-    if (const char* e = getenv("WSLDA_MEGA_CTAS")) { int v = atoi(e); if (v > 0) c->mega_grid = v; }
+    if (g_tune.persistent_ctas > 0) c->mega_grid = g_tune.persistent_ctas;
   }
   if (P.f6) {
     char* b = base + P.off_f6;

@@ -115,12 +115,13 @@ __device__ __forceinline__ int f3_ld_acquire(const int* p) {
 __device__ __forceinline__ void f3_red_release(int* p) {
   asm volatile("red.release.gpu.global.add.s32 [%0], 1;" :: "l"(p) : "memory");
 }
+__constant__ int g_f3_spin_limit = 1 << 25;      // polls of 200 ns (about 7 s); wslda_tuning.spin_limit, set at context creation
 __device__ __forceinline__ void f3_wait(int* ctr, int target, F3Sync* sy) {
   if (threadIdx.x == 0) {
     int spins = 0;
     while (f3_ld_acquire(ctr) < target) {
       __nanosleep(200);
-      if (++spins > (1 << 25)) { sy->error = 1; break; }       // ~7 s; the host reads the flag after the launch (ctx.cuh cuda_check)
+      if (++spins > g_f3_spin_limit) { sy->error = 1; break; }    // the host reads the flag after the launch (ctx.cuh cuda_check)
     }
   }
   __syncthreads();

@@ -6,7 +6,8 @@
 static inline cudaStream_t S(void* s) { return (cudaStream_t)s; }
 static inline unsigned nb(int64_t n, int t) { return (unsigned)((n + t - 1) / t); }
 
-extern "C" wslda_status wslda_set_modes(wslda_ctx* c, int n_modes, const double* kperp, const double* mult, const int64_t* first) {
+extern "C" wslda_status wslda_set_modes(wslda_ctx* c, int n_modes, const double* kperp, const double* mult, const int64_t* first,
+                                        void* stream) {
   if (!c) return WSLDA_EINVAL;
   if (n_modes < 1 || !kperp || !mult || !first || first[0] != 0 || first[n_modes] != c->P.n_wf)
     return fail(c, WSLDA_EINVAL, "set_modes: first[] must run from 0 to n_wf");
@@ -19,15 +20,16 @@ extern "C" wslda_status wslda_set_modes(wslda_ctx* c, int n_modes, const double*
       cp[n] = mult[m] / c->Lperp;
     }
   }
-  cudaMemcpy(c->kperp2, k2.data(), n_wf * 8, cudaMemcpyHostToDevice);
-  cudaMemcpy(c->cpref, cp.data(), n_wf * 8, cudaMemcpyHostToDevice);
+  // pageable host source: the runtime stages the data before returning, the device copy is ordered on the stream
+  cudaMemcpyAsync(c->kperp2, k2.data(), n_wf * 8, cudaMemcpyHostToDevice, S(stream));
+  cudaMemcpyAsync(c->cpref, cp.data(), n_wf * 8, cudaMemcpyHostToDevice, S(stream));
   return cuda_check(c, "set_modes");
 }
 
-extern "C" wslda_status wslda_set_weights(wslda_ctx* c, const double* w_a, const double* w_b) {
+extern "C" wslda_status wslda_set_weights(wslda_ctx* c, const double* w_a, const double* w_b, void* stream) {
   if (!c || !w_a || !w_b) return fail(c, WSLDA_EINVAL, "set_weights: null argument");
-  cudaMemcpy(c->w_a, w_a, c->P.n_wf * 8, cudaMemcpyDeviceToDevice);
-  cudaMemcpy(c->w_b, w_b, c->P.n_wf * 8, cudaMemcpyDeviceToDevice);
+  cudaMemcpyAsync(c->w_a, w_a, c->P.n_wf * 8, cudaMemcpyDeviceToDevice, S(stream));
+  cudaMemcpyAsync(c->w_b, w_b, c->P.n_wf * 8, cudaMemcpyDeviceToDevice, S(stream));
   return cuda_check(c, "set_weights");
 }
 
@@ -37,12 +39,13 @@ extern "C" wslda_status wslda_set_mu(wslda_ctx* c, double mu_a, double mu_b) {
   return WSLDA_OK;
 }
 
-extern "C" wslda_status wslda_set_external(wslda_ctx* c, const double* va, const double* vb, const void* de) {
+extern "C" wslda_status wslda_set_external(wslda_ctx* c, const double* va, const double* vb, const void* de, void* stream) {
   if (!c) return WSLDA_EINVAL;
   const int64_t M = c->P.M;
-  if (va) cudaMemcpy(c->vext_a, va, M * 8, cudaMemcpyDeviceToDevice); else cudaMemset(c->vext_a, 0, M * 8);
-  if (vb) cudaMemcpy(c->vext_b, vb, M * 8, cudaMemcpyDeviceToDevice); else cudaMemset(c->vext_b, 0, M * 8);
-  if (de) cudaMemcpy(c->dext, de, M * 16, cudaMemcpyDeviceToDevice); else cudaMemset(c->dext, 0, M * 16);
+  cudaStream_t st = S(stream);
+  if (va) cudaMemcpyAsync(c->vext_a, va, M * 8, cudaMemcpyDeviceToDevice, st); else cudaMemsetAsync(c->vext_a, 0, M * 8, st);
+  if (vb) cudaMemcpyAsync(c->vext_b, vb, M * 8, cudaMemcpyDeviceToDevice, st); else cudaMemsetAsync(c->vext_b, 0, M * 8, st);
+  if (de) cudaMemcpyAsync(c->dext, de, M * 16, cudaMemcpyDeviceToDevice, st); else cudaMemsetAsync(c->dext, 0, M * 16, st);
   return cuda_check(c, "set_external");
 }
 
@@ -101,6 +104,10 @@ extern "C" wslda_status wslda_set_potentials(wslda_ctx* c, const double* aa, con
 }
 
 static void reduce_densities(wslda_ctx* c, cudaStream_t st);
+static unsigned step_mask(const wslda_ctx* c);
+static inline unsigned dens_group_of_field(int id) {
+  return id <= WSLDA_F_RHO_B ? WSLDA_D_RHO : id <= WSLDA_F_TAU_B ? WSLDA_D_TAU : id == WSLDA_F_NU ? WSLDA_D_NU : WSLDA_D_J;
+}
 
 extern "C" wslda_status wslda_set_reduce_hook(wslda_ctx* c, wslda_reduce_hook hook, void* user) {
   if (!c) return WSLDA_EINVAL;
@@ -124,7 +131,7 @@ extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* s
   }
   if (src) { cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st); return cuda_check(c, "get_field"); }
   if (id < 0 || id > WSLDA_F_JB_Z) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
-  if (c->reduce_hook && c->raw_local) reduce_densities(c, st);
+  if (c->reduce_hook && (c->raw_local & (c->f.spin_symmetric ? WSLDA_D_ALL : dens_group_of_field(id)))) reduce_densities(c, st);
   LAUNCH(c, k_get_density, nb(M, 256), 256, 0, st, c->raw, M, c->f.spin_symmetric, id, (double*)dst);
   return cuda_check(c, "get_field");
 }
@@ -141,12 +148,12 @@ extern "C" wslda_status wslda_set_field(wslda_ctx* c, int id, const void* src, v
     case WSLDA_F_NU:   // interleaved complex -> two planes
       cudaMemcpy2DAsync(c->raw + DP_NU_RE * M, 8, src, 16, 8, M, cudaMemcpyDeviceToDevice, st);
       cudaMemcpy2DAsync(c->raw + DP_NU_IM * M, 8, (const char*)src + 8, 16, 8, M, cudaMemcpyDeviceToDevice, st);
-      c->raw_local = 0;
+      c->raw_local &= ~WSLDA_D_NU;
       return cuda_check(c, "set_field");
     default: return fail(c, WSLDA_EINVAL, "set_field: only raw rho/tau/nu and lambda_c can be set");
   }
   cudaMemcpyAsync(dst, src, M * 8, cudaMemcpyDeviceToDevice, st);
-  if (id != WSLDA_F_LAMBDA_C) c->raw_local = 0;            // the caller supplies whole-system densities
+  if (id != WSLDA_F_LAMBDA_C) c->raw_local &= ~dens_group_of_field(id);     // the caller supplies whole-system densities
   return cuda_check(c, "set_field");
 }
 
@@ -243,8 +250,8 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
   if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
   if (n_first < 0 || n_count < 0 || n_first + n_count > c->P.n_wf) return fail(c, WSLDA_EINVAL, "densities: spinor range out of bounds");
   if (!mask || (mask & ~WSLDA_D_ALL)) return fail(c, WSLDA_EINVAL, "densities: bad which_mask");
-  if (c->reduce_hook && accumulate && !c->raw_local) return fail(c, WSLDA_EINVAL, "densities: accumulate onto a block already summed over the ranks");
-  c->raw_local = 1;
+  if (c->reduce_hook && accumulate && (mask & ~c->raw_local)) return fail(c, WSLDA_EINVAL, "densities: accumulate onto a block already summed over the ranks");
+  c->raw_local |= mask;
   cudaStream_t st = S(stream);
   if (n_count == 0 && !accumulate) {
     LAUNCH(c, k_density_reduce, dim3(nb(c->P.M, 256), DP_COUNT), 256, 0, st, c->dpart, 0, c->raw, c->P.M, mask, 0);
@@ -258,15 +265,31 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
 
 // Sharded runs (wslda_set_reduce_hook): the density block holds this rank's partial sums until the hook has summed it
 // over the ranks; every potential is formed from the reduced block.
+// raw_local is the set of density groups (WSLDA_D_* bits) whose planes hold LOCAL sums: only those are handed to the
+// hook -- a plane that is already a whole-system sum (tau and j left by an earlier wslda_densities while a step rebuilds
+// rho and nu only) must not be summed again.  The groups' planes are contiguous in the order RHO, NU, TAU, J, so the
+// dirty groups are reduced as maximal contiguous runs (one hook call for rho + nu inside a step).
 static void reduce_densities(wslda_ctx* c, cudaStream_t st) {
-  if (c->reduce_hook) c->reduce_hook(c->reduce_user, c->raw, (int64_t)DP_COUNT * c->P.M, (void*)st);
+  if (c->reduce_hook) {
+    static const unsigned grp[4] = {WSLDA_D_RHO, WSLDA_D_NU, WSLDA_D_TAU, WSLDA_D_J};
+    static const int first[5] = {DP_RHO_A, DP_NU_RE, DP_TAU_A, DP_JA0, DP_COUNT};
+    int g = 0;
+    while (g < 4) {
+      if (!(c->raw_local & grp[g])) { ++g; continue; }
+      int h = g;
+      while (h + 1 < 4 && (c->raw_local & grp[h + 1])) ++h;
+      c->reduce_hook(c->reduce_user, c->raw + (int64_t)first[g] * c->P.M, (int64_t)(first[h + 1] - first[g]) * c->P.M, (void*)st);
+      g = h + 1;
+    }
+  }
   c->raw_local = 0;
 }
 
 // fresh: the block was just rebuilt from this rank's spinors (every call inside a step)
 static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
   if (c->f.func_id == WSLDA_FUNC_FIXED) return;
-  if (fresh || c->raw_local) reduce_densities(c, st);
+  if (fresh) c->raw_local |= step_mask(c);               // the planes the step has just rebuilt from this rank's spinors
+  if (c->raw_local) reduce_densities(c, st);
   const int64_t M = c->P.M;
   FuncParams fp;
   fp.func_id = c->f.func_id; fp.force_a1 = c->f.force_a1; fp.spin_symmetric = c->f.spin_symmetric;

@@ -6,6 +6,7 @@ max|x - ref| / max|ref| over the returned array.
 import numpy as np
 import pytest
 
+import paper_2602_08982_b200 as ws
 import workloads as wl
 from harness import make_gpu, make_oracle, relerr, to_gpu, to_np
 
@@ -193,11 +194,19 @@ def test_run_to_run_bit_reproducible():
 
 
 # ---- the fused 3-D path (Ny = Nz = 32): ragged chunks over several concurrent streams ---------------------------
+SMALL = dict(fused_chunk=3, fused_streams=3, group=3)     # ragged last chunk / group, more groups than ring slots
+
+
 @pytest.fixture
-def small_fast_chunks(monkeypatch):
-    monkeypatch.setenv("WSLDA_FAST_CHUNK", "3")
-    monkeypatch.setenv("WSLDA_FAST_STREAMS", "3")
-    monkeypatch.setenv("WSLDA_MEGA_GROUP", "3")          # ragged last group, more groups than ring slots
+def tuning():
+    """tuning(**fields): process-wide wslda_set_tuning for the contexts the test creates; defaults restored afterwards."""
+    yield ws.set_tuning
+    ws.set_tuning()
+
+
+@pytest.fixture
+def small_fast_chunks(tuning):
+    tuning(**SMALL)
 
 
 @pytest.mark.parametrize("kin_form", [0, 1])
@@ -220,9 +229,9 @@ def _kernels_of(g, fn):
     return list(rep)
 
 
-def test_fast3d_multikernel_fallback(small_fast_chunks, monkeypatch):
-    """WSLDA_MEGA=0: the three-pass chunk pipeline on concurrent streams (fast3d.cuh kernels) instead of the persistent kernel."""
-    monkeypatch.setenv("WSLDA_MEGA", "0")
+def test_fast3d_multikernel_fallback(tuning):
+    """disable_persistent: the three-pass chunk pipeline on concurrent streams (fast3d.cuh kernels) instead of the persistent kernel."""
+    tuning(disable_persistent=1, **SMALL)
     w = wl.cfg4(n_side=32, n_wf=10, kin_form=1, n_steps=3)
     psi0 = w.spinors()
     pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
@@ -234,14 +243,11 @@ def test_fast3d_multikernel_fallback(small_fast_chunks, monkeypatch):
     assert "k_f3_pass_c" in _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
 
 
-@pytest.mark.parametrize("sep,pm,em", [("0", None, None), ("1", "1", "1"), ("1", "8", "4"), ("1", "2", "2")])
-def test_axis_by_axis_stage_kernel_32cubed(small_fast_chunks, monkeypatch, sep, pm, em):
+@pytest.mark.parametrize("sep,pm,em", [("0", 0, 0), ("1", 1, 1), ("1", 8, 4), ("1", 2, 2)])
+def test_axis_by_axis_stage_kernel_32cubed(tuning, sep, pm, em):
     """The default 32^3 Eq. 40 stage kernels (mega3s.cuh: Laplacian axis by axis) for several item sizes, ragged groups
-    of 3 spinors, and the three-pass kernels they replace (WSLDA_SEP=0): H psi and self-consistent steps."""
-    monkeypatch.setenv("WSLDA_SEP", sep)
-    if pm:
-        monkeypatch.setenv("WSLDA_SEP_PM", pm)
-        monkeypatch.setenv("WSLDA_SEP_EM", em)
+    of 3 spinors, and the three-pass kernels they replace (disable_axis_split): H psi and self-consistent steps."""
+    tuning(disable_axis_split=int(sep == "0"), p_planes=pm, x_rows=em, **SMALL)
     w = wl.cfg4(n_side=32, n_wf=10, kin_form=1, n_steps=3)
     psi0 = w.spinors()
     o, g = make_oracle(w), make_gpu(w)
@@ -258,6 +264,81 @@ def test_axis_by_axis_stage_kernel_32cubed(small_fast_chunks, monkeypatch, sep, 
     hist = g.abm_init(phi, hist, w.dt, 0)
     names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
     assert ("k_f3s_mega_corr" in names) == (sep == "1") and ("k_f3_mega_corr" in names) == (sep == "0")
+
+
+@pytest.mark.parametrize("nwf,group,block,ring,lag", [(10, 4, 2, 4, 1), (21, 8, 2, 20, 5), (7, 8, 4, 6, 2)])
+def test_tma_stage_kernel_32cubed(tuning, nwf, group, block, ring, lag):
+    """The opt-in TMA-fed, warp-specialised 32^3 Eq. 40 stage kernel (mega3t.cuh, enable_tma_stage): H psi with eps_n,
+    self-consistent steps with ragged groups / blocks and more blocks than ring slots, and the kernels really ran."""
+    tuning(enable_tma_stage=1, tma_group=group, tma_block=block, tma_ring=ring, tma_lag=lag, fused_chunk=3, fused_streams=3)
+    w = wl.cfg4(n_side=32, n_wf=nwf, kin_form=1, n_steps=3)
+    psi0 = w.spinors()
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi0)
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    h2, _ = g.apply_h(to_gpu(psi0), n_first=1, n_count=3)
+    h2 = to_np(h2)
+    assert relerr(h2[1:4], ref[1:4]) < TOL_H and not h2[:1].any() and not h2[4:].any()
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("delta", "U_a", "rho_a", "nu"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_t3_mega_corr" in names and "k_t3_mega_rhs" in names and "k_f3s_mega_corr" not in names
+
+
+@pytest.mark.parametrize("which", ["mega3s_32", "mega3d_16", "mega64", "tma_32"])
+def test_persistent_kernels_bit_reproducible(tuning, which):
+    """The ticketed persistent kernels hand items to whichever CTA is free, but every sum is taken in a fixed order
+    (partial sums per item, densities per ring slot in group order): two runs give identical bits."""
+    if which == "mega3s_32":
+        tuning(group=5); w = wl.cfg4(n_side=32, n_wf=23, kin_form=1, n_steps=3)
+    elif which == "mega3d_16":
+        tuning(group=3); w = generic((16, 32, 32), (1.0, 1.0, 1.0), 11, 1, func_id=2, dt=0.004)
+    elif which == "mega64":
+        w = wl.cfg4(n_side=64, n_wf=5, kin_form=1, n_steps=2)
+    else:
+        tuning(enable_tma_stage=1, tma_group=4, tma_ring=6, tma_lag=2); w = wl.cfg4(n_side=32, n_wf=13, kin_form=1, n_steps=3)
+    psi0 = w.spinors() if w.kidx is not None else spinors(w)
+    import torch
+    outs = []
+    for _ in range(2):
+        g = make_gpu(w)
+        phi = to_gpu(psi0)
+        hist = [torch.zeros_like(phi) for _ in range(g.m)]
+        hist = g.abm_init(phi, hist, w.dt, 0)
+        for _ in range(3):
+            hist = g.abm_step(phi, hist, w.dt)
+        outs.append((to_np(phi).copy(), to_np(hist[0]).copy(), to_np(g.get_field("rho_a")).copy(), to_np(g.get_field("nu")).copy()))
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+def test_device_wait_timeout_is_reported(tuning):
+    """A device-side dependency wait that runs out must not pass silently: with a bound of one poll the
+    persistent kernel flags the launch, the flag travels to the host behind it, and every later call fails with
+    WSLDA_ECUDA and a message naming the cause."""
+    tuning(spin_limit=1, group=2)
+    w = wl.cfg4(n_side=32, n_wf=64, kin_form=1, n_steps=1)
+    g = make_gpu(w)
+    import torch
+    psi = to_gpu(w.spinors())
+    failed = None
+    for _ in range(6):                                   # a wait has to be hit; a handful of launches make it certain
+        try:
+            g.apply_h(psi)
+            torch.cuda.synchronize()
+        except ws.WsldaError as e:
+            failed = str(e)
+            break
+    assert failed is not None and "timed out" in failed
+    with pytest.raises(ws.WsldaError):
+        g.get_field("rho_a")
 
 
 @pytest.mark.parametrize("case", ["fixed_sym40", "fixed_laplace_noshift", "bdg", "slda_trap_32", "fixed_ab5am5_nonorm"])
@@ -442,7 +523,7 @@ def test_cfg5_full_size_sampled_against_oracle():
 
 
 # ---- NEXT-2: the spinor index sharded over ranks, one density sum per build (include/wslda.h: wslda_set_reduce_hook) --
-def _run_sharded(w, psi0, n_steps, n_shards, selfstart=1):
+def _run_sharded(w, psi0, n_steps, n_shards, selfstart=1, pre_all=False, fields=("rho_a", "nu", "delta", "U_a")):
     """n_shards contexts on this GPU, each over its own share of the spinors and stepped by its own host thread;
     the reduce hook is a host rendezvous that sums the density blocks of all shards (what ncclAllReduce does across
     GPUs).  Nothing on the device waits on another launch.  Returns (phi, f_hist[0]) gathered in spinor order."""
@@ -471,11 +552,13 @@ def _run_sharded(w, psi0, n_steps, n_shards, selfstart=1):
 
             g.set_reduce_hook(hook)
             phi = to_gpu(psi0[n0:n1])
+            if pre_all:                                   # every density plane (tau, j too) built once, before the steps
+                g.densities(phi)
             hist = [torch.zeros_like(phi) for _ in range(g.m)]
             hist = g.abm_init(phi, hist, w.dt, selfstart)
             for _ in range(n_steps):
                 hist = g.abm_step(phi, hist, w.dt)
-            out[r] = (to_np(phi), to_np(hist[0]), {f: to_np(g.get_field(f)) for f in ("rho_a", "nu", "delta", "U_a")})
+            out[r] = (to_np(phi), to_np(hist[0]), {f: to_np(g.get_field(f)) for f in fields})
         except BaseException as e:                     # release the other threads, then report
             errs.append(e)
             bar.abort()
@@ -512,6 +595,34 @@ def test_sharded_contexts_match_unsharded_oracle(case, small_fast_chunks):
         for fl in fields:                                          # every shard ends with the whole-system fields
             for f in ("rho_a", "nu", "delta", "U_a"):
                 assert relerr(fl[f], o.get_field(f)) < 1e-8, f
+
+
+@pytest.mark.parametrize("case", ["mega32_sym40", "general_8"])
+def test_sharded_steps_do_not_resum_planes_they_did_not_rebuild(case, small_fast_chunks):
+    """a step rebuilds rho and nu only; the tau and j planes left by an earlier wslda_densities(D_ALL) are
+    already whole-system sums and must not go through the all-reduce again (they grew by world_size per reduction).
+    densities(all) -> steps with the hook: rho, nu, delta equal the unsharded oracle's after the steps, and tau, j --
+    which wslda_abm_step does not refresh (DESIGN R25; the oracle rebuilds every plane) -- still equal the unsharded
+    oracle's densities of the INITIAL spinors, however many reductions went by."""
+    w = wl.cfg4(n_side=32, n_wf=9, kin_form=1, n_steps=3) if case == "mega32_sym40" else wl.cfg4(n_side=8, n_wf=9, kin_form=1, n_steps=3)
+    psi0 = w.spinors()
+    o = make_oracle(w)
+    phi_o = psi0.copy()
+    o.densities(phi_o)
+    stale = {f: o.get_field(f).copy() for f in ("tau_a", "tau_b", "ja_x", "jb_z")}
+    hist_o = [np.zeros_like(psi0) for _ in range(o.m)]
+    hist_o = o.abm_init(phi_o, hist_o, w.dt, 0)
+    for _ in range(w.n_steps):
+        hist_o = o.abm_step(phi_o, hist_o, w.dt)
+    names = ("rho_a", "nu", "tau_a", "tau_b", "ja_x", "jb_z", "delta")
+    for n_shards in (2, 3):
+        phi, f0, fields = _run_sharded(w, psi0, w.n_steps, n_shards, selfstart=0, pre_all=True, fields=names)
+        assert relerr(phi, phi_o) < TOL_ABM
+        for fl in fields:
+            for f in names:
+                ref = stale[f] if f in stale else o.get_field(f)
+                scale = max(np.abs(ref).max(), 1e-30)
+                assert np.abs(fl[f] - ref).max() <= 1e-8 * scale + 1e-13, (f, n_shards)
 
 
 def test_density_allreduce_through_nccl_single_rank():
