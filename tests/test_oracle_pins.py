@@ -615,3 +615,164 @@ def test_p11_conservation_selfconsistent_bdg_full_basis():
         assert relerr(phi, psi0) > 1e-4                       # the state really moved (initial Delta not self-consistent)
         drift.append(abs(E1 - E0) / abs(E0))
     assert drift[0] < 1e-6 and drift[1] < drift[0] / 8, drift   # integrator-level drift, shrinking like dt^p
+
+
+# ------------------------------------------------ P16b: the mode multiplicity (Eqs. 29b-e; k_z list PAPER.md:889)
+def test_p16_mode_multiplicity_folds_plus_minus_kz():
+    """configs[2] keeps k_z >= 0 only and gives every k_z > 0 mode multiplicity 2 (R16).  A quasi-2D run with modes
+    k_z = 0, k_1, k_2, k_3 of multiplicity 1, 2, 2, 2 must give the densities of the FULL 3-D lattice that holds the same
+    in-plane spinors with e^{+i k_z z} AND e^{-i k_z z}: rho, tau, nu are even in k_z and j_x, j_y do not depend on it.
+    A multiplicity that is dropped, squared or applied to the wrong mode fails this."""
+    dims, dx = (8, 4, 8), (1.0, 1.1, 0.9)
+    held = dims[:2]
+    kz = wl.kgrid(dims[2], dx[2])[: dims[2] // 2]                 # 0, k_1, k_2, k_3 (no Nyquist member, R16/R17)
+    mult = np.array([1.0] + [2.0] * (len(kz) - 1))
+    per = 3
+    nq = len(kz) * per
+    psi_q = wl.random_spinors(161, nq, held, dV=np.prod(dx[:2]))
+    wa, wb = wl.uniform01(162, 0, nq), wl.uniform01(163, 0, nq)
+    f = random_fields(164, held)
+    oq = make_fixed(held, dx, nq, 1, f, mode=2, full_dims=list(dims))
+    oq.set_modes(np.stack([kz, 0 * kz], 1), mult, np.arange(len(kz) + 1) * per)
+    oq.set_weights(wa, wb)
+    oq.densities(psi_q)
+    Lz = dims[2] * dx[2]
+    z = np.arange(dims[2]) * dx[2]
+    states, w3a, w3b = [], [], []
+    for n in range(nq):
+        k = kz[n // per]
+        for sgn in ((1.0,) if k == 0 else (1.0, -1.0)):
+            states.append(np.multiply.outer(psi_q[n], np.exp(1j * sgn * k * z)) / np.sqrt(Lz))
+            w3a.append(wa[n]); w3b.append(wb[n])
+    psi3 = np.ascontiguousarray(np.array(states))
+    assert len(states) == per * (1 + 2 * (len(kz) - 1))
+    f3 = {k: np.broadcast_to(v[..., None], dims).copy() for k, v in f.items()}
+    o3 = make_fixed(dims, dx, len(states), 1, f3)
+    o3.set_weights(np.array(w3a), np.array(w3b))
+    o3.densities(psi3)
+    for fld in ("rho_a", "rho_b", "tau_a", "tau_b", "nu", "ja_x", "ja_y", "jb_x", "jb_y"):
+        assert relerr(oq.get_field(fld), o3.get_field(fld)[..., 0]) < 1e-12, fld
+    assert np.abs(o3.get_field("ja_z")).max() < 1e-13 * np.abs(o3.get_field("ja_x")).max() + 1e-15    # +k_z and -k_z cancel
+
+
+# ------------------------------------------------------------------- O8: the energy terms (Eqs. 33a, b, f PAPER.md:479-512)
+def test_o8_kinetic_energy_is_the_expectation_value_of_the_kinetic_operator():
+    """Eq. 33a (in-scope form, no current term): E_kin = int sum_sigma alpha_sigma tau_sigma / 2.  With first derivatives
+    taken as in Eq. 26 (Nyquist dropped) summation by parts is exact, so for H = -1/2 sum_j d_j alpha d_j (DIVGRAD, U = mu =
+    Delta = 0) E_kin = sum_n c_n [w^a_n <u|H_uu|u> + w^b_n <v|(-H_vv)|v>] -- evaluated through orc_apply_h, which the dense
+    matrices of P5 pin, not through the density routine."""
+    shape, dx = (8, 4, 8), (1.0, 0.9, 1.1)
+    n = 7
+    f = random_fields(171, shape)
+    zero = np.zeros(shape)
+    fields = dict(alpha_a=f["alpha_a"], alpha_b=f["alpha_b"], U_a=zero, U_b=zero, delta=zero.astype(complex))
+    o = make_fixed(shape, dx, n, 2, fields, mu=(0.0, 0.0))
+    wa, wb = wl.uniform01(172, 0, n), wl.uniform01(173, 0, n)
+    o.set_weights(wa, wb)
+    dV = float(np.prod(dx))
+    psi = wl.random_spinors(174, n, shape, dV=dV)
+    h, _ = o.apply_h(psi)
+    eu = np.real(np.sum(psi[:, 0].conj() * h[:, 0], axis=(1, 2, 3))) * dV
+    ev = np.real(np.sum(psi[:, 1].conj() * h[:, 1], axis=(1, 2, 3))) * dV
+    o.densities(psi)
+    e = o.energy()
+    assert abs(e["E_kin"] - np.sum(wa * eu - wb * ev)) < 1e-12 * abs(e["E_kin"])
+    assert e["E_kin"] > 0 and abs(e["E_pot"]) == 0 and abs(e["E_pair"]) < 1e-15
+
+
+def test_o8_potential_energy_restores_the_normal_state_energy_of_eq_12b():
+    """Eq. 12b is built so that a free Fermi sea (nu = 0, tau_sigma = (3/5)(6 pi^2 rho_sigma)^{2/3} rho_sigma) has the
+    energy (3/5) rho eps_F 2^{2/3} (0.357 + 0.642 p^2): the alpha-dependent terms of E_kin (33a) and E_pot (33b)
+    cancel.  That closed form pins E_pot once E_kin is pinned, at p = 0 and at finite polarisation."""
+    shape, dx = (4, 4, 4), (1.0, 1.0, 1.0)
+    V = float(np.prod(shape))
+    for ra, rb in ((0.02, 0.02), (0.03, 0.01), (0.011, 0.027)):
+        o = orc.Oracle(3, shape, dx, 1, func_id=2, kin_form=1)
+        one = np.ones(shape)
+        ta = 0.6 * (6 * np.pi ** 2 * ra) ** (2 / 3) * ra
+        tb = 0.6 * (6 * np.pi ** 2 * rb) ** (2 / 3) * rb
+        for name, v in (("rho_a", ra), ("rho_b", rb), ("tau_a", ta), ("tau_b", tb)):
+            o.set_field(name, v * one)
+        o.set_field("nu", 0j * one)
+        o.update_potentials()
+        e = o.energy()
+        rho, p = ra + rb, (ra - rb) / (ra + rb)
+        eF = 0.5 * (3 * np.pi ** 2 * rho) ** (2 / 3)
+        want = 0.6 * rho * eF * 2 ** (2 / 3) * (0.357 + 0.642 * p * p) * V
+        assert abs(e["E_kin"] + e["E_pot"] - want) < 1e-12 * want, (ra, rb)
+        assert e["E_pot"] < 0 < e["E_kin"]
+
+
+def test_o8_external_pairing_energy_is_the_response_of_eps_n_to_delta_ext():
+    """Eq. 33f: E_pair.ext = -int (Delta_ext nu^* + h.c.).  Switching Delta_ext on changes <psi_n|H|psi_n> by
+    2 Re int u_n^* Delta_ext v_n (Eq. 5), and nu = 1/2 sum (w^b - w^a) c_n u_n v_n^* (Eq. 7e), so
+    E_pair.ext = -1/2 sum_n c_n (w^b_n - w^a_n) [eps_n(Delta_ext) - eps_n(0)] -- through orc_apply_h's eps_n."""
+    shape, dx = (8, 4, 4), (1.0, 1.0, 1.2)
+    n = 6
+    M = int(np.prod(shape))
+    dV = float(np.prod(dx))
+    f = random_fields(181, shape)
+    psi = wl.random_spinors(182, n, shape, dV=dV)
+    wa, wb = wl.uniform01(183, 0, n), wl.uniform01(184, 0, n)
+    dext = 0.3 * (wl.normal(185, 0, M) + 1j * wl.normal(186, 0, M)).reshape(shape)
+    o = make_fixed(shape, dx, n, 1, f)
+    o.set_weights(wa, wb)
+    _, e0 = o.apply_h(psi)
+    o.set_external(None, None, dext)
+    _, e1 = o.apply_h(psi)
+    o.densities(psi)
+    e = o.energy()
+    want = -0.5 * np.sum((wb - wa) * (e1 - e0))
+    assert abs(e["E_pair_ext"] - want) < 1e-11 * abs(want) and abs(want) > 1e-5
+
+
+# ------------------------------------------------------- O7: the midpoint rebuild of the starter (Eq. 53 PAPER.md:680-697)
+def test_o7_starter_rebuilds_the_potentials_at_the_midpoint():
+    """Self-consistent BdG on 4x4x2 (Lambda_c static, so Delta(t) = -g_eff(r) nu(t) is the whole nonlinearity).  The
+    starter's single step is exp(-i dt H[phi^(p)]) phi with H rebuilt from the half-step predictor phi^(p) (Eq. 53): a
+    midpoint rule, local error O(dt^3).  Without that rebuild H would be the one of time t and the local error O(dt^2).
+    Reference: the same nonlinear ODE written with the dense matrices of Eq. 28b and integrated by scipy's DOP853."""
+    from scipy.integrate import solve_ivp
+    shape, dx = (4, 4, 2), (1.0, 1.0, 1.0)
+    M = int(np.prod(shape))
+    mu = (0.6, 0.6)
+    vext = 0.2 * wl.normal(191, 0, M).reshape(shape)
+    delta0 = 0.3 + 0.05 * wl.normal(192, 0, M).reshape(shape)
+    one = np.ones(shape)
+    H0 = dense_h(shape, dx, one, one, vext, vext, delta0.astype(complex), mu, 0)
+    lam, Vv = np.linalg.eigh(H0)
+    psi0 = np.ascontiguousarray(Vv.T.reshape(2 * M, 2, *shape))
+    wa, wb = (lam < 0).astype(float), (lam > 0).astype(float)
+
+    def oracle(am):
+        o = orc.Oracle(3, shape, dx, 2 * M, func_id=1, kin_form=0, four_pi_as=-6.0, ab_order=4, am_order=am,
+                       subtract_mean_energy=0, normalize=0)
+        o.set_mu(*mu); o.set_external(vext, vext); o.set_weights(wa, wb)
+        return o
+
+    o = oracle(5)
+    o.densities(psi0); o.update_potentials()
+    geff = o.get_field("g_eff").ravel()
+    assert relerr(o.get_field("delta").ravel(), -geff * o.get_field("nu").ravel()) < 1e-13      # Eq. 10
+    Hkin = dense_h(shape, dx, one, one, vext, vext, 0j * one, mu, 0)                              # everything but Delta
+
+    def rhs(t, y):
+        phi = y.reshape(2 * M, 2, M)
+        u, v = phi[:, 0], phi[:, 1]
+        nu = 0.5 * np.sum((wb - wa)[:, None] * u * v.conj(), axis=0)                              # Eq. 7e, dV = L_perp = 1
+        d = -geff * nu
+        hu = u @ Hkin[:M, :M].T + d[None] * v
+        hv = d.conj()[None] * u + v @ Hkin[M:, M:].T
+        return (-1j * np.stack([hu, hv], 1)).ravel()
+
+    def starter_error(dt):
+        oo = oracle(5)
+        phi = psi0.copy()
+        hist = [np.zeros_like(phi) for _ in range(oo.m)]
+        oo.abm_init(phi, hist, dt, 1)                                                            # m - 1 = 3 starter steps
+        ref = solve_ivp(rhs, (0.0, 3 * dt), psi0.ravel().astype(complex), method="DOP853", rtol=1e-12, atol=1e-14).y[:, -1]
+        return np.max(np.abs(phi.ravel() - ref))
+
+    e1, e2 = starter_error(0.02), starter_error(0.01)
+    assert e1 > 1e-9                                             # far above rounding: the ratio below means something
+    assert 6.0 < e1 / e2 < 10.0, (e1, e2)                        # dt^3 (8); a starter with H frozen at time t gives dt^2 (4)
