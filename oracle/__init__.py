@@ -32,12 +32,12 @@ class Params(C.Structure):
                 ("func_id", C.c_int), ("force_a1", C.c_int), ("spin_symmetric", C.c_int), ("kin_form", C.c_int),
                 ("ab_order", C.c_int), ("am_order", C.c_int), ("subtract_mean_energy", C.c_int),
                 ("normalize", C.c_int), ("four_pi_as", C.c_double), ("C", C.c_double), ("E_cut", C.c_double),
-                ("lambda_mode", C.c_int), ("rho_floor", C.c_double)]
+                ("lambda_mode", C.c_int), ("rho_floor", C.c_double), ("current_terms", C.c_int)]
 
 
 FIELD = dict(rho_a=0, rho_b=1, tau_a=2, tau_b=3, nu=4, ja_x=5, ja_y=6, ja_z=7, jb_x=8, jb_y=9, jb_z=10,
              alpha_a=16, alpha_b=17, U_a=18, U_b=19, delta=20, lap_alpha_a=21, lap_alpha_b=22, lambda_c=23,
-             g_eff=24, V_a=25, V_b=26)
+             g_eff=24, V_a=25, V_b=26, Aa_x=27, Aa_y=28, Aa_z=29, Ab_x=30, Ab_y=31, Ab_z=32)
 _COMPLEX = {4, 20}
 
 _lib = None
@@ -98,14 +98,14 @@ class Oracle:
 
     def __init__(self, mode, dims, dx, n_wf, func_id=0, force_a1=0, spin_symmetric=0, kin_form=0, ab_order=4,
                  am_order=5, subtract_mean_energy=1, normalize=1, four_pi_as=-1.0, C_=-11.11, E_cut=None,
-                 lambda_mode=0, rho_floor=1e-14):
+                 lambda_mode=0, rho_floor=1e-14, current_terms=0):
         dims = list(dims) + [1] * (3 - len(dims))
         dx = list(dx) + [1.0] * (3 - len(dx))
         if E_cut is None:
             E_cut = np.pi ** 2 / (2 * dx[0] ** 2)          # Eq. 22
         self.p = Params(mode, (C.c_int * 3)(*dims), (C.c_double * 3)(*dx), n_wf, func_id, force_a1,
                         spin_symmetric, kin_form, ab_order, am_order, subtract_mean_energy, normalize,
-                        four_pi_as, C_, E_cut, lambda_mode, rho_floor)
+                        four_pi_as, C_, E_cut, lambda_mode, rho_floor, current_terms)
         self.mode, self.dims, self.dx, self.n_wf = mode, dims, dx, n_wf
         self.shape = tuple(dims[:mode])
         self.M = int(np.prod(self.shape))
@@ -175,13 +175,28 @@ class Oracle:
     def update_potentials(self):
         self._chk(lib().orc_update_potentials(self.ctx), "update_potentials")
 
-    def functional_point(self, rho_a, rho_b, tau_a, tau_b, nu, vext_a=0.0, vext_b=0.0, lambda_in=None):
+    def functional_point(self, rho_a, rho_b, tau_a, tau_b, nu, vext_a=0.0, vext_b=0.0, lambda_in=None, j_a=None, j_b=None):
         vin = (C.c_double * 9)(rho_a, rho_b, tau_a, tau_b, complex(nu).real, complex(nu).imag, vext_a, vext_b,
                                0.0 if lambda_in is None else lambda_in)
         out = (C.c_double * 10)()
-        self._chk(lib().orc_functional_point(self.ctx, vin, C.c_int(lambda_in is not None), out), "functional")
+        ja = (C.c_double * 3)(*(j_a if j_a is not None else (0.0, 0.0, 0.0)))
+        jb = (C.c_double * 3)(*(j_b if j_b is not None else (0.0, 0.0, 0.0)))
+        A = (C.c_double * 6)()
+        self._chk(lib().orc_functional_point_j(self.ctx, vin, ja, jb, C.c_int(lambda_in is not None), out, A), "functional")
         return dict(alpha_a=out[0], alpha_b=out[1], V_a=out[2], V_b=out[3], delta=complex(out[4], out[5]),
-                    lambda_c=out[6], g_eff=out[7], edens=out[8])
+                    lambda_c=out[6], g_eff=out[7], edens=out[8], A_a=np.array(A[0:3]), A_b=np.array(A[3:6]))
+
+    def set_velocity(self, vel_a=None, vel_b=None):
+        """External velocity fields v_ext_sigma, arrays [3, *held_dims] (components along non-held axes are ignored)."""
+        def prep(v):
+            if v is None:
+                return None
+            a = np.zeros((3, self.M))
+            v = np.asarray(v, dtype=np.float64).reshape(len(v), self.M)
+            a[: len(v)] = v
+            return a
+        va, vb = prep(vel_a), prep(vel_b)
+        self._chk(lib().orc_set_velocity(self.ctx, _p(va), _p(vb)), "set_velocity")
 
     def _hist_ptrs(self, f_hist):
         assert len(f_hist) == self.m
@@ -204,9 +219,10 @@ class Oracle:
         return self._reorder(f_hist, list(ptrs))
 
     def energy(self):
-        out = (C.c_double * 8)()
+        out = (C.c_double * 10)()
         self._chk(lib().orc_energy(self.ctx, out), "energy")
-        return dict(zip(["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total"], out))
+        return dict(zip(["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total", "E_curr",
+                         "E_vel_ext"], out))
 
 
 def num_threads():

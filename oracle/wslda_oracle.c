@@ -30,6 +30,8 @@ struct orc_ctx {
   cplx   *nu;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
   cplx   *delta, *dext;
+  double *Aa, *Ab;                      /* current potentials A_sigma = dE/dj_sigma, [3][M] */
+  double *vel_a, *vel_b;                /* external velocity fields v_ext_sigma, [3][M] */
   int lambda_valid;
 };
 
@@ -162,6 +164,7 @@ int orc_create(orc_ctx** out, const orc_params* p) {
   c->U_a = dalloc(M); c->U_b = dalloc(M); c->lap_a = dalloc(M); c->lap_b = dalloc(M);
   c->lambda = dalloc(M); c->geff = dalloc(M); c->vext_a = dalloc(M); c->vext_b = dalloc(M);
   c->delta = (cplx*)dalloc(2 * M); c->dext = (cplx*)dalloc(2 * M);
+  c->Aa = dalloc(3 * M); c->Ab = dalloc(3 * M); c->vel_a = dalloc(3 * M); c->vel_b = dalloc(3 * M);
   for (int64_t i = 0; i < M; ++i) c->alpha_a[i] = c->alpha_b[i] = 1.0;
   *out = c;
   return 0;
@@ -171,7 +174,8 @@ void orc_destroy(orc_ctx* c) {
   if (!c) return;
   double* v[] = {c->k[0], c->k[1], c->k[2], c->kperp2, c->cpref, c->w_a, c->w_b, c->rho_a, c->rho_b, c->tau_a,
                  c->tau_b, c->ja, c->jb, (double*)c->nu, c->alpha_a, c->alpha_b, c->V_a, c->V_b, c->U_a, c->U_b,
-                 c->lap_a, c->lap_b, c->lambda, c->geff, c->vext_a, c->vext_b, (double*)c->delta, (double*)c->dext};
+                 c->lap_a, c->lap_b, c->lambda, c->geff, c->vext_a, c->vext_b, (double*)c->delta, (double*)c->dext,
+                 c->Aa, c->Ab, c->vel_a, c->vel_b};
   for (size_t i = 0; i < sizeof(v) / sizeof(v[0]); ++i) free(v[i]);
   free(c);
 }
@@ -198,6 +202,13 @@ int orc_set_external(orc_ctx* c, const double* va, const double* vb, const doubl
   if (va) memcpy(c->vext_a, va, sizeof(double) * M); else memset(c->vext_a, 0, sizeof(double) * M);
   if (vb) memcpy(c->vext_b, vb, sizeof(double) * M); else memset(c->vext_b, 0, sizeof(double) * M);
   if (de) memcpy(c->dext, de, sizeof(cplx) * M); else memset(c->dext, 0, sizeof(cplx) * M);
+  return 0;
+}
+
+int orc_set_velocity(orc_ctx* c, const double* va, const double* vb) {
+  int64_t M = c->M;
+  if (va) memcpy(c->vel_a, va, sizeof(double) * 3 * M); else memset(c->vel_a, 0, sizeof(double) * 3 * M);
+  if (vb) memcpy(c->vel_b, vb, sizeof(double) * 3 * M); else memset(c->vel_b, 0, sizeof(double) * 3 * M);
   return 0;
 }
 
@@ -244,6 +255,7 @@ int orc_get_field(orc_ctx* c, int id, double* dst) {
     case ORC_DELTA: memcpy(dst, c->delta, sizeof(cplx) * M); return 0;
     default: break;
   }
+  if (id >= ORC_AA_X && id <= ORC_AB_Z) src = (id <= ORC_AA_Z ? c->Aa + (id - ORC_AA_X) * M : c->Ab + (id - ORC_AB_X) * M);
   if (src) { memcpy(dst, src, sizeof(double) * M); return 0; }
   if (id < 0 || id > ORC_JB_Z) return -1;
   for (int64_t i = 0; i < M; ++i) {
@@ -303,12 +315,37 @@ static void kinetic(const orc_ctx* c, const cplx* w, const double* alpha, const 
   free(lap);
 }
 
+/* The current / velocity coupling of Eq. 4c: out += -(i/2) {W, grad} w with W = A_sigma - v_ext_sigma real,
+ * {W, grad} w = W . grad w + grad . (W w) over the held axes, both derivatives spectral with the Nyquist rule of an odd
+ * derivative.  In this form the discrete operator is exactly Hermitian (R27). */
+static void add_current_term(const orc_ctx* c, const cplx* w, const double* A, const double* vel, cplx* out) {
+  int64_t M = c->M; int nd = c->nd;
+  cplx* g = (cplx*)malloc(sizeof(cplx) * M * nd); cplx* Ww = (cplx*)malloc(sizeof(cplx) * M);
+  cplx* g2 = (cplx*)malloc(sizeof(cplx) * M * nd);
+  derivs(nd, c->N, c->k, w, NULL, g);
+  for (int d = 0; d < nd; ++d) {
+    for (int64_t i = 0; i < M; ++i) Ww[i] = (A[d * M + i] - vel[d * M + i]) * w[i];
+    derivs(nd, c->N, c->k, Ww, NULL, g2);
+    for (int64_t i = 0; i < M; ++i)
+      out[i] += -0.5 * I * ((A[d * M + i] - vel[d * M + i]) * g[d * M + i] + g2[d * M + i]);
+  }
+  free(g); free(Ww); free(g2);
+}
+
 static double apply_h_one(const orc_ctx* c, int64_t n, const cplx* psi, cplx* hpsi) {
   int64_t M = c->M;
   const cplx *u = psi, *v = psi + M;
   cplx* Ku = (cplx*)malloc(sizeof(cplx) * M); cplx* Kv = (cplx*)malloc(sizeof(cplx) * M);
   kinetic(c, u, c->alpha_a, c->lap_a, c->kperp2[n], Ku);
   kinetic(c, v, c->alpha_b, c->lap_b, c->kperp2[n], Kv);
+  if (c->p.current_terms) {
+    /* row u: h_a u.  Row v: -h_b^* v, and the conjugate of -(i/2){W, grad} is +(i/2){W, grad}, so that
+     * -h_b^* v = -(K_b + U_b) v - (i/2){W_b, grad} v: the coupling enters Kv with the opposite sign (Eq. 4b) */
+    add_current_term(c, u, c->Aa, c->vel_a, Ku);
+    for (int64_t i = 0; i < M; ++i) Kv[i] = -Kv[i];
+    add_current_term(c, v, c->Ab, c->vel_b, Kv);
+    for (int64_t i = 0; i < M; ++i) Kv[i] = -Kv[i];
+  }
   cplx e = 0.0;
   for (int64_t i = 0; i < M; ++i) {
     cplx D = c->delta[i] + c->dext[i];
@@ -402,7 +439,15 @@ static double lambda_c(double alpha_p, double V_p, double mu_p, double E_c, int*
 }
 
 int orc_functional_point(const orc_ctx* c, const double in[9], int use_lambda_in, double out[10]) {
+  const double z[3] = {0, 0, 0}; double A[6];
+  return orc_functional_point_j(c, in, z, z, use_lambda_in, out, A);
+}
+
+int orc_functional_point_j(const orc_ctx* c, const double in[9], const double ja[3], const double jb[3], int use_lambda_in,
+                           double out[10], double A_out[6]) {
   double ra = in[0], rb = in[1], ta = in[2], tb = in[3]; cplx nu = in[4] + I * in[5];
+  double ja2 = ja[0] * ja[0] + ja[1] * ja[1] + ja[2] * ja[2], jb2 = jb[0] * jb[0] + jb[1] * jb[1] + jb[2] * jb[2];
+  for (int d = 0; d < 6; ++d) A_out[d] = 0;
   double va = in[6], vb = in[7];
   double rho = ra + rb; if (rho < c->p.rho_floor) rho = c->p.rho_floor;
   double aa = 1, ab = 1, Va0 = 0, Vb0 = 0, edens = 0, inv_g0;
@@ -424,6 +469,16 @@ int orc_functional_point(const orc_ctx* c, const double in[9], int use_lambda_in
     Vb0 = common * dp_b + B * eF;
     inv_g0 = cbrt(rho) / c->p.C;
     edens = 0.5 * aa * ta + 0.5 * ab * tb + 0.6 * B * rho * eF;
+    if (c->p.current_terms) {
+      /* E_CM + the j-part of E_0 (Eqs. 9b, 9c): sum_sigma (1 - alpha_sigma) j_sigma^2 / (2 rho_sigma);
+       * A_sigma = dE/dj_sigma; V_sigma += dE/drho_sigma of that term, alpha_a = A(p), alpha_b = A(-p) */
+      double rsa = ra < c->p.rho_floor ? c->p.rho_floor : ra, rsb = rb < c->p.rho_floor ? c->p.rho_floor : rb;
+      edens += 0.5 * (1 - aa) * ja2 / rsa + 0.5 * (1 - ab) * jb2 / rsb;
+      for (int d = 0; d < 3; ++d) { A_out[d] = (1 - aa) * ja[d] / rsa; A_out[3 + d] = (1 - ab) * jb[d] / rsb; }
+      double dal = -0.5 * dAp * ja2 / rsa + 0.5 * dAm * jb2 / rsb;      /* through d alpha_sigma / dp */
+      Va0 += dal * dp_a - 0.5 * (1 - aa) * ja2 / (rsa * rsa);
+      Vb0 += dal * dp_b - 0.5 * (1 - ab) * jb2 / (rsb * rsb);
+    }
   }
   int empty = 0;
   double lam = use_lambda_in ? in[8]
@@ -444,11 +499,12 @@ int orc_update_potentials(orc_ctx* c) {
   int64_t M = c->M;
   int frozen = c->p.lambda_mode == 1 && c->lambda_valid;
   for (int64_t i = 0; i < M; ++i) {
-    double ra, rb, ta, tb, ja[3], jb[3], in[9], out[10]; cplx nu;
+    double ra, rb, ta, tb, ja[3], jb[3], in[9], out[10], A[6]; cplx nu;
     folded(c, i, &ra, &rb, &ta, &tb, &nu, ja, jb);
     in[0] = ra; in[1] = rb; in[2] = ta; in[3] = tb; in[4] = creal(nu); in[5] = cimag(nu);
     in[6] = c->vext_a[i]; in[7] = c->vext_b[i]; in[8] = c->lambda[i];
-    orc_functional_point(c, in, frozen, out);
+    orc_functional_point_j(c, in, ja, jb, frozen, out, A);
+    for (int d = 0; d < 3; ++d) { c->Aa[d * M + i] = A[d]; c->Ab[d * M + i] = A[3 + d]; }
     c->alpha_a[i] = out[0]; c->alpha_b[i] = out[1]; c->V_a[i] = out[2]; c->V_b[i] = out[3];
     c->delta[i] = out[4] + I * out[5]; c->lambda[i] = out[6]; c->geff[i] = out[7];
     c->U_a[i] = c->V_a[i] + c->vext_a[i]; c->U_b[i] = c->V_b[i] + c->vext_b[i];
@@ -587,14 +643,21 @@ int orc_abm_step(orc_ctx* c, double* phi_, double** f_hist, double dt) {
 }
 
 /* O8: Eqs. 33a-g with the in-scope energy density (no current terms) */
-int orc_energy(orc_ctx* c, double out[8]) {
+int orc_energy(orc_ctx* c, double out[10]) {
   int64_t M = c->M; double dVf = c->dV * c->Lperp;
-  for (int q = 0; q < 8; ++q) out[q] = 0;
+  for (int q = 0; q < 10; ++q) out[q] = 0;
   for (int64_t i = 0; i < M; ++i) {
     double ra, rb, ta, tb, ja[3], jb[3]; cplx nu;
     folded(c, i, &ra, &rb, &ta, &tb, &nu, ja, jb);
     out[0] += ra * dVf; out[1] += rb * dVf;
     out[2] += 0.5 * (c->alpha_a[i] * ta + c->alpha_b[i] * tb) * dVf;                        /* 33a */
+    if (c->p.current_terms) {
+      double rsa = ra < c->p.rho_floor ? c->p.rho_floor : ra, rsb = rb < c->p.rho_floor ? c->p.rho_floor : rb;
+      double ja2 = ja[0] * ja[0] + ja[1] * ja[1] + ja[2] * ja[2], jb2 = jb[0] * jb[0] + jb[1] * jb[1] + jb[2] * jb[2];
+      out[2] -= 0.5 * (c->alpha_a[i] * ja2 / rsa + c->alpha_b[i] * jb2 / rsb) * dVf;         /* 33a, the -j^2/rho part */
+      out[8] += 0.5 * (ja2 / rsa + jb2 / rsb) * dVf;                                         /* 33d */
+      for (int d = 0; d < 3; ++d) out[9] -= (c->vel_a[d * M + i] * ja[d] + c->vel_b[d * M + i] * jb[d]) * dVf;   /* 33g */
+    }
     if (c->p.func_id == 2) {
       double rho = ra + rb; if (rho < c->p.rho_floor) rho = c->p.rho_floor;
       double p = (ra - rb) / rho; if (p > 1) p = 1; if (p < -1) p = -1;
@@ -605,6 +668,6 @@ int orc_energy(orc_ctx* c, double out[8]) {
     out[5] += (c->vext_a[i] * ra + c->vext_b[i] * rb) * dVf;                                /* 33e */
     out[6] += -2.0 * creal(c->dext[i] * conj(nu)) * dVf;                                    /* 33f */
   }
-  out[7] = out[2] + out[3] + out[4] + out[5] + out[6];
+  out[7] = out[2] + out[3] + out[4] + out[5] + out[6] + out[8] + out[9];
   return 0;
 }

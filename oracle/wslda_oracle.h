@@ -35,13 +35,15 @@ typedef struct {
   double E_cut;                /* Eq. 22                                                                     */
   int    lambda_mode;          /* 0: Lambda_c recomputed at each potential update; 1: frozen after the first */
   double rho_floor;
+  int    current_terms;        /* 1: the current / velocity coupling of Eq. 4c and the j-terms of Eqs. 9b-c */
 } orc_params;
 
 /* field ids for orc_get_field / orc_set_field */
 enum { ORC_RHO_A = 0, ORC_RHO_B = 1, ORC_TAU_A = 2, ORC_TAU_B = 3, ORC_NU = 4 /* complex */,
        ORC_JA_X = 5, ORC_JA_Y = 6, ORC_JA_Z = 7, ORC_JB_X = 8, ORC_JB_Y = 9, ORC_JB_Z = 10,
        ORC_ALPHA_A = 16, ORC_ALPHA_B = 17, ORC_U_A = 18, ORC_U_B = 19, ORC_DELTA = 20 /* complex */,
-       ORC_LAP_ALPHA_A = 21, ORC_LAP_ALPHA_B = 22, ORC_LAMBDA_C = 23, ORC_G_EFF = 24, ORC_V_A = 25, ORC_V_B = 26 };
+       ORC_LAP_ALPHA_A = 21, ORC_LAP_ALPHA_B = 22, ORC_LAMBDA_C = 23, ORC_G_EFF = 24, ORC_V_A = 25, ORC_V_B = 26,
+       ORC_AA_X = 27, ORC_AA_Y = 28, ORC_AA_Z = 29, ORC_AB_X = 30, ORC_AB_Y = 31, ORC_AB_Z = 32 /* current potentials A_sigma */ };
 
 /* --- transforms (O1) ----------------------------------------------------------------------------------- */
 /* in-place radix-2 FFT of n = 2^p complex numbers (interleaved re,im); sign = -1 forward (Eq. 26 convention
@@ -61,6 +63,8 @@ int  orc_set_modes(orc_ctx*, int n_modes, const double* kperp, const double* mul
 int  orc_set_weights(orc_ctx*, const double* w_a, const double* w_b);   /* f_beta(E_n), f_beta(-E_n), frozen */
 int  orc_set_mu(orc_ctx*, double mu_a, double mu_b);
 int  orc_set_external(orc_ctx*, const double* vext_a, const double* vext_b, const double* delta_ext /* complex, nullable */);
+/* external velocity fields v_ext_sigma, [3][M] doubles each (held axes first), nullable = 0 */
+int  orc_set_velocity(orc_ctx*, const double* vel_a, const double* vel_b);
 int  orc_set_potentials(orc_ctx*, const double* alpha_a, const double* alpha_b, const double* U_a,
                         const double* U_b, const double* delta /* complex */);
 int  orc_get_field(orc_ctx*, int field_id, double* dst);
@@ -78,13 +82,19 @@ int  orc_update_potentials(orc_ctx*);
  * in : rho_a, rho_b, tau_a, tau_b, nu(re,im), vext_a, vext_b, lambda_in (used iff use_lambda_in)
  * out: alpha_a, alpha_b, V_a, V_b, delta(re,im), lambda_c, g_eff, energy density (in-scope terms of Eq. 9c) */
 int  orc_functional_point(const orc_ctx*, const double in[9], int use_lambda_in, double out[10]);
+/* the same with the currents j_a, j_b (3 doubles each): with current_terms the energy density gains
+ * sum_sigma (1 - alpha_sigma) j_sigma^2 / (2 rho_sigma) (Eqs. 9b + 9c), V_sigma its derivative, and
+ * A_out[0..2] / A_out[3..5] receive the current potentials A_sigma = dE/dj_sigma. */
+int  orc_functional_point_j(const orc_ctx*, const double in[9], const double ja[3], const double jb[3], int use_lambda_in,
+                            double out[10], double A_out[6]);
 /* O7: fill the ABM history: selfstart=0 -> zeros (stationary start), else f(phi_0) and m-1 Taylor steps
  * (Eqs. 52-54).  f_hist: array of m = max(ab_order, am_order-1) buffers, f_hist[0] = newest. */
 int  orc_abm_init(orc_ctx*, double* phi, double** f_hist, double dt, int selfstart);
 /* O6: one predictor-corrector step following Alg. 2; rotates the roles of f_hist[]. */
 int  orc_abm_step(orc_ctx*, double* phi, double** f_hist, double dt);
-/* O8 diagnostics: out[0..7] = N_a, N_b, E_kin, E_pot, E_pair, E_pot_ext, E_pair_ext, E_total (Eqs. 33a-g). */
-int  orc_energy(orc_ctx*, double out[8]);
+/* O8 diagnostics: out[0..9] = N_a, N_b, E_kin, E_pot, E_pair, E_pot_ext, E_pair_ext, E_total, E_curr, E_vel_ext
+ * (Eqs. 33a-g; E_curr and E_vel_ext, and the -j^2/rho part of E_kin, only with current_terms). */
+int  orc_energy(orc_ctx*, double out[10]);
 int  orc_history_length(const orc_ctx*);
 int  orc_num_threads(void);
 #endif
