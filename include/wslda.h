@@ -57,6 +57,12 @@ typedef struct {
   double E_cut;              /* Eq. 22: default pi^2 / (2 dx^2)                                             */
   int lambda_mode;           /* 0: Lambda_c (Eq. 20) recomputed at every update; 1: frozen after the first  */
   double rho_floor;          /* guard for rho^(1/3) and p at rho -> 0                                       */
+  int current_terms;         /* 1: the current / velocity coupling -(i/2){A_sigma - v_ext_sigma, grad} of Eq. 4c
+                                 with A_sigma = dE/dj_sigma = (1 - alpha_sigma) j_sigma / rho_sigma
+                                 and the j-terms of Eqs. 9b-c in V_sigma.  The
+                                anticommutator is applied as W.grad + grad.(W .), both derivatives spectral with the
+                                Nyquist rule: exactly Hermitian.  Served by the general path (no fused kernels);
+                                wslda_abm_step then also rebuilds j at both stages.  0: h of Eq. 4c without it  */
 } wslda_functional;
 
 /* field ids for wslda_get_field / wslda_set_field.  Densities are returned folded per Eq. 8 when
@@ -65,7 +71,9 @@ enum { WSLDA_F_RHO_A = 0, WSLDA_F_RHO_B = 1, WSLDA_F_TAU_A = 2, WSLDA_F_TAU_B = 
        WSLDA_F_JA_X = 5, WSLDA_F_JA_Y = 6, WSLDA_F_JA_Z = 7, WSLDA_F_JB_X = 8, WSLDA_F_JB_Y = 9, WSLDA_F_JB_Z = 10,
        WSLDA_F_ALPHA_A = 16, WSLDA_F_ALPHA_B = 17, WSLDA_F_U_A = 18, WSLDA_F_U_B = 19, WSLDA_F_DELTA = 20,
        WSLDA_F_LAP_ALPHA_A = 21, WSLDA_F_LAP_ALPHA_B = 22, WSLDA_F_LAMBDA_C = 23, WSLDA_F_G_EFF = 24,
-       WSLDA_F_V_A = 25, WSLDA_F_V_B = 26 };
+       WSLDA_F_V_A = 25, WSLDA_F_V_B = 26,
+       WSLDA_F_AA_X = 27, WSLDA_F_AA_Y = 28, WSLDA_F_AA_Z = 29, WSLDA_F_AB_X = 30, WSLDA_F_AB_Y = 31, WSLDA_F_AB_Z = 32
+       /* current potentials A_sigma (get only; zero unless current_terms and alpha != 1) */ };
 
 /* which_mask bits of wslda_densities (Eqs. 7a-g) */
 enum { WSLDA_D_RHO = 1u, WSLDA_D_NU = 2u, WSLDA_D_TAU = 4u, WSLDA_D_J = 8u, WSLDA_D_ALL = 15u };
@@ -120,7 +128,11 @@ wslda_status wslda_set_mu(wslda_ctx*, double mu_a, double mu_b);
 /* External fields (device, nullable = zero): V_ext_sigma real [M], Delta_ext complex [M]. Copied. */
 wslda_status wslda_set_external(wslda_ctx*, const double* vext_a_dev, const double* vext_b_dev, const void* delta_ext_dev,
                                 void* cuda_stream);
-/* The three setters above copy on the given stream (stream-ordered like every compute call; the host arrays of
+/* External velocity fields v_ext_sigma (a frame moving with v_0, or Omega x r for a rotating frame):
+ * device arrays [3][M] doubles each (components along x, y, z; those of non-held axes are ignored), nullable = zero.
+ * Copied.  WSLDA_ESTATE unless the context was created with current_terms = 1. */
+wslda_status wslda_set_external_velocity(wslda_ctx*, const double* vel_a_dev, const double* vel_b_dev, void* cuda_stream);
+/* The setters above copy on the given stream (stream-ordered like every compute call; the host arrays of
  * wslda_set_modes may be freed as soon as it returns). */
 /* Fixed potentials (FUNC_FIXED and tests): device arrays alpha_sigma, U_sigma real [M], Delta complex [M];
  * copied; Laplacian of alpha_sigma (Eq. 40) is recomputed spectrally. */

@@ -32,7 +32,7 @@ class Functional(C.Structure):
     _fields_ = [("func_id", C.c_int), ("force_a1", C.c_int), ("spin_symmetric", C.c_int), ("kin_form", C.c_int),
                 ("ab_order", C.c_int), ("am_order", C.c_int), ("subtract_mean_energy", C.c_int), ("normalize", C.c_int),
                 ("four_pi_as", C.c_double), ("C", C.c_double), ("E_cut", C.c_double), ("lambda_mode", C.c_int),
-                ("rho_floor", C.c_double)]
+                ("rho_floor", C.c_double), ("current_terms", C.c_int)]
 
 
 class Tuning(C.Structure):
@@ -60,14 +60,14 @@ def set_tuning(**kw):
 
 FIELD = dict(rho_a=0, rho_b=1, tau_a=2, tau_b=3, nu=4, ja_x=5, ja_y=6, ja_z=7, jb_x=8, jb_y=9, jb_z=10,
              alpha_a=16, alpha_b=17, U_a=18, U_b=19, delta=20, lap_alpha_a=21, lap_alpha_b=22, lambda_c=23,
-             g_eff=24, V_a=25, V_b=26)
+             g_eff=24, V_a=25, V_b=26, Aa_x=27, Aa_y=28, Aa_z=29, Ab_x=30, Ab_y=31, Ab_z=32)
 _COMPLEX = {4, 20}
 D_RHO, D_NU, D_TAU, D_J, D_ALL = 1, 2, 4, 8, 15
 SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "wslda_set_modes", "wslda_set_weights",
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
-           "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning"]
+           "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning", "wslda_set_external_velocity"]
 REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 _lib = None
@@ -101,6 +101,7 @@ def lib():
                                           C.POINTER(C.c_void_p), C.c_double, C.c_void_p]
         L.wslda_set_reduce_hook.argtypes = [C.c_void_p, REDUCE_HOOK, C.c_void_p]
         L.wslda_set_tuning.argtypes = [C.c_void_p]
+        L.wslda_set_external_velocity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
         L.wslda_profile_report.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.wslda_launch_count.restype = C.c_int64
@@ -117,11 +118,11 @@ class WsldaError(RuntimeError):
 
 def make_functional(func_id=0, force_a1=0, spin_symmetric=0, kin_form=0, ab_order=4, am_order=5,
                     subtract_mean_energy=1, normalize=1, four_pi_as=-1.0, C_=-11.11, E_cut=None, lambda_mode=0,
-                    rho_floor=1e-14, dx0=1.0):
+                    rho_floor=1e-14, dx0=1.0, current_terms=0):
     if E_cut is None:
         E_cut = 3.141592653589793 ** 2 / (2 * dx0 ** 2)      # Eq. 22
     return Functional(func_id, force_a1, spin_symmetric, kin_form, ab_order, am_order, subtract_mean_energy, normalize,
-                      four_pi_as, C_, E_cut, lambda_mode, rho_floor)
+                      four_pi_as, C_, E_cut, lambda_mode, rho_floor, current_terms)
 
 
 def workspace_bytes(dims, mode, n_wf, functional) -> int:
@@ -220,6 +221,21 @@ class Context:
         t = self.torch
         a, b, d = self._dev(vext_a, t.float64, self.M), self._dev(vext_b, t.float64, self.M), self._dev(delta_ext, t.complex128, self.M)
         self._chk(lib().wslda_set_external(self.ctx, self._ptr(a), self._ptr(b), self._ptr(d), self._stream()), "set_external")
+        t.cuda.current_stream().synchronize()
+
+    def set_velocity(self, vel_a=None, vel_b=None):
+        """External velocity fields v_ext_sigma, arrays [<=3, *held_dims]; needs current_terms=1."""
+        t = self.torch
+
+        def prep(v):
+            if v is None:
+                return None
+            v = self._dev(v, t.float64)
+            out = t.zeros((3, self.M), dtype=t.float64, device="cuda")
+            out[: v.shape[0]] = v.reshape(v.shape[0], self.M)
+            return out
+        a, b = prep(vel_a), prep(vel_b)
+        self._chk(lib().wslda_set_external_velocity(self.ctx, self._ptr(a), self._ptr(b), self._stream()), "set_external_velocity")
         t.cuda.current_stream().synchronize()
 
     def set_potentials(self, alpha_a, alpha_b, U_a, U_b, delta):

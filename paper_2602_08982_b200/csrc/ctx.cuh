@@ -36,6 +36,7 @@ struct Plan {
   size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes, f6_partn_bytes;
   int mega, gs, mG, sep;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
+  size_t off_cur;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -88,18 +89,19 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   }
   int64_t dg = (1184 + P.nblk - 1) / P.nblk; if (dg < 1) dg = 1; if (dg > cn) dg = cn;
   P.dG = (int)dg;
-  P.nscr = 7;
+  P.nscr = f->current_terms ? 8 : 7;          // + the accumulator of the current / velocity term
   size_t o = 0;
   P.off_tables = o; for (int d = 0; d < 3; ++d) o += align_up((size_t)P.N[d] * 40);       // tw (16) + kk (8) + ko (8) + k^2 natural (8)
   P.off_perwf = o; o += 7 * align_up((size_t)n_wf * 8);
   P.off_fields = o; o += align_up((size_t)DP_COUNT * M * 8) + 12 * align_up((size_t)M * 8) + 2 * align_up((size_t)M * 16);
+  P.off_cur = o; if (f->current_terms) o += 3 * align_up((size_t)6 * M * 8);      // A_sigma, v_ext_sigma, W_sigma = A - v: [2][3][M] each
   P.off_part = o; o += 2 * align_up((size_t)cn * P.nblk * 8);
   P.off_dpart = o; o += align_up((size_t)P.dG * DP_COUNT * M * 8);
   P.scr_bytes = align_up((size_t)cn * 2 * M * 16);
   P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
   // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
-           f->kin_form != WSLDA_KIN_DIVGRAD;
+           f->kin_form != WSLDA_KIN_DIVGRAD && !f->current_terms;
   if (g_tune.disable_fused3d) P.fast = 0;
   P.fc = 32; P.ns = 3;
   if (g_tune.fused_chunk > 0) P.fc = g_tune.fused_chunk;
@@ -130,7 +132,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_pack_bytes = align_up((size_t)M * 48);
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
-  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40;
+  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms;
   if (g_tune.disable_mega64) P.f6 = 0;
   P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = P.f6_partn_bytes = 0;
   if (P.f6) {
@@ -142,7 +144,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
-  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE;
+  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->current_terms;
   if (g_tune.disable_onchip) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
   { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
@@ -192,6 +194,7 @@ struct wslda_ctx {
   double* raw;
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
   cplx *delta, *dext;
+  double *cur_A, *cur_v, *cur_W;   // current_terms: [2][3][M] each: A_sigma, v_ext_sigma, W_sigma = A_sigma - v_ext_sigma
   double *part_n, *part_e, *dpart;
   cplx* scr[WS_MAX_SCR];
   int64_t launches;
@@ -335,6 +338,10 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   for (int q = 0; q < 12; ++q) { *pf[q] = (double*)(base + o); o += align_up((size_t)M * 8); }
   c->delta = (cplx*)(base + o); o += align_up((size_t)M * 16);
   c->dext = (cplx*)(base + o); o += align_up((size_t)M * 16);
+  if (f->current_terms) {
+    c->cur_A = (double*)(base + P.off_cur); c->cur_v = c->cur_A + 6 * M; c->cur_W = c->cur_v + 6 * M;
+    cudaMemset(c->cur_A, 0, (size_t)18 * M * 8);
+  }
   c->part_n = (double*)(base + P.off_part);
   c->part_e = (double*)(base + P.off_part + align_up((size_t)P.chunk_n * P.nblk * 8));
   c->dpart = (double*)(base + P.off_dpart);

@@ -71,7 +71,7 @@ __global__ void k_density_reduce(const double* part, int G, double* raw, int64_t
 }
 
 struct FuncParams {
-  int func_id, force_a1, spin_symmetric;
+  int func_id, force_a1, spin_symmetric, current_terms;
   double four_pi_as, C, E_cut, rho_floor, mu_a, mu_b;
 };
 
@@ -107,9 +107,12 @@ __device__ inline double lambda_c(double alpha_p, double V_p, double mu_p, doubl
 }
 
 // One thread per lattice point: alpha_sigma, V_sigma, U_sigma, Lambda_c, g_eff, Delta = -g_eff nu (Eq. 10).
+// With current_terms: A_sigma = dE/dj_sigma = (1 - alpha_sigma) j_sigma / rho_sigma (Eqs. 9b-c)
+// into cur_A [2][3][M], W_sigma = A_sigma - v_ext_sigma into cur_W, and the j-terms of V_sigma.
 __global__ void k_potentials(FuncParams P, const double* raw, const double* vext_a, const double* vext_b, int use_frozen,
                              double* alpha_a, double* alpha_b, double* V_a, double* V_b, double* U_a, double* U_b,
-                             double* lambda, double* geff, cplx* delta, int64_t M) {
+                             double* lambda, double* geff, cplx* delta, int64_t M, double* cur_A, const double* cur_v,
+                             double* cur_W) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M) return;
   const double PI = 3.14159265358979323846;
@@ -133,6 +136,29 @@ __global__ void k_potentials(FuncParams P, const double* raw, const double* vext
     Va0 = common * dp_a + B * eF;
     Vb0 = common * dp_b + B * eF;
     inv_g0 = cbrt(rho) / P.C;                                  // Eq. 19 in reading R1
+    if (P.current_terms) {                                     // energy density + sum (1 - alpha) j^2 / (2 rho_sigma)
+      double ja[3], jb[3], ja2 = 0.0, jb2 = 0.0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double a = raw[(DP_JA0 + d) * M + i], b = raw[(DP_JB0 + d) * M + i];
+        ja[d] = P.spin_symmetric ? a + b : a; jb[d] = P.spin_symmetric ? a + b : b;
+        ja2 += ja[d] * ja[d]; jb2 += jb[d] * jb[d];
+      }
+      const double rsa = ra < P.rho_floor ? P.rho_floor : ra, rsb = rb < P.rho_floor ? P.rho_floor : rb;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { cur_A[d * M + i] = (1.0 - aa) * ja[d] / rsa; cur_A[(3 + d) * M + i] = (1.0 - ab) * jb[d] / rsb; }
+      const double dal = -0.5 * dAp * ja2 / rsa + 0.5 * dAm * jb2 / rsb;
+      Va0 += dal * dp_a - 0.5 * (1.0 - aa) * ja2 / (rsa * rsa);
+      Vb0 += dal * dp_b - 0.5 * (1.0 - ab) * jb2 / (rsb * rsb);
+    }
+  }
+  if (P.current_terms) {
+#pragma unroll
+    for (int d = 0; d < 6; ++d) {
+      const double A = P.func_id == WSLDA_FUNC_BDG ? 0.0 : cur_A[d * M + i];
+      if (P.func_id == WSLDA_FUNC_BDG) cur_A[d * M + i] = 0.0;
+      cur_W[d * M + i] = A - cur_v[d * M + i];
+    }
   }
   bool empty = false;
   const double va = vext_a[i], vb = vext_b[i];

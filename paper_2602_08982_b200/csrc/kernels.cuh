@@ -134,9 +134,11 @@ struct Fields {
 // Pointwise BdG mix (Eqs. 5, 15 PAPER.md:154, 289) from the spectral terms held in scratch s0..s2, laid out
 // [2 n + c][M]:  LAPLACE s0 = lap w;  SYM40 s0 = lap w, s1 = lap(alpha w);  DIVGRAD s_j = d_j(alpha d_j w).
 // psi is scaled by scale_n on the fly.  Writes H psi and per-block partial sums of Re psi^+ H psi.
+// cur (nullable): {W_sigma, grad} w of the current / velocity coupling, same layout; it enters both rows as -(i/2) cur
+// (Eq. 4c; the v row holds -h_b^*, whose coupling term is -conj(-(i/2){W, grad}) = -(i/2){W, grad}).
 __global__ void __launch_bounds__(WS_PT_THREADS) k_hmix(const cplx* psi, const double* scale, const double* kperp2,
                                                         int kin, int nd, const cplx* s0, const cplx* s1, const cplx* s2,
-                                                        Fields F, int64_t M, cplx* out, double* epart, int nblk) {
+                                                        Fields F, int64_t M, cplx* out, double* epart, int nblk, const cplx* cur) {
   __shared__ double sh[32];
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, n = blockIdx.y;
   double acc = 0.0;
@@ -172,6 +174,11 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_hmix(const cplx* psi, const d
     const double pa = F.U_a[i] - F.mu_a, pb = F.U_b[i] - F.mu_b;
     cplx hu = cadd(K[0], cadd(cscale(u, pa), cmul(D, v)));
     cplx hv = csub(cmul(cconj(D), u), cadd(K[1], cscale(v, pb)));
+    if (cur) {
+      const cplx cu = cur[ou], cv = cur[ov];
+      hu.x += 0.5 * cu.y; hu.y -= 0.5 * cu.x;
+      hv.x += 0.5 * cv.y; hv.y -= 0.5 * cv.x;
+    }
     out[ou] = hu; out[ov] = hv;
     acc = u.x * hu.x + u.y * hu.y + v.x * hv.x + v.y * hv.y;   // Re(conj(u) hu + conj(v) hv)
   }
@@ -236,4 +243,20 @@ __global__ void k_real_to_cplx(const double* a, const double* b, cplx* dst, int6
 __global__ void k_cplx_real_part(const cplx* src, double* a, double* b, int64_t M) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < M) { a[i] = src[i].x; b[i] = src[M + i].x; }
+}
+
+// current / velocity coupling, accumulation of {W, grad} w = sum_d [ W_d (d_d w) + d_d (W_d w) ]:
+//   acc (=, +=) f[sigma of the component][i] * t   (f = W_d, [2][M] with stride 3 M between the spins; null: factor 1)
+__global__ void k_cur_acc(cplx* acc, const cplx* t, const double* f, int64_t fstride, int64_t M, int64_t ncomp, int first) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= ncomp * M) return;
+  const int64_t comp = q / M, i = q - comp * M;
+  const double w = f ? f[(comp & 1) * fstride + i] : 1.0;
+  const cplx v = cscale(t[q], w);
+  acc[q] = first ? v : cadd(acc[q], v);
+}
+// W = A - v for the six planes
+__global__ void k_cur_w(const double* A, const double* v, double* W, int64_t n) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q < n) W[q] = A[q] - v[q];
 }

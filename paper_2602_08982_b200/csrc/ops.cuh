@@ -49,6 +49,17 @@ extern "C" wslda_status wslda_set_external(wslda_ctx* c, const double* va, const
   return cuda_check(c, "set_external");
 }
 
+extern "C" wslda_status wslda_set_external_velocity(wslda_ctx* c, const double* va, const double* vb, void* stream) {
+  if (!c) return WSLDA_EINVAL;
+  if (!c->f.current_terms) return fail(c, WSLDA_ESTATE, "set_external_velocity: the context was created without current_terms");
+  const int64_t M = c->P.M;
+  cudaStream_t st = S(stream);
+  if (va) cudaMemcpyAsync(c->cur_v, va, 3 * M * 8, cudaMemcpyDeviceToDevice, st); else cudaMemsetAsync(c->cur_v, 0, 3 * M * 8, st);
+  if (vb) cudaMemcpyAsync(c->cur_v + 3 * M, vb, 3 * M * 8, cudaMemcpyDeviceToDevice, st); else cudaMemsetAsync(c->cur_v + 3 * M, 0, 3 * M * 8, st);
+  LAUNCH(c, k_cur_w, nb(6 * M, 256), 256, 0, st, c->cur_A, c->cur_v, c->cur_W, 6 * M);
+  return cuda_check(c, "set_external_velocity");
+}
+
 // ---- derivative engine: lap / grad of a batch of components (DerivArgs) -------------------------------------
 static void deriv(wslda_ctx* c, const DerivArgs& a, cudaStream_t st) {
   const Plan& P = c->P;
@@ -129,6 +140,10 @@ extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* s
     case WSLDA_F_DELTA: src = c->delta; bytes = M * 16; break;
     default: break;
   }
+  if (id >= WSLDA_F_AA_X && id <= WSLDA_F_AB_Z) {
+    if (c->f.current_terms) src = c->cur_A + (int64_t)(id - WSLDA_F_AA_X) * M;
+    else { cudaMemsetAsync(dst, 0, bytes, st); return cuda_check(c, "get_field"); }
+  }
   if (src) { cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st); return cuda_check(c, "get_field"); }
   if (id < 0 || id > WSLDA_F_JB_Z) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
   if (c->reduce_hook && (c->raw_local & (c->f.spin_symmetric ? WSLDA_D_ALL : dens_group_of_field(id)))) reduce_densities(c, st);
@@ -180,6 +195,21 @@ static void h_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_chu
   const int kin = c->f.kin_form;
   DerivArgs a; memset(&a, 0, sizeof a);
   a.src = psi_chunk; a.src_comp0 = 0; a.ncomp = (int)(2 * cnt); a.scale = scale_chunk;
+  cplx* cur = nullptr;
+  if (c->f.current_terms) {                               // {W, grad} w first: scr[2] is free until the kinetic terms
+    cur = c->scr[7];
+    cplx* tmp = c->scr[2];
+    const int64_t tot = 2 * cnt * M;
+    for (int d = 0; d < P.nd; ++d) {
+      const double* Wd = c->cur_W + (int64_t)d * M;      // W_a,d; W_b,d sits 3 M further
+      DerivArgs g = a; g.out[1 + d] = tmp;
+      deriv(c, g, st);
+      LAUNCH(c, k_cur_acc, nb(tot, 256), 256, 0, st, cur, tmp, Wd, 3 * M, M, 2 * cnt, d == 0 ? 1 : 0);
+      DerivArgs h = a; h.premul[0] = Wd; h.premul[1] = Wd + 3 * M; h.out[1 + d] = tmp;
+      deriv(c, h, st);
+      LAUNCH(c, k_cur_acc, nb(tot, 256), 256, 0, st, cur, tmp, (const double*)nullptr, 0, M, 2 * cnt, 0);
+    }
+  }
   if (kin == WSLDA_KIN_DIVGRAD) {
     for (int d = 0; d < P.nd; ++d) a.out[1 + d] = c->scr[d];
     deriv(c, a, st);
@@ -200,7 +230,7 @@ static void h_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_chu
   }
   WORK(c, 64.0 * M * cnt, 0);      // reads psi, writes H psi
   LAUNCH(c, k_hmix, dim3(P.nblk, (unsigned)cnt), P.pt_threads, 0, st, psi_chunk, scale_chunk, c->kperp2 + n0, kin, P.nd,
-         c->scr[0], c->scr[1], c->scr[2], fields_of(c), M, out, want_eps ? c->part_e : nullptr, P.nblk);
+         c->scr[0], c->scr[1], c->scr[2], fields_of(c), M, out, want_eps ? c->part_e : nullptr, P.nblk, (const cplx*)cur);
 }
 
 extern "C" wslda_status wslda_apply_h(wslda_ctx* c, const void* psi_, void* hpsi_, double* eps_dev, int64_t n_first,
@@ -293,11 +323,12 @@ static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
   const int64_t M = c->P.M;
   FuncParams fp;
   fp.func_id = c->f.func_id; fp.force_a1 = c->f.force_a1; fp.spin_symmetric = c->f.spin_symmetric;
+  fp.current_terms = c->f.current_terms;
   fp.four_pi_as = c->f.four_pi_as; fp.C = c->f.C; fp.E_cut = c->f.E_cut; fp.rho_floor = c->f.rho_floor;
   fp.mu_a = c->mu_a; fp.mu_b = c->mu_b;
   const int frozen = c->f.lambda_mode == 1 && c->lambda_valid;
   LAUNCH(c, k_potentials, nb(M, 128), 128, 0, st, fp, c->raw, c->vext_a, c->vext_b, frozen, c->alpha_a, c->alpha_b, c->V_a,
-         c->V_b, c->U_a, c->U_b, c->lambda, c->geff, c->delta, M);
+         c->V_b, c->U_a, c->U_b, c->lambda, c->geff, c->delta, M, c->cur_A, c->cur_v, c->cur_W);
   c->lambda_valid = 1;
   if (c->f.kin_form == WSLDA_KIN_SYM40 && c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1) update_lap_alpha(c, st);
 }

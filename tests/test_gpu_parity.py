@@ -658,3 +658,61 @@ def test_density_allreduce_through_nccl_single_rank():
     finally:
         if created:
             dist.destroy_process_group()
+
+
+# ---- NEXT-1: current / velocity coupling (Eq. 4c, Eqs. 9b-c), general path ---------------
+def _with_currents(w, seed, amp=0.2):
+    M = int(np.prod(w.shape))
+    nd = len(w.shape)
+    v = amp * wl.normal(seed, 0, 6 * M).reshape(2, 3, *w.shape)
+    w.current_terms = 1
+    w.vel = (v[0, :nd], v[1, :nd])
+    return w
+
+
+@pytest.mark.parametrize("kin_form", [0, 1, 2])
+@pytest.mark.parametrize("shape,dx", [((8, 4, 8), (1.0, 0.9, 1.1)), ((16, 8), (1.0, 1.2)), ((32,), (0.8,)),
+                                      ((32, 16, 16), (1.0, 1.0, 0.9)), ((8, 32, 32), (1.0, 1.1, 0.9))])
+def test_current_coupling_apply_h_matches_oracle(shape, dx, kin_form):
+    """H psi with rough external velocity fields on every lattice regime of the general path (on-chip, multi-pass, and
+    a Ny = Nz = 32 lattice, where the fused kernels step aside for the coupling term)."""
+    n_wf = 5 if np.prod(shape) > 4096 else 13
+    w = _with_currents(generic(shape, dx, n_wf, kin_form, n_modes=2), 401)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi)
+    h, e = g.apply_h(to_gpu(psi))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    w0 = generic(shape, dx, n_wf, kin_form, n_modes=2)            # and the term is not a rounding matter
+    assert relerr(make_oracle(w0).apply_h(psi)[0], ref) > 1e-3
+
+
+@pytest.mark.parametrize("case", ["aslda_polarised", "aslda_symmetric", "bdg_moving_frame", "fixed"])
+def test_current_coupling_selfconsistent_steps(case):
+    """Self-consistent steps with the coupling: A_sigma = (1 - alpha_sigma) j_sigma / rho_sigma rebuilt at both stages of
+    Alg. 2 (j joins the densities the step refreshes), the j-terms of V_sigma, a uniform frame velocity for BdG."""
+    shape, dx = (8, 8, 8), (1.0, 1.0, 1.0)
+    if case == "fixed":
+        w = _with_currents(generic(shape, dx, 12, 1, dt=0.004), 411)
+    else:
+        w = wl.cfg4(n_side=8, n_wf=24, kin_form=1, n_steps=4)
+        if case == "aslda_polarised":
+            w.spin_symmetric = 0
+            w.w_a = 0.6 * np.asarray(w.w_b)                     # both spin densities populated, p != 0: alpha_a != alpha_b != 1
+        elif case == "bdg_moving_frame":
+            w.func_id, w.kin_form, w.four_pi_as = 1, 0, -3.0
+        w = _with_currents(w, 412, amp=0.05)
+        if case == "bdg_moving_frame":
+            v = np.zeros((3,) + shape); v[0] = 0.1
+            w.vel = (v, v)
+    psi0 = w.spinors() if w.kidx is not None else spinors(w)
+    pg, po, fg, fo, o, g = run_both(w, psi0, 4, selfstart=1)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    if case != "fixed":
+        for f in ("rho_a", "nu", "delta", "U_a", "U_b", "alpha_a"):
+            assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    if case.startswith("aslda"):
+        for f in ("ja_x", "jb_z", "Aa_x", "Ab_y", "V_a"):
+            ref = o.get_field(f)
+            assert np.abs(ref).max() > 0
+            assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f

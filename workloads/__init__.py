@@ -358,6 +358,8 @@ def context_kwargs(w: "Workload", over=None) -> dict:
     kw = dict(func_id=w.func_id, force_a1=w.force_a1, spin_symmetric=w.spin_symmetric, kin_form=w.kin_form,
               ab_order=w.ab_order, am_order=w.am_order, subtract_mean_energy=w.subtract_mean_energy,
               normalize=w.normalize, four_pi_as=w.four_pi_as, E_cut=w.E_cut, lambda_mode=w.lambda_mode)
+    if getattr(w, "current_terms", 0):
+        kw["current_terms"] = 1
     kw.update(over or {})
     return kw
 
@@ -376,4 +378,6 @@ def configure(c, w: "Workload", n_wf: int | None = None):
         c.set_external(va, vb, w.delta_ext)
     if w.fixed:
         c.set_potentials(**w.fixed)
+    if getattr(w, "vel", None) is not None:               # external velocity fields (v_a, v_b), only with current_terms
+        c.set_velocity(*w.vel)
     return c
