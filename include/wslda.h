@@ -157,6 +157,22 @@ wslda_status wslda_densities(wslda_ctx*, const void* psi_dev, int64_t n_first, i
  * lap(alpha_sigma) spectrally.  FUNC_FIXED: no-op. */
 wslda_status wslda_update_potentials(wslda_ctx*, void* cuda_stream);
 
+/* Observables of the state whose densities are in the context (Eqs. 33a-g), computed on the device:
+ * obs_dev (device, 10 doubles) = N_a, N_b, E_kin, E_pot, E_pair, E_pot.ext, E_pair.ext, E_total, E_curr, E_vel.ext
+ * (the last two, and the -j^2/rho part of E_kin, only with current_terms).  Uses the density block as it stands --
+ * call wslda_densities(WSLDA_D_ALL) on the state first (wslda_abm_step refreshes rho and nu only) -- and the current
+ * potentials.  Sums are taken in a fixed order: bit-reproducible.  Sharded runs: the block is reduced first. */
+enum { WSLDA_OBS_N_A = 0, WSLDA_OBS_N_B, WSLDA_OBS_E_KIN, WSLDA_OBS_E_POT, WSLDA_OBS_E_PAIR, WSLDA_OBS_E_POT_EXT,
+       WSLDA_OBS_E_PAIR_EXT, WSLDA_OBS_E_TOTAL, WSLDA_OBS_E_CURR, WSLDA_OBS_E_VEL_EXT, WSLDA_OBS_COUNT };
+wslda_status wslda_energy(wslda_ctx*, double* obs_dev, void* cuda_stream);
+/* The stability check of the time-dependent codes: computes the observables (into obs_dev,
+ * nullable) and compares them ON THE DEVICE with ref_dev (10 doubles from an earlier wslda_energy): if
+ * |N_sigma - N_ref| > tol_number N_ref or |E_total - E_ref| > tol_energy |E_ref| (or E is NaN) the context is
+ * poisoned -- the verdict travels to the host behind the check, and from the first call that sees it every call
+ * returns WSLDA_ESTATE ("conservation violated"), the library's form of "terminate the run".  No host sync. */
+wslda_status wslda_watchdog(wslda_ctx*, const double* ref_dev, double tol_number, double tol_energy, double* obs_dev,
+                            void* cuda_stream);
+
 /* History length m = max(ab_order, am_order-1). */
 int wslda_history_length(const wslda_ctx*);
 /* Fill the ABM history for phi (device, [n_wf][2][M], in/out).  f_hist: HOST array of m DEVICE buffers of the

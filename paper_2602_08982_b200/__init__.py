@@ -67,7 +67,9 @@ SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "ws
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
-           "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning", "wslda_set_external_velocity"]
+           "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning", "wslda_set_external_velocity",
+           "wslda_energy", "wslda_watchdog"]
+OBS = ["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total", "E_curr", "E_vel_ext"]
 REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 _lib = None
@@ -102,6 +104,8 @@ def lib():
         L.wslda_set_reduce_hook.argtypes = [C.c_void_p, REDUCE_HOOK, C.c_void_p]
         L.wslda_set_tuning.argtypes = [C.c_void_p]
         L.wslda_set_external_velocity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_watchdog.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
         L.wslda_profile_report.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.wslda_launch_count.restype = C.c_int64
@@ -279,6 +283,23 @@ class Context:
         self._spinors(psi, "densities psi")
         self._chk(lib().wslda_densities(self.ctx, self._ptr(psi), n_first, n_count, which, accumulate, self._stream()),
                   "densities")
+
+    def energy(self, out=None):
+        """Observables of Eqs. 33a-g as a float64 CUDA tensor of 10 (order: OBS); no host synchronisation."""
+        t = self.torch
+        if out is None:
+            out = t.empty(len(OBS), dtype=t.float64, device="cuda")
+        self._chk(lib().wslda_energy(self.ctx, self._ptr(out), self._stream()), "energy")
+        return out
+
+    def watchdog(self, ref, tol_number, tol_energy, out=None):
+        """Device-side conservation check against `ref` (a tensor from energy()); a violation poisons the context."""
+        t = self.torch
+        if out is None:
+            out = t.empty(len(OBS), dtype=t.float64, device="cuda")
+        self._chk(lib().wslda_watchdog(self.ctx, self._ptr(ref), float(tol_number), float(tol_energy), self._ptr(out),
+                                       self._stream()), "watchdog")
+        return out
 
     def update_potentials(self):
         self._chk(lib().wslda_update_potentials(self.ctx, self._stream()), "update_potentials")

@@ -36,7 +36,7 @@ struct Plan {
   size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes, f6_partn_bytes;
   int mega, gs, mG, sep;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
-  size_t off_cur;
+  size_t off_cur, off_obs;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -95,6 +95,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_perwf = o; o += 7 * align_up((size_t)n_wf * 8);
   P.off_fields = o; o += align_up((size_t)DP_COUNT * M * 8) + 12 * align_up((size_t)M * 8) + 2 * align_up((size_t)M * 16);
   P.off_cur = o; if (f->current_terms) o += 3 * align_up((size_t)6 * M * 8);      // A_sigma, v_ext_sigma, W_sigma = A - v: [2][3][M] each
+  P.off_obs = o; o += align_up(((size_t)((M + 255) / 256) + 2) * WS_NOBS * 8 + 64);
   P.off_part = o; o += 2 * align_up((size_t)cn * P.nblk * 8);
   P.off_dpart = o; o += align_up((size_t)P.dG * DP_COUNT * M * 8);
   P.scr_bytes = align_up((size_t)cn * 2 * M * 16);
@@ -187,7 +188,9 @@ struct wslda_ctx {
   int t3, t3_gs, t3_r, t3_ring, t3_lag, t3_grid;    // 32^3 Eq. 40: warp-specialised TMA-fed stage kernel (mega3t.cuh): spinors per group, per heavy super-item
   T3Maps t3_maps;                  // tensor maps of the arrays the library owns (QL ring, alpha); psi is encoded per launch
   int spin_limit;                  // bound of the device-side dependency waits (polls of 200 ns)
-  int* err_host;                   // pinned: error word of the last persistent launch (copied back asynchronously)
+  int* err_host;                   // pinned: [0] error word of the last persistent launch, [1] watchdog verdict (copied back asynchronously)
+  int* wd_flag;                    // device: watchdog verdict
+  double* obs_part; double* obs_out;   // observables: per-block partial sums, result
   int sticky;                      // a launch could not be made or a device-side wait timed out: every later call fails
   double *f_part[4], *f_partn[4], *f_acc[4];
   int* f_cnt[4];                   // per-spinor arrival counters of k_f3_combine (self-resetting)
@@ -219,7 +222,11 @@ static wslda_status cuda_check(wslda_ctx* c, const char* where) {
     c->sticky = 1;
     snprintf(c->err, 256, "a device-side dependency wait timed out in a persistent stage kernel: results since then are invalid");
   }
-  if (c && c->sticky) return WSLDA_ECUDA;
+  if (c && c->err_host && c->err_host[1] && !c->sticky) {
+    c->sticky = 2;
+    snprintf(c->err, 256, "conservation violated: particle number or total energy left the tolerance given to wslda_watchdog");
+  }
+  if (c && c->sticky) return c->sticky == 2 ? WSLDA_ESTATE : WSLDA_ECUDA;
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) return WSLDA_OK;
   snprintf(c ? c->err : g_err, 256, "CUDA error at %s: %s", where, cudaGetErrorString(e));
@@ -287,8 +294,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   c->spin_limit = 1 << 25;           // ~7 s of polling: far beyond any step, short enough to report a stall
   if (g_tune.spin_limit > 0) c->spin_limit = g_tune.spin_limit;
   cudaMemcpyToSymbol(g_f3_spin_limit, &c->spin_limit, sizeof(int));
-  cudaHostAlloc((void**)&c->err_host, sizeof(int), cudaHostAllocDefault);
-  if (c->err_host) *c->err_host = 0;
+  cudaHostAlloc((void**)&c->err_host, 2 * sizeof(int), cudaHostAllocDefault);
+  if (c->err_host) c->err_host[0] = c->err_host[1] = 0;
   c->dV = 1.0; c->Lperp = 1.0;
   for (int d = 0; d < 3; ++d) {
     c->dx[d] = dx[d];
@@ -342,6 +349,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->cur_A = (double*)(base + P.off_cur); c->cur_v = c->cur_A + 6 * M; c->cur_W = c->cur_v + 6 * M;
     cudaMemset(c->cur_A, 0, (size_t)18 * M * 8);
   }
+  c->obs_part = (double*)(base + P.off_obs); c->obs_out = c->obs_part + ((M + 255) / 256) * WS_NOBS;
+  c->wd_flag = (int*)(c->obs_out + WS_NOBS);
   c->part_n = (double*)(base + P.off_part);
   c->part_e = (double*)(base + P.off_part + align_up((size_t)P.chunk_n * P.nblk * 8));
   c->dpart = (double*)(base + P.off_dpart);

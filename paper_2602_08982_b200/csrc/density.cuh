@@ -207,3 +207,78 @@ __global__ void k_get_density(const double* raw, int64_t M, int sym, int field_i
     }
   }
 }
+
+// ---- observables (Eqs. 33a-g): particle numbers and the energy terms from the current density block
+// and potentials.  One thread per lattice point, fixed-order block sums -> epart[block][WS_NOBS]; k_energy_final adds the
+// blocks in index order (bit-reproducible) and, given a reference, runs the conservation check of the time-dependent
+// codes: |N_sigma - N_ref| <= tol_n N_ref and |E - E_ref| <= tol_e |E_ref|, else *flag = 1.
+#define WS_NOBS 10      // N_a N_b E_kin E_pot E_pair E_pot_ext E_pair_ext E_total E_curr E_vel_ext
+struct ObsArgs {
+  FuncParams P;
+  const double *raw, *alpha_a, *alpha_b, *vext_a, *vext_b, *cur_v;
+  const cplx *delta, *dext;
+  double dVf;           // dV * L_perp
+  int64_t M;
+};
+__global__ void __launch_bounds__(256) k_energy(ObsArgs a, double* epart) {
+  __shared__ double sh[32];
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, M = a.M;
+  double v[WS_NOBS];
+#pragma unroll
+  for (int q = 0; q < WS_NOBS; ++q) v[q] = 0.0;
+  if (i < M) {
+    const double PI = 3.14159265358979323846;
+    double ra, rb, ta, tb; cplx nu;
+    folded(a.raw, M, i, a.P.spin_symmetric, ra, rb, ta, tb, nu);
+    const double aa = a.alpha_a[i], ab = a.alpha_b[i];
+    v[0] = ra; v[1] = rb;
+    v[2] = 0.5 * (aa * ta + ab * tb);                                                      // 33a
+    if (a.P.func_id == WSLDA_FUNC_ASLDA) {
+      double rho = ra + rb; if (rho < a.P.rho_floor) rho = a.P.rho_floor;
+      double p = (ra - rb) / rho; p = fmin(1.0, fmax(-1.0, p));
+      const double sp = 0.5 * (1.0 + p), sm = 0.5 * (1.0 - p);
+      const double B = cbrt(4.0) * (0.357 + 0.642 * p * p - aa * sp * cbrt(sp * sp) - ab * sm * cbrt(sm * sm));
+      const double x = cbrt(3.0 * PI * PI * rho);
+      v[3] = 0.6 * B * rho * 0.5 * x * x;                                                  // 33b
+    }
+    const cplx D = a.delta[i], De = a.dext[i];
+    v[4] = -(D.x * nu.x + D.y * nu.y);                                                     // 33c: -Re(conj(Delta) nu)
+    v[5] = a.vext_a[i] * ra + a.vext_b[i] * rb;                                            // 33e
+    v[6] = -2.0 * (De.x * nu.x + De.y * nu.y);                                             // 33f: -(Delta_ext nu^* + h.c.)
+    if (a.P.current_terms) {
+      double ja2 = 0.0, jb2 = 0.0, vj = 0.0;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double x = a.raw[(DP_JA0 + d) * M + i], y = a.raw[(DP_JB0 + d) * M + i];
+        const double ja = a.P.spin_symmetric ? x + y : x, jb = a.P.spin_symmetric ? x + y : y;
+        ja2 += ja * ja; jb2 += jb * jb;
+        vj += a.cur_v[d * M + i] * ja + a.cur_v[(3 + d) * M + i] * jb;
+      }
+      const double rsa = ra < a.P.rho_floor ? a.P.rho_floor : ra, rsb = rb < a.P.rho_floor ? a.P.rho_floor : rb;
+      v[2] -= 0.5 * (aa * ja2 / rsa + ab * jb2 / rsb);                                     // 33a, the -j^2/rho part
+      v[8] = 0.5 * (ja2 / rsa + jb2 / rsb);                                                // 33d
+      v[9] = -vj;                                                                          // 33g
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < WS_NOBS; ++q) {
+    if (q == 7) continue;
+    const double r = block_sum(v[q], sh);
+    if (threadIdx.x == 0) epart[(int64_t)blockIdx.x * WS_NOBS + q] = r * a.dVf;
+  }
+}
+__global__ void k_energy_final(const double* epart, int nblk, double* out, const double* ref, double tol_n, double tol_e, int* flag) {
+  if (threadIdx.x || blockIdx.x) return;
+  double s[WS_NOBS];
+  for (int q = 0; q < WS_NOBS; ++q) s[q] = 0.0;
+  for (int b = 0; b < nblk; ++b)
+    for (int q = 0; q < WS_NOBS; ++q) if (q != 7) s[q] += epart[(int64_t)b * WS_NOBS + q];
+  s[7] = s[2] + s[3] + s[4] + s[5] + s[6] + s[8] + s[9];
+  for (int q = 0; q < WS_NOBS; ++q) out[q] = s[q];
+  if (ref && flag) {
+    bool bad = !(s[7] == s[7]);                                                            // NaN
+    for (int q = 0; q < 2; ++q) bad = bad || fabs(s[q] - ref[q]) > tol_n * fabs(ref[q]);
+    bad = bad || fabs(s[7] - ref[7]) > tol_e * fabs(ref[7]);
+    if (bad) *flag = 1;
+  }
+}

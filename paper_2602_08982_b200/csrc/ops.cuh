@@ -333,6 +333,37 @@ static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
   if (c->f.kin_form == WSLDA_KIN_SYM40 && c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1) update_lap_alpha(c, st);
 }
 
+// observables from the density block as it stands (Eqs. 33a-g); ref != null adds the device-side conservation check
+static wslda_status observables(wslda_ctx* c, double* obs_dev, const double* ref_dev, double tol_n, double tol_e, cudaStream_t st,
+                                const char* where) {
+  const int64_t M = c->P.M;
+  if (c->reduce_hook && c->raw_local) reduce_densities(c, st);
+  ObsArgs a;
+  a.P.func_id = c->f.func_id; a.P.force_a1 = c->f.force_a1; a.P.spin_symmetric = c->f.spin_symmetric;
+  a.P.current_terms = c->f.current_terms; a.P.four_pi_as = c->f.four_pi_as; a.P.C = c->f.C; a.P.E_cut = c->f.E_cut;
+  a.P.rho_floor = c->f.rho_floor; a.P.mu_a = c->mu_a; a.P.mu_b = c->mu_b;
+  a.raw = c->raw; a.alpha_a = c->alpha_a; a.alpha_b = c->alpha_b; a.vext_a = c->vext_a; a.vext_b = c->vext_b;
+  a.cur_v = c->cur_v; a.delta = c->delta; a.dext = c->dext; a.dVf = c->dV * c->Lperp; a.M = M;
+  const int nblk = (int)((M + 255) / 256);
+  LAUNCH(c, k_energy, nblk, 256, 0, st, a, c->obs_part);
+  LAUNCH(c, k_energy_final, 1, 32, 0, st, c->obs_part, nblk, c->obs_out, ref_dev, tol_n, tol_e, ref_dev ? c->wd_flag : (int*)nullptr);
+  if (obs_dev) cudaMemcpyAsync(obs_dev, c->obs_out, WS_NOBS * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (ref_dev && c->err_host) cudaMemcpyAsync(c->err_host + 1, c->wd_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  return cuda_check(c, where);
+}
+
+extern "C" wslda_status wslda_energy(wslda_ctx* c, double* obs_dev, void* stream) {
+  if (!c || !obs_dev) return fail(c, WSLDA_EINVAL, "energy: null argument");
+  return observables(c, obs_dev, nullptr, 0.0, 0.0, S(stream), "energy");
+}
+
+extern "C" wslda_status wslda_watchdog(wslda_ctx* c, const double* ref_dev, double tol_number, double tol_energy, double* obs_dev,
+                                       void* stream) {
+  if (!c || !ref_dev) return fail(c, WSLDA_EINVAL, "watchdog: null argument");
+  if (!(tol_number >= 0) || !(tol_energy >= 0)) return fail(c, WSLDA_EINVAL, "watchdog: tolerances must be >= 0");
+  return observables(c, obs_dev, ref_dev, tol_number, tol_energy, S(stream), "watchdog");
+}
+
 extern "C" wslda_status wslda_update_potentials(wslda_ctx* c, void* stream) {
   if (!c) return WSLDA_EINVAL;
   potentials(c, S(stream), false);

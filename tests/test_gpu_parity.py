@@ -716,3 +716,64 @@ def test_current_coupling_selfconsistent_steps(case):
             ref = o.get_field(f)
             assert np.abs(ref).max() > 0
             assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f
+
+
+# ---- NEXT-4: on-device observables (Eqs. 33a-g) and the conservation watchdog -----
+OBS_ORACLE = ["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total", "E_curr", "E_vel_ext"]
+
+
+@pytest.mark.parametrize("case", ["cfg4_32", "cfg3_q2d", "polarised_currents", "bdg_8", "cfg4_64"])
+def test_energy_matches_oracle(case):
+    import torch
+    if case == "cfg4_32":
+        w = wl.cfg4(n_side=32, n_wf=9, kin_form=1, n_steps=1)
+    elif case == "cfg4_64":
+        w = wl.cfg4(n_side=64, n_wf=3, kin_form=1, n_steps=1)
+    elif case == "cfg3_q2d":
+        w = wl.cfg3(n_side=16, n_kz=3, nz=8, n_steps=1)             # multiplicities 1, 2, 2; Delta_ext; L_perp != 1
+    elif case == "bdg_8":
+        w = wl.cfg4(n_side=8, n_wf=20, kin_form=0, n_steps=1); w.func_id, w.four_pi_as = 1, -3.0
+    else:
+        w = wl.cfg4(n_side=8, n_wf=24, kin_form=1, n_steps=1)
+        w.spin_symmetric = 0; w.w_a = 0.6 * np.asarray(w.w_b)
+        w = _with_currents(w, 431, amp=0.05)
+    psi0 = w.spinors()
+    o, g = make_oracle(w), make_gpu(w)
+    o.densities(psi0); o.update_potentials()
+    g.densities(to_gpu(psi0)); g.update_potentials()
+    ref = o.energy()
+    got = to_np(g.energy())
+    scale = max(abs(ref[k]) for k in OBS_ORACLE[2:])
+    for i, k in enumerate(OBS_ORACLE):
+        assert abs(got[i] - ref[k]) <= 1e-11 * (abs(ref[k]) if i < 2 else scale), (k, got[i], ref[k])
+    assert np.array_equal(got, to_np(g.energy()))                   # fixed summation order
+    assert abs(ref["E_kin"]) > 0 and abs(ref["E_pair"]) > 0
+
+
+def test_watchdog_passes_a_conserving_run_and_stops_a_violating_one():
+    """The conservation check of the time-dependent codes on the device: a self-consistent BdG run within tolerance
+    passes silently; the same check with an impossible tolerance poisons the context (every later call WSLDA_ESTATE)."""
+    import torch
+    w = wl.cfg4(n_side=8, n_wf=32, kin_form=0, n_steps=1)
+    w.func_id, w.four_pi_as, w.lambda_mode = 1, -3.0, 1
+    psi0 = w.spinors()
+    g = make_gpu(w)
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 1)
+    g.densities(phi); g.update_potentials()
+    ref = g.energy()
+    for _ in range(5):
+        hist = g.abm_step(phi, hist, w.dt)
+    g.densities(phi); g.update_potentials()
+    now = g.watchdog(ref, 1e-6, 1e-3)
+    torch.cuda.synchronize()
+    g.get_field("rho_a")                                            # still alive
+    r, n = to_np(ref), to_np(now)
+    assert abs(n[0] - r[0]) < 1e-8 * abs(r[0]) and abs(n[7] - r[7]) < 1e-3 * abs(r[7]) and n[7] != r[7]
+    g.watchdog(ref, 1e-6, 1e-16)                                    # nobody conserves energy to 1e-16 over 5 steps
+    torch.cuda.synchronize()
+    with pytest.raises(ws.WsldaError, match="conservation"):
+        g.get_field("rho_a")
+    with pytest.raises(ws.WsldaError):
+        g.abm_step(phi, hist, w.dt)
