@@ -239,7 +239,9 @@ def run_gpu(args):
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md 6.65 TB/s)"
-    fp64_peak = 35.2e12            # measured DFMA-chain rate on this pool's B200 (148 SMs x 64 lanes x 2 x 1.965 GHz = 37.2 nominal)
+    fp64_peak, n_sm = ws.fp64_probe()          # measured now, on this device: dependent-chain DFMA kernel (wslda_fp64_probe)
+    fp64_src = (f"measured in this run: DFMA-chain probe {fp64_peak / 1e12:.2f} TFLOP/s on {n_sm} SMs "
+                f"(nominal {n_sm} x 64 lanes x 2 x 1.965 GHz = {n_sm * 64 * 2 * 1.965e9 / 1e12:.1f})")
 
     # ---- resident state: every rank holds its own replica of the workload ("replicas only")
     g = make_gpu(w)
@@ -296,15 +298,9 @@ def run_gpu(args):
     else:
         ach = top_flops / (top_ms * 1e-3) / 1e12
         roof = {"kernel": top, "bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                "frac": ach / (fp64_peak / 1e12), "traffic": None,
-                "peak_source": "measured FP64 DFMA chain on this pool's B200 (DESIGN.md 7)"}
-    try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "r01_mega_traffic.json.txt")))
-        if top in tr["dram_bytes_per_spinor"]:
-            roof["traffic"] = tr["dram_bytes_per_spinor"][top] * w.n_wf * (top_cnt / prof_steps)
-            roof["traffic_source"] = tr["source"] + ", per-spinor DRAM bytes x n_wf"
-    except (OSError, ValueError, KeyError):
-        pass
+                "frac": ach / (fp64_peak / 1e12), "traffic": None, "peak_source": fp64_src}
+    # `traffic` (DRAM bytes per launch) is an ncu figure and is not measured by this run: see profiles/ for the captures
+    roof["traffic_note"] = "not measured in a bench run; ncu --set full captures of this kernel are summarised under profiles/"
     roof.update({"share_of_step": top_share / tot_ms, "launches_per_step": top_cnt / prof_steps,
                  "avg_launch_ms": top_ms / top_cnt, "alg_bytes_per_launch": top_bytes / top_cnt,
                  "alg_flops_per_launch": top_flops / top_cnt})
@@ -313,7 +309,8 @@ def run_gpu(args):
     step_roof = {"bound": "hbm" if B / (hbm_peak * 1e9) >= F / fp64_peak else "alu",
                  "t_roof_us_per_spinor_step": t_roof * 1e6, "t_measured_us_per_spinor_step": 1e6 * world / value,
                  "frac": t_roof * value / world, "bytes_per_spinor_step": B, "flops_per_spinor_step": F,
-                 "hbm_gbs_achieved": B * value / world / 1e9, "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak / 1e12}
+                 "hbm_gbs_achieved": B * value / world / 1e9, "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak / 1e12,
+                 "fp64_peak_source": fp64_src}
     kernels = {k: {"launches_per_step": v[0] / prof_steps, "ms_per_step": round(v[1] / prof_steps, 4),
                    "attributed_ms_per_step": round(v[4] / prof_steps, 4), "share": round(v[4] / tot_ms, 4)} for k, v in kern}
     del hist, phi
@@ -376,6 +373,83 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """configs[4] as BASELINE.json words it: resident batches of 512 / 1024 / 2048 spinors streamed over 32768
+    wavefunctions on the 64^3 lattice (R23: device-resident batches, re-used; no host traffic in the timed path), with
+    H psi, the accumulation of ALL density fields (rho, nu, tau, j; accumulate = 1 across the batches) and the ABM step
+    timed separately with CUDA events.  One JSON line per batch size."""
+    import torch
+    import paper_2602_08982_b200 as ws
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sweep needs a CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    ws.build()
+    total = args.sweep_total
+    fp64_peak, n_sm = ws.fp64_probe()
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    for batch in [int(b) for b in args.sweep_batches.split(",")]:
+        w, desc = make_workload("cfg5", batch)
+        g = make_gpu(w)
+        shape = (batch, 2) + w.shape
+        phi = torch.empty(shape, dtype=torch.complex128, device="cuda")
+        wl.spinors_device(w, 0, batch, phi)
+        hpsi = torch.empty_like(phi)
+        eps = torch.zeros(batch, dtype=torch.float64, device="cuda")
+        hist = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(g.m)]
+        hist = g.abm_init(phi, hist, w.dt, 0)
+        nb = max(1, total // batch)
+        ev = lambda: torch.cuda.Event(enable_timing=True)
+        for _ in range(2):                                     # warm-up of every piece
+            g.apply_h(phi, hpsi, eps); g.densities(phi); hist = g.abm_step(phi, hist, w.dt)
+        torch.cuda.synchronize()
+        t = {"h_psi": 0.0, "densities_all": 0.0, "abm_step": 0.0}
+        l0 = g.launch_count()
+        sampler = ClockSampler(torch.cuda.current_device())
+        for b in range(nb):
+            for key, fn in (("h_psi", lambda: g.apply_h(phi, hpsi, eps)),
+                            ("densities_all", lambda: g.densities(phi, accumulate=1 if b else 0)),
+                            ("abm_step", lambda: g.abm_step(phi, hist, w.dt))):
+                e0, e1 = ev(), ev()
+                e0.record()
+                r = fn()
+                e1.record()
+                e1.synchronize()
+                t[key] += e0.elapsed_time(e1)
+                if key == "abm_step":
+                    hist = r
+        clocks = sampler.stop()
+        launches = g.launch_count() - l0
+        n_done = nb * batch
+        M = w.M
+        per = {k: v * 1e3 / n_done for k, v in t.items()}      # us per spinor
+        lg = math.log2(M)
+        # algorithmic work per spinor (DESIGN.md 7): H psi reads + writes a spinor, 8 transforms (Eq. 40, w and alpha w,
+        # two components, forward + inverse); densities read a spinor, 2 forward + 6 inverse transforms for the gradients
+        alg = {"h_psi": (64.0 * M, 8 * 5.0 * M * lg), "densities_all": (32.0 * M, 8 * 5.0 * M * lg),
+               "abm_step": (alg_bytes_per_spinor_step(w), alg_flops_per_spinor_step(w))}
+        roof = {k: max(by / (hbm_peak * 1e9), fl / fp64_peak) * 1e6 for k, (by, fl) in alg.items()}
+        out = {"metric": METRIC, "value": n_done / (t["abm_step"] * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": nb, "warmup": 2,
+               "ms_per_step": t["abm_step"] / nb, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "c128", "data": "synthetic",
+               "config": {"workload": desc + f"; sweep: resident batch {batch}, {nb} batches = {n_done} wavefunctions",
+                          "resident_batch": batch, "wavefunctions": n_done, "M": M, "kin_form": w.kin_form,
+                          "l2": "inputs larger than L2 (no flush)"},
+               "pieces_us_per_spinor": per,
+               "pieces_spinors_per_s": {k: 1e6 / v for k, v in per.items()},
+               "pieces_roofline_frac": {k: roof[k] / per[k] for k in per},
+               "pieces_alg_bytes_flops_per_spinor": {k: list(v) for k, v in alg.items()},
+               "peaks": {"hbm_gbs": hbm_peak, "fp64_tflops": fp64_peak / 1e12},
+               "clocks": clocks, "gpu_launches": launches}
+        print(json.dumps(out), flush=True)
+        del g, phi, hpsi, hist
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -388,9 +462,15 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="configs[4]: resident batches streamed over --sweep-total wavefunctions, pieces timed separately")
+    ap.add_argument("--sweep-batches", default="512,1024,2048")
+    ap.add_argument("--sweep-total", type=int, default=32768)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     run_gpu(args)
 
 

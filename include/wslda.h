@@ -214,6 +214,11 @@ wslda_status wslda_set_reduce_hook(wslda_ctx*, wslda_reduce_hook hook, void* use
  * of kernels, -1 on bad arguments. */
 wslda_status wslda_profile(wslda_ctx*, int enable);
 int wslda_profile_report(wslda_ctx*, char* buf, size_t buf_bytes);
+/* Measures the FP64 FMA rate of the current device for the bench's roofline denominator: a kernel of dependent DFMA
+ * chains (8 per thread, 2048 threads per SM), best of five timed launches with CUDA events, 2 flops per DFMA.
+ * Needs no context; allocates and frees 8 bytes of device memory; synchronises.  flops_per_s: host.  sm_count: host,
+ * nullable. */
+wslda_status wslda_fp64_probe(double* flops_per_s, double* sm_count);
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 int64_t wslda_launch_count(const wslda_ctx*);
 const char* wslda_last_error(const wslda_ctx*);

@@ -44,6 +44,15 @@ class Tuning(C.Structure):
                 ("tma_ring", C.c_int), ("tma_lag", C.c_int)]
 
 
+def fp64_probe():
+    """Measured FP64 FMA rate of the current device in flop/s (wslda_fp64_probe) and its SM count."""
+    f, n = C.c_double(), C.c_double()
+    rc = lib().wslda_fp64_probe(C.byref(f), C.byref(n))
+    if rc:
+        raise WsldaError(f"fp64_probe failed ({rc}): {lib().wslda_last_error(None).decode()}")
+    return f.value, int(n.value)
+
+
 def set_tuning(**kw):
     """Process-wide kernel selection / tile sizes for contexts created afterwards (wslda_set_tuning); no arguments
     restores the defaults."""
@@ -68,7 +77,7 @@ SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "ws
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
            "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning", "wslda_set_external_velocity",
-           "wslda_energy", "wslda_watchdog"]
+           "wslda_energy", "wslda_watchdog", "wslda_fp64_probe"]
 OBS = ["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total", "E_curr", "E_vel_ext"]
 REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
@@ -104,6 +113,7 @@ def lib():
         L.wslda_set_reduce_hook.argtypes = [C.c_void_p, REDUCE_HOOK, C.c_void_p]
         L.wslda_set_tuning.argtypes = [C.c_void_p]
         L.wslda_set_external_velocity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.wslda_fp64_probe.argtypes = [C.c_void_p, C.c_void_p]
         L.wslda_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_watchdog.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]

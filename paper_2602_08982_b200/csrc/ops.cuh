@@ -275,6 +275,35 @@ static void dens_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_
   else LAUNCH(c, k_density_reduce, dim3(nb(M, 256), DP_COUNT), 256, 0, st, c->dpart, (int)G, c->raw, M, mask, accumulate);
 }
 
+// tau and j of spinors [n_first, n_first + n_count) on a cubic 32^3 / 64^3 lattice, axis by axis (gdens.cuh)
+static bool gdens_ok(const wslda_ctx* c) {
+  const Plan& P = c->P;
+  return P.nd == 3 && P.N[0] == P.N[1] && P.N[1] == P.N[2] && (P.N[0] == 32 || P.N[0] == 64) && !g_tune.disable_axis_split;
+}
+static void gdens(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_count, unsigned mask, int accumulate, cudaStream_t st) {
+  const Plan& P = c->P;
+  const int N = P.N[0];
+  const int64_t M = P.M;
+  GdArgs a;
+  a.psi = psi + 2 * n_first * M; a.cpref = c->cpref + n_first; a.w_a = c->w_a + n_first; a.w_b = c->w_b + n_first;
+  const double PI = 3.14159265358979323846264338327950288;
+  for (int d = 0; d < 3; ++d) {
+    const double len = N * c->dx[d];
+    for (int j = 0; j < 64; ++j) a.kd[d][j] = (j >= N || j == N / 2) ? 0.0 : (j < N / 2 ? 2.0 * PI * j / len : 2.0 * PI * (j - N) / len);
+  }
+  a.part = c->dpart; a.n = (int)n_count;
+  int G = P.dG;                                          // the partial planes share the general path's buffer: G x 12 planes
+  if (G > n_count) G = (int)n_count;
+  if (G < 1) G = 1;
+  a.G = G;
+  const int tiles = N * N / (N == 32 ? 128 : 64);
+  const double lines = 3.0 * 2.0 * (double)N * N * (double)n_count;
+  WORK(c, 32.0 * M * n_count, lines * 2.0 * 5.0 * N * P.lg[0]);
+  if (N == 32) LAUNCHN(c, "k_gdens", k_gdens<32>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
+  else LAUNCHN(c, "k_gdens", k_gdens<64>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
+  LAUNCH(c, k_gdens_reduce, nb(M, 256), 256, 0, st, c->dpart, G, M, c->raw, mask, accumulate);
+}
+
 extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t n_first, int64_t n_count, unsigned mask,
                                         int accumulate, void* stream) {
   if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
@@ -286,8 +315,15 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
   if (n_count == 0 && !accumulate) {
     LAUNCH(c, k_density_reduce, dim3(nb(c->P.M, 256), DP_COUNT), 256, 0, st, c->dpart, 0, c->raw, c->P.M, mask, 0);
   }
-  for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += c->P.chunk_n) {
-    const int64_t cnt = (n_first + n_count - n0 < c->P.chunk_n) ? n_first + n_count - n0 : c->P.chunk_n;
+  if (n_count > 0 && (mask & (WSLDA_D_TAU | WSLDA_D_J)) && gdens_ok(c)) {     // cubic 32^3 / 64^3: gradients axis by axis
+    gdens(c, (const cplx*)psi_, n_first, n_count, mask & (WSLDA_D_TAU | WSLDA_D_J), accumulate, st);
+    mask &= ~(WSLDA_D_TAU | WSLDA_D_J);
+    if (!mask) return cuda_check(c, "densities");
+  }
+  // without gradient fields no scratch is involved: the whole range is one "chunk" (one k_density launch)
+  const int64_t step = (mask & (WSLDA_D_TAU | WSLDA_D_J)) ? c->P.chunk_n : (n_count > 0 ? n_count : 1);
+  for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += step) {
+    const int64_t cnt = (n_first + n_count - n0 < step) ? n_first + n_count - n0 : step;
     dens_chunk(c, (const cplx*)psi_ + 2 * n0 * c->P.M, nullptr, n0, cnt, mask, (accumulate || n0 > n_first) ? 1 : 0, st);
   }
   return cuda_check(c, "densities");
@@ -362,6 +398,44 @@ extern "C" wslda_status wslda_watchdog(wslda_ctx* c, const double* ref_dev, doub
   if (!c || !ref_dev) return fail(c, WSLDA_EINVAL, "watchdog: null argument");
   if (!(tol_number >= 0) || !(tol_energy >= 0)) return fail(c, WSLDA_EINVAL, "watchdog: tolerances must be >= 0");
   return observables(c, obs_dev, ref_dev, tol_number, tol_energy, S(stream), "watchdog");
+}
+
+// ---- the FP64 denominator of the roofline: a dependent-chain DFMA probe (8 independent chains per thread, 16 warps per
+// SM scheduler's worth of threads), timed with CUDA events; reports 2 flops per DFMA ----------------------------------------
+__global__ void __launch_bounds__(256) k_fp64_probe(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0, x7 = x0 + 7.0;
+  for (int i = 0; i < iters; ++i) {
+    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  }
+  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 123.456) out[0] = s;                             // never true: keeps the chains alive
+}
+extern "C" wslda_status wslda_fp64_probe(double* flops_per_s, double* sm_count_out) {
+  if (!flops_per_s) return WSLDA_EINVAL;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+    snprintf(g_err, 256, "fp64_probe: no CUDA device"); return WSLDA_ECUDA;
+  }
+  double* d = nullptr;
+  if (cudaMalloc(&d, 8) != cudaSuccess) { snprintf(g_err, 256, "fp64_probe: cudaMalloc failed"); return WSLDA_ECUDA; }
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = sms * 8, iters = 1 << 15;
+  double best = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {                       // first repetition warms up; keep the best of the rest
+    cudaEventRecord(e0);
+    k_fp64_probe<<<blocks, 256>>>(d, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+    const double f = 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3);
+    if (rep > 0 && f > best) best = f;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  if (cudaGetLastError() != cudaSuccess) { snprintf(g_err, 256, "fp64_probe: CUDA error"); return WSLDA_ECUDA; }
+  *flops_per_s = best;
+  if (sm_count_out) *sm_count_out = (double)sms;
+  return WSLDA_OK;
 }
 
 extern "C" wslda_status wslda_update_potentials(wslda_ctx* c, void* stream) {
