@@ -28,6 +28,7 @@ struct orc_ctx {
   double *w_a, *w_b, mu_a, mu_b;
   double *rho_a, *rho_b, *tau_a, *tau_b, *ja, *jb;   /* raw (unfolded) sums; ja/jb are [3][M] */
   cplx   *nu;
+  cplx   *bp;                           /* B' of Eq. 68, raw sum like nu */
   double *alpha_a, *alpha_b, *V_a, *V_b, *U_a, *U_b, *lap_a, *lap_b, *lambda, *geff, *vext_a, *vext_b;
   cplx   *delta, *dext;
   double *Aa, *Ab;                      /* current potentials A_sigma = dE/dj_sigma, [3][M] */
@@ -159,7 +160,7 @@ int orc_create(orc_ctx** out, const orc_params* p) {
   c->kperp2 = dalloc(n); c->cpref = dalloc(n); c->w_a = dalloc(n); c->w_b = dalloc(n);
   for (int64_t i = 0; i < n; ++i) { c->cpref[i] = 1.0 / c->Lperp; c->w_a[i] = 0.0; c->w_b[i] = 1.0; }
   c->rho_a = dalloc(M); c->rho_b = dalloc(M); c->tau_a = dalloc(M); c->tau_b = dalloc(M);
-  c->ja = dalloc(3 * M); c->jb = dalloc(3 * M); c->nu = (cplx*)dalloc(2 * M);
+  c->ja = dalloc(3 * M); c->jb = dalloc(3 * M); c->nu = (cplx*)dalloc(2 * M); c->bp = (cplx*)dalloc(2 * M);
   c->alpha_a = dalloc(M); c->alpha_b = dalloc(M); c->V_a = dalloc(M); c->V_b = dalloc(M);
   c->U_a = dalloc(M); c->U_b = dalloc(M); c->lap_a = dalloc(M); c->lap_b = dalloc(M);
   c->lambda = dalloc(M); c->geff = dalloc(M); c->vext_a = dalloc(M); c->vext_b = dalloc(M);
@@ -175,7 +176,7 @@ void orc_destroy(orc_ctx* c) {
   double* v[] = {c->k[0], c->k[1], c->k[2], c->kperp2, c->cpref, c->w_a, c->w_b, c->rho_a, c->rho_b, c->tau_a,
                  c->tau_b, c->ja, c->jb, (double*)c->nu, c->alpha_a, c->alpha_b, c->V_a, c->V_b, c->U_a, c->U_b,
                  c->lap_a, c->lap_b, c->lambda, c->geff, c->vext_a, c->vext_b, (double*)c->delta, (double*)c->dext,
-                 c->Aa, c->Ab, c->vel_a, c->vel_b};
+                 c->Aa, c->Ab, c->vel_a, c->vel_b, (double*)c->bp};
   for (size_t i = 0; i < sizeof(v) / sizeof(v[0]); ++i) free(v[i]);
   free(c);
 }
@@ -253,6 +254,9 @@ int orc_get_field(orc_ctx* c, int id, double* dst) {
     case ORC_LAMBDA_C: src = c->lambda; break; case ORC_G_EFF: src = c->geff; break;
     case ORC_V_A: src = c->V_a; break; case ORC_V_B: src = c->V_b; break;
     case ORC_DELTA: memcpy(dst, c->delta, sizeof(cplx) * M); return 0;
+    case ORC_BP:
+      for (int64_t i = 0; i < M; ++i) { cplx b = (c->p.spin_symmetric ? 2.0 : 1.0) * c->bp[i]; dst[2 * i] = creal(b); dst[2 * i + 1] = cimag(b); }
+      return 0;
     default: break;
   }
   if (id >= ORC_AA_X && id <= ORC_AB_Z) src = (id <= ORC_AA_Z ? c->Aa + (id - ORC_AA_X) * M : c->Ab + (id - ORC_AB_X) * M);
@@ -378,16 +382,17 @@ int orc_densities(orc_ctx* c, const double* psi_, int64_t n_first, int64_t n_cou
   const cplx* psi = (const cplx*)psi_;
   if (!accumulate) {
     memset(c->rho_a, 0, 8 * M); memset(c->rho_b, 0, 8 * M); memset(c->tau_a, 0, 8 * M); memset(c->tau_b, 0, 8 * M);
-    memset(c->ja, 0, 24 * M); memset(c->jb, 0, 24 * M); memset(c->nu, 0, 16 * M);
+    memset(c->ja, 0, 24 * M); memset(c->jb, 0, 24 * M); memset(c->nu, 0, 16 * M); memset(c->bp, 0, 16 * M);
   }
   const int64_t CH = 64;                       /* gradients of CH spinors at a time, then sum them in n order */
   cplx* g = (cplx*)malloc(sizeof(cplx) * CH * 2 * nd * M);
+  cplx* lp = (cplx*)malloc(sizeof(cplx) * CH * 2 * M);          /* Laplacians, for B' of Eq. 68 */
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += CH) {
     int64_t nc = (n_first + n_count - n0 < CH) ? n_first + n_count - n0 : CH;
 #pragma omp parallel for schedule(static)
     for (int64_t q = 0; q < 2 * nc; ++q) {
       int64_t n = n0 + q / 2; int comp = (int)(q % 2);
-      derivs(nd, c->N, c->k, psi + (2 * n + comp) * M, NULL, g + q * nd * M);
+      derivs(nd, c->N, c->k, psi + (2 * n + comp) * M, lp + q * M, g + q * nd * M);
     }
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < M; ++i)
@@ -404,6 +409,11 @@ int orc_densities(orc_ctx* c, const double* psi_, int64_t n_first, int64_t n_cou
           c->ja[d * M + i] += -cw_a * cimag(u * conj(a));                  /* Eq. 7f */
           c->jb[d * M + i] += cw_b * cimag(v * conj(b));                   /* Eq. 7g */
         }
+        {                                                                    /* Eq. 68 (reading R29): the weights of nu; the
+                                                                                plane-wave factor turns lap into lap - k_perp^2 */
+          cplx lu = lp[(2 * s) * M + i] - c->kperp2[n] * u, lv = lp[(2 * s + 1) * M + i] - c->kperp2[n] * v;
+          c->bp[i] += -0.5 * 0.5 * c->cpref[n] * (c->w_b[n] - c->w_a[n]) * (u * conj(lv) + conj(v) * lu);
+        }
         c->rho_a[i] += cw_a * u2;                                            /* Eq. 7a */
         c->rho_b[i] += cw_b * v2;                                            /* Eq. 7b */
         c->tau_a[i] += cw_a * (gu2 + c->kperp2[n] * u2);                     /* Eq. 7c, 29c, 30c */
@@ -411,7 +421,7 @@ int orc_densities(orc_ctx* c, const double* psi_, int64_t n_first, int64_t n_cou
         c->nu[i] += 0.5 * c->cpref[n] * (c->w_b[n] - c->w_a[n]) * u * conj(v);   /* Eq. 7e */
       }
   }
-  free(g);
+  free(g); free(lp);
   return 0;
 }
 
@@ -511,6 +521,39 @@ int orc_update_potentials(orc_ctx* c) {
   }
   c->lambda_valid = 1;
   lap_of_real_field(c, c->alpha_a, c->lap_a); lap_of_real_field(c, c->alpha_b, c->lap_b);
+  if (c->p.quantum_friction) {
+    /* Eqs. 66-70: V_sigma += -(alpha_qf / rho_0) div j_sigma;
+     * Delta += Delta [beta_qf sin(theta_nu - theta_B') + i gamma_qf (N - N_req) / N_req] */
+    int nd = c->nd;
+    cplx* f = (cplx*)malloc(sizeof(cplx) * M); cplx* gr = (cplx*)malloc(sizeof(cplx) * M * nd);
+    double* dv[2] = {dalloc(M), dalloc(M)};
+    double N = 0;
+    for (int64_t i = 0; i < M; ++i) {
+      double ra, rb, ta, tb, ja[3], jb[3]; cplx nu;
+      folded(c, i, &ra, &rb, &ta, &tb, &nu, ja, jb);
+      N += (ra + rb) * c->dV * c->Lperp;
+    }
+    for (int sg = 0; sg < 2; ++sg)
+      for (int d = 0; d < nd; ++d) {
+        for (int64_t i = 0; i < M; ++i) {
+          double ra, rb, ta, tb, ja[3], jb[3]; cplx nu;
+          folded(c, i, &ra, &rb, &ta, &tb, &nu, ja, jb);
+          f[i] = sg ? jb[d] : ja[d];
+        }
+        derivs(nd, c->N, c->k, f, NULL, gr);
+        for (int64_t i = 0; i < M; ++i) dv[sg][i] += creal(gr[d * M + i]);
+      }
+    double gt = c->p.qf_gamma * (N - c->p.qf_nreq) / c->p.qf_nreq;                        /* Eq. 70 */
+    for (int64_t i = 0; i < M; ++i) {
+      double Vd_a = -c->p.qf_alpha / c->p.qf_rho0 * dv[0][i], Vd_b = -c->p.qf_alpha / c->p.qf_rho0 * dv[1][i];   /* Eq. 66 */
+      c->V_a[i] += Vd_a; c->V_b[i] += Vd_b; c->U_a[i] += Vd_a; c->U_b[i] += Vd_b;
+      double f2 = c->p.spin_symmetric ? 2.0 : 1.0;
+      cplx nu = f2 * c->nu[i], bp = f2 * c->bp[i];
+      double th_nu = atan2(cimag(nu), creal(nu)), th_b = atan2(cimag(bp), creal(bp));      /* Eqs. 69, 68 */
+      c->delta[i] += c->delta[i] * (c->p.qf_beta * sin(th_nu - th_b) + I * gt);           /* Eq. 67 */
+    }
+    free(f); free(gr); free(dv[0]); free(dv[1]);
+  }
   return 0;
 }
 

@@ -36,6 +36,9 @@ typedef struct {
   int    lambda_mode;          /* 0: Lambda_c recomputed at each potential update; 1: frozen after the first */
   double rho_floor;
   int    current_terms;        /* 1: the current / velocity coupling of Eq. 4c and the j-terms of Eqs. 9b-c */
+  int    quantum_friction;     /* 1: the dissipative potentials of Eqs. 66-70 are added at every potential update */
+  double qf_alpha, qf_beta, qf_gamma;   /* alpha_qf (Eq. 66), beta_qf, gamma_qf (Eq. 67, 70)                   */
+  double qf_rho0, qf_nreq;     /* reference density rho_0 (Eq. 66) and requested particle number N_req (Eq. 70) */
 } orc_params;
 
 /* field ids for orc_get_field / orc_set_field */
@@ -43,7 +46,8 @@ enum { ORC_RHO_A = 0, ORC_RHO_B = 1, ORC_TAU_A = 2, ORC_TAU_B = 3, ORC_NU = 4 /*
        ORC_JA_X = 5, ORC_JA_Y = 6, ORC_JA_Z = 7, ORC_JB_X = 8, ORC_JB_Y = 9, ORC_JB_Z = 10,
        ORC_ALPHA_A = 16, ORC_ALPHA_B = 17, ORC_U_A = 18, ORC_U_B = 19, ORC_DELTA = 20 /* complex */,
        ORC_LAP_ALPHA_A = 21, ORC_LAP_ALPHA_B = 22, ORC_LAMBDA_C = 23, ORC_G_EFF = 24, ORC_V_A = 25, ORC_V_B = 26,
-       ORC_AA_X = 27, ORC_AA_Y = 28, ORC_AA_Z = 29, ORC_AB_X = 30, ORC_AB_Y = 31, ORC_AB_Z = 32 /* current potentials A_sigma */ };
+       ORC_AA_X = 27, ORC_AA_Y = 28, ORC_AA_Z = 29, ORC_AB_X = 30, ORC_AB_Y = 31, ORC_AB_Z = 32 /* current potentials A_sigma */,
+       ORC_BP = 33 /* complex: the kinetic anomalous density B' of Eq. 68 */ };
 
 /* --- transforms (O1) ----------------------------------------------------------------------------------- */
 /* in-place radix-2 FFT of n = 2^p complex numbers (interleaved re,im); sign = -1 forward (Eq. 26 convention
