@@ -63,6 +63,12 @@ typedef struct {
                                 anticommutator is applied as W.grad + grad.(W .), both derivatives spectral with the
                                 Nyquist rule: exactly Hermitian.  Served by the general path (no fused kernels);
                                 wslda_abm_step then also rebuilds j at both stages.  0: h of Eq. 4c without it  */
+  int quantum_friction;      /* 1: the dissipative potentials of Eqs. 66-70 are added at every
+                                potential update: V_sigma += -(qf_alpha / qf_rho0) div j_sigma, Delta += Delta [qf_beta
+                                sin(arg nu - arg B') + i qf_gamma (N - qf_nreq) / qf_nreq].  General path; the step then
+                                rebuilds j and B' (WSLDA_D_BP) as well.  Not with FUNC_FIXED                      */
+  double qf_alpha, qf_beta, qf_gamma;   /* alpha_qf (Eq. 66; 5-10), beta_qf (Eq. 67; about 5), gamma_qf (Eq. 70; about 0.1) */
+  double qf_rho0, qf_nreq;   /* reference density rho_0 of Eq. 66, requested particle number N_req of Eq. 70 (> 0)  */
 } wslda_functional;
 
 /* field ids for wslda_get_field / wslda_set_field.  Densities are returned folded per Eq. 8 when
@@ -73,10 +79,12 @@ enum { WSLDA_F_RHO_A = 0, WSLDA_F_RHO_B = 1, WSLDA_F_TAU_A = 2, WSLDA_F_TAU_B = 
        WSLDA_F_LAP_ALPHA_A = 21, WSLDA_F_LAP_ALPHA_B = 22, WSLDA_F_LAMBDA_C = 23, WSLDA_F_G_EFF = 24,
        WSLDA_F_V_A = 25, WSLDA_F_V_B = 26,
        WSLDA_F_AA_X = 27, WSLDA_F_AA_Y = 28, WSLDA_F_AA_Z = 29, WSLDA_F_AB_X = 30, WSLDA_F_AB_Y = 31, WSLDA_F_AB_Z = 32
-       /* current potentials A_sigma (get only; zero unless current_terms and alpha != 1) */ };
+       /* current potentials A_sigma (get only; zero unless current_terms and alpha != 1) */,
+       WSLDA_F_BP = 33 /* complex, get only: the kinetic anomalous density B' of Eq. 68 */ };
 
 /* which_mask bits of wslda_densities (Eqs. 7a-g) */
-enum { WSLDA_D_RHO = 1u, WSLDA_D_NU = 2u, WSLDA_D_TAU = 4u, WSLDA_D_J = 8u, WSLDA_D_ALL = 15u };
+enum { WSLDA_D_RHO = 1u, WSLDA_D_NU = 2u, WSLDA_D_TAU = 4u, WSLDA_D_J = 8u, WSLDA_D_ALL = 15u,
+       WSLDA_D_BP = 16u /* B' = -1/2 sum [u lap v^* + v^* lap u] with the weights of nu (Eq. 68); not part of D_ALL */ };
 
 /* Optional tuning of the kernel selection and of the tile / group sizes.  Process-wide: it is read by
  * wslda_workspace_bytes and wslda_ctx_create (contexts that exist keep what they were created with), so set it

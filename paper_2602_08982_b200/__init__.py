@@ -32,7 +32,9 @@ class Functional(C.Structure):
     _fields_ = [("func_id", C.c_int), ("force_a1", C.c_int), ("spin_symmetric", C.c_int), ("kin_form", C.c_int),
                 ("ab_order", C.c_int), ("am_order", C.c_int), ("subtract_mean_energy", C.c_int), ("normalize", C.c_int),
                 ("four_pi_as", C.c_double), ("C", C.c_double), ("E_cut", C.c_double), ("lambda_mode", C.c_int),
-                ("rho_floor", C.c_double), ("current_terms", C.c_int)]
+                ("rho_floor", C.c_double), ("current_terms", C.c_int), ("quantum_friction", C.c_int),
+                ("qf_alpha", C.c_double), ("qf_beta", C.c_double), ("qf_gamma", C.c_double), ("qf_rho0", C.c_double),
+                ("qf_nreq", C.c_double)]
 
 
 class Tuning(C.Structure):
@@ -69,9 +71,9 @@ def set_tuning(**kw):
 
 FIELD = dict(rho_a=0, rho_b=1, tau_a=2, tau_b=3, nu=4, ja_x=5, ja_y=6, ja_z=7, jb_x=8, jb_y=9, jb_z=10,
              alpha_a=16, alpha_b=17, U_a=18, U_b=19, delta=20, lap_alpha_a=21, lap_alpha_b=22, lambda_c=23,
-             g_eff=24, V_a=25, V_b=26, Aa_x=27, Aa_y=28, Aa_z=29, Ab_x=30, Ab_y=31, Ab_z=32)
-_COMPLEX = {4, 20}
-D_RHO, D_NU, D_TAU, D_J, D_ALL = 1, 2, 4, 8, 15
+             g_eff=24, V_a=25, V_b=26, Aa_x=27, Aa_y=28, Aa_z=29, Ab_x=30, Ab_y=31, Ab_z=32, bp=33)
+_COMPLEX = {4, 20, 33}
+D_RHO, D_NU, D_TAU, D_J, D_ALL, D_BP = 1, 2, 4, 8, 15, 16
 SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "wslda_set_modes", "wslda_set_weights",
            "wslda_set_mu", "wslda_set_external", "wslda_set_potentials", "wslda_get_field", "wslda_set_field",
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
@@ -132,11 +134,13 @@ class WsldaError(RuntimeError):
 
 def make_functional(func_id=0, force_a1=0, spin_symmetric=0, kin_form=0, ab_order=4, am_order=5,
                     subtract_mean_energy=1, normalize=1, four_pi_as=-1.0, C_=-11.11, E_cut=None, lambda_mode=0,
-                    rho_floor=1e-14, dx0=1.0, current_terms=0):
+                    rho_floor=1e-14, dx0=1.0, current_terms=0, quantum_friction=0, qf_alpha=0.0, qf_beta=0.0, qf_gamma=0.0,
+                    qf_rho0=1.0, qf_nreq=1.0):
     if E_cut is None:
         E_cut = 3.141592653589793 ** 2 / (2 * dx0 ** 2)      # Eq. 22
     return Functional(func_id, force_a1, spin_symmetric, kin_form, ab_order, am_order, subtract_mean_energy, normalize,
-                      four_pi_as, C_, E_cut, lambda_mode, rho_floor, current_terms)
+                      four_pi_as, C_, E_cut, lambda_mode, rho_floor, current_terms, quantum_friction, qf_alpha, qf_beta,
+                      qf_gamma, qf_rho0, qf_nreq)
 
 
 def workspace_bytes(dims, mode, n_wf, functional) -> int:

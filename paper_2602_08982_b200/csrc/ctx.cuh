@@ -37,7 +37,7 @@ struct Plan {
   size_t off_f6, f6_ring_bytes, f6_part_bytes, f6_acc_bytes, f6_sync_bytes, f6_pack_bytes, f6_partn_bytes;
   int mega, gs, mG, sep;
   size_t off_mega, mega_ring_bytes, mega_part_bytes, mega_acc_bytes, mega_sync_bytes, mega_pack_bytes;
-  size_t off_cur, off_obs;
+  size_t off_cur, off_obs, off_qf;
   size_t off_tables, off_perwf, off_fields, off_part, off_dpart, off_scr, scr_bytes, total;
 };
 
@@ -58,6 +58,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   bool okpair = (f->ab_order == 3 && f->am_order == 4) || (f->ab_order == 4 && f->am_order == 4) ||
                 (f->ab_order == 4 && f->am_order == 5) || (f->ab_order == 5 && f->am_order == 5);
   if (!okpair || f->kin_form < 0 || f->kin_form > 2 || f->func_id < 0 || f->func_id > 2) return WSLDA_EINVAL;
+  if (f->quantum_friction && (f->func_id == WSLDA_FUNC_FIXED || !(f->qf_rho0 > 0) || !(f->qf_nreq > 0))) return WSLDA_EINVAL;
   P.nd = mode; P.M = 1;
   for (int d = 0; d < 3; ++d) {
     P.N[d] = d < mode ? dims[d] : 1;
@@ -97,13 +98,14 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_fields = o; o += align_up((size_t)DP_COUNT * M * 8) + 12 * align_up((size_t)M * 8) + 2 * align_up((size_t)M * 16);
   P.off_cur = o; if (f->current_terms) o += 3 * align_up((size_t)6 * M * 8);      // A_sigma, v_ext_sigma, W_sigma = A - v: [2][3][M] each
   P.off_obs = o; o += align_up(((size_t)((M + 255) / 256) + 2) * WS_NOBS * 8 + 64);
+  P.off_qf = o; if (f->quantum_friction) o += align_up((size_t)2 * M * 8);          // div j_sigma
   P.off_part = o; o += 2 * align_up((size_t)cn * P.nblk * 8);
   P.off_dpart = o; o += align_up((size_t)P.dG * DP_COUNT * M * 8);
   P.scr_bytes = align_up((size_t)cn * 2 * M * 16);
   P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
   // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
-           f->kin_form != WSLDA_KIN_DIVGRAD && !f->current_terms;
+           f->kin_form != WSLDA_KIN_DIVGRAD && !f->current_terms && !f->quantum_friction;
   if (g_tune.disable_fused3d) P.fast = 0;
   P.fc = 32; P.ns = 3;
   if (g_tune.fused_chunk > 0) P.fc = g_tune.fused_chunk;
@@ -134,7 +136,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_pack_bytes = align_up((size_t)M * 48);
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
-  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms;
+  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms && !f->quantum_friction;
   if (g_tune.disable_mega64) P.f6 = 0;
   P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = P.f6_partn_bytes = 0;
   if (P.f6) {
@@ -146,7 +148,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
-  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->current_terms;
+  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->current_terms && !f->quantum_friction;
   if (g_tune.disable_onchip) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
   { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
@@ -192,6 +194,7 @@ struct wslda_ctx {
   int* err_host;                   // pinned: [0] error word of the last persistent launch, [1] watchdog verdict (copied back asynchronously)
   int* wd_flag;                    // device: watchdog verdict
   double* obs_part; double* obs_out;   // observables: per-block partial sums, result
+  double* qf_divj;                 // quantum friction: div j_sigma, [2][M]
   int sticky;                      // a launch could not be made or a device-side wait timed out: every later call fails
   double *f_part[4], *f_partn[4], *f_acc[4];
   int* f_cnt[4];                   // per-spinor arrival counters of k_f3_combine (self-resetting)
@@ -352,6 +355,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   }
   c->obs_part = (double*)(base + P.off_obs); c->obs_out = c->obs_part + ((M + 255) / 256) * WS_NOBS;
   c->wd_flag = (int*)(c->obs_out + WS_NOBS);
+  if (f->quantum_friction) c->qf_divj = (double*)(base + P.off_qf);
   c->part_n = (double*)(base + P.off_part);
   c->part_e = (double*)(base + P.off_part + align_up((size_t)P.chunk_n * P.nblk * 8));
   c->dpart = (double*)(base + P.off_dpart);

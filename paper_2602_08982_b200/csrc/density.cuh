@@ -4,12 +4,13 @@
 #include "common.cuh"
 
 // raw density planes, each M doubles
-enum { DP_RHO_A = 0, DP_RHO_B, DP_NU_RE, DP_NU_IM, DP_TAU_A, DP_TAU_B, DP_JA0, DP_JA1, DP_JA2, DP_JB0, DP_JB1, DP_JB2, DP_COUNT };
+enum { DP_RHO_A = 0, DP_RHO_B, DP_NU_RE, DP_NU_IM, DP_TAU_A, DP_TAU_B, DP_JA0, DP_JA1, DP_JA2, DP_JB0, DP_JB1, DP_JB2, DP_BP_RE, DP_BP_IM, DP_COUNT };
 
 struct DensArgs {
   const cplx* psi;                       // chunk base
   const double *scale, *cpref, *kperp2, *w_a, *w_b;   // per spinor of the chunk (scale nullable)
   const cplx* grad[3];                   // d_j psi (already scaled), [2 n + c][M]; null when not needed
+  const cplx* lap;                       // lap psi (already scaled), same layout; for B' of Eq. 68 (mask WSLDA_D_BP)
   int nd;
   int64_t M, n_count, per_group;
   unsigned mask;                         // WSLDA_D_* bits
@@ -50,6 +51,13 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_density(DensArgs a, double* p
       acc[DP_TAU_A] += cwa * (gu2 + a.kperp2[n] * u2);                        // Eqs. 7c, 29c, 30c
       acc[DP_TAU_B] += cwb * (gv2 + a.kperp2[n] * v2);                        // Eq. 7d
     }
+    if (a.mask & WSLDA_D_BP) {                                                // Eq. 68; lap -> lap - k_perp^2 for a plane-wave factor
+      const cplx lu = a.lap[2 * n * a.M + i], lv = a.lap[(2 * n + 1) * a.M + i];
+      const cplx Lu = make_double2(lu.x - a.kperp2[n] * u.x, lu.y - a.kperp2[n] * u.y);
+      const cplx Lv = make_double2(lv.x - a.kperp2[n] * v.x, lv.y - a.kperp2[n] * v.y);
+      const cplx t = cadd(cmul(u, cconj(Lv)), cmul(cconj(v), Lu));
+      acc[DP_BP_RE] += -0.5 * wn * t.x; acc[DP_BP_IM] += -0.5 * wn * t.y;
+    }
   }
   double* p = part + (int64_t)blockIdx.y * DP_COUNT * a.M + i;
 #pragma unroll
@@ -57,7 +65,7 @@ __global__ void __launch_bounds__(WS_PT_THREADS) k_density(DensArgs a, double* p
 }
 
 __device__ __host__ inline unsigned plane_bit(int f) {
-  return (f <= DP_RHO_B) ? WSLDA_D_RHO : (f <= DP_NU_IM) ? WSLDA_D_NU : (f <= DP_TAU_B) ? WSLDA_D_TAU : WSLDA_D_J;
+  return (f <= DP_RHO_B) ? WSLDA_D_RHO : (f <= DP_NU_IM) ? WSLDA_D_NU : (f <= DP_TAU_B) ? WSLDA_D_TAU : (f <= DP_JB2) ? WSLDA_D_J : WSLDA_D_BP;
 }
 
 // raw[f][i] = (accumulate ? raw[f][i] : 0) + sum_g part[g][f][i], groups in increasing order
@@ -71,7 +79,8 @@ __global__ void k_density_reduce(const double* part, int G, double* raw, int64_t
 }
 
 struct FuncParams {
-  int func_id, force_a1, spin_symmetric, current_terms;
+  int func_id, force_a1, spin_symmetric, current_terms, quantum_friction;
+  double qf_alpha, qf_beta, qf_gamma, qf_rho0, qf_nreq;
   double four_pi_as, C, E_cut, rho_floor, mu_a, mu_b;
 };
 
@@ -199,6 +208,7 @@ __global__ void k_get_density(const double* raw, int64_t M, int sym, int field_i
     case WSLDA_F_TAU_A: dst[i] = ta; break;
     case WSLDA_F_TAU_B: dst[i] = tb; break;
     case WSLDA_F_NU: dst[2 * i] = nu.x; dst[2 * i + 1] = nu.y; break;
+    case WSLDA_F_BP: { const double f2 = sym ? 2.0 : 1.0; dst[2 * i] = f2 * raw[DP_BP_RE * M + i]; dst[2 * i + 1] = f2 * raw[DP_BP_IM * M + i]; } break;
     default: {
       const bool is_a = field_id <= WSLDA_F_JA_Z;
       const int d = is_a ? field_id - WSLDA_F_JA_X : field_id - WSLDA_F_JB_X;
@@ -281,4 +291,32 @@ __global__ void k_energy_final(const double* epart, int nblk, double* out, const
     bad = bad || fabs(s[7] - ref[7]) > tol_e * fabs(ref[7]);
     if (bad) *flag = 1;
   }
+}
+
+// ---- quantum friction (Eqs. 66-70), applied after k_potentials: divj[2][M] = div j_sigma (spectral),
+// obs = the observables of k_energy_final (N_a, N_b in obs[0], obs[1]) -----------------------------------------------------
+__global__ void k_qf(FuncParams P, const double* raw, const double* divj, const double* obs, double* V_a, double* V_b, double* U_a,
+                     double* U_b, cplx* delta, int64_t M) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const double va = -P.qf_alpha / P.qf_rho0 * divj[i], vb = -P.qf_alpha / P.qf_rho0 * divj[M + i];          // Eq. 66
+  V_a[i] += va; U_a[i] += va; V_b[i] += vb; U_b[i] += vb;
+  const double gt = P.qf_gamma * ((obs[0] + obs[1]) - P.qf_nreq) / P.qf_nreq;                                 // Eq. 70
+  const double th_nu = atan2(raw[DP_NU_IM * M + i], raw[DP_NU_RE * M + i]);                                  // Eq. 69 (the fold factor 2 has no phase)
+  const double th_b = atan2(raw[DP_BP_IM * M + i], raw[DP_BP_RE * M + i]);                                   // Eq. 68
+  const double f = P.qf_beta * sin(th_nu - th_b);
+  const cplx D = delta[i];
+  delta[i] = make_double2(D.x + D.x * f - D.y * gt, D.y + D.y * f + D.x * gt);                               // Eq. 67
+}
+// out[i] (=, +=) Re t[i] for a field derivative
+__global__ void k_real_acc(double* out, const cplx* t, int64_t M, int first) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < M) out[i] = (first ? 0.0 : out[i]) + t[i].x;
+}
+// one (folded) current component of each spin as a complex field pair, for the derivative engine
+__global__ void k_j_to_cplx(const double* raw, int d, int sym, cplx* dst, int64_t M) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const double a = raw[(DP_JA0 + d) * M + i], b = raw[(DP_JB0 + d) * M + i];
+  dst[i] = make_double2(sym ? a + b : a, 0.0); dst[M + i] = make_double2(sym ? a + b : b, 0.0);
 }

@@ -117,7 +117,8 @@ extern "C" wslda_status wslda_set_potentials(wslda_ctx* c, const double* aa, con
 static void reduce_densities(wslda_ctx* c, cudaStream_t st);
 static unsigned step_mask(const wslda_ctx* c);
 static inline unsigned dens_group_of_field(int id) {
-  return id <= WSLDA_F_RHO_B ? WSLDA_D_RHO : id <= WSLDA_F_TAU_B ? WSLDA_D_TAU : id == WSLDA_F_NU ? WSLDA_D_NU : WSLDA_D_J;
+  return id <= WSLDA_F_RHO_B ? WSLDA_D_RHO : id <= WSLDA_F_TAU_B ? WSLDA_D_TAU : id == WSLDA_F_NU ? WSLDA_D_NU
+       : id == WSLDA_F_BP ? WSLDA_D_BP : WSLDA_D_J;
 }
 
 extern "C" wslda_status wslda_set_reduce_hook(wslda_ctx* c, wslda_reduce_hook hook, void* user) {
@@ -145,8 +146,8 @@ extern "C" wslda_status wslda_get_field(wslda_ctx* c, int id, void* dst, void* s
     else { cudaMemsetAsync(dst, 0, bytes, st); return cuda_check(c, "get_field"); }
   }
   if (src) { cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st); return cuda_check(c, "get_field"); }
-  if (id < 0 || id > WSLDA_F_JB_Z) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
-  if (c->reduce_hook && (c->raw_local & (c->f.spin_symmetric ? WSLDA_D_ALL : dens_group_of_field(id)))) reduce_densities(c, st);
+  if (id < 0 || (id > WSLDA_F_JB_Z && id != WSLDA_F_BP)) return fail(c, WSLDA_EINVAL, "get_field: unknown field id");
+  if (c->reduce_hook && (c->raw_local & (c->f.spin_symmetric ? (WSLDA_D_ALL | WSLDA_D_BP) : dens_group_of_field(id)))) reduce_densities(c, st);
   LAUNCH(c, k_get_density, nb(M, 256), 256, 0, st, c->raw, M, c->f.spin_symmetric, id, (double*)dst);
   return cuda_check(c, "get_field");
 }
@@ -258,10 +259,11 @@ static void dens_chunk(wslda_ctx* c, const cplx* psi_chunk, const double* scale_
   const Plan& P = c->P;
   const int64_t M = P.M;
   DensArgs d; memset(&d, 0, sizeof d);
-  if (mask & (WSLDA_D_TAU | WSLDA_D_J)) {
+  if (mask & (WSLDA_D_TAU | WSLDA_D_J | WSLDA_D_BP)) {
     DerivArgs a; memset(&a, 0, sizeof a);
     a.src = psi_chunk; a.src_comp0 = 0; a.ncomp = (int)(2 * cnt); a.scale = scale_chunk;
-    for (int k = 0; k < P.nd; ++k) { a.out[1 + k] = c->scr[k]; d.grad[k] = c->scr[k]; }
+    if (mask & (WSLDA_D_TAU | WSLDA_D_J)) for (int k = 0; k < P.nd; ++k) { a.out[1 + k] = c->scr[k]; d.grad[k] = c->scr[k]; }
+    if (mask & WSLDA_D_BP) { a.out[0] = c->scr[5]; d.lap = c->scr[5]; }      // Laplacians for B' (Eq. 68)
     deriv(c, a, st);
   }
   int64_t G = P.dG < cnt ? P.dG : cnt;
@@ -308,7 +310,7 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
                                         int accumulate, void* stream) {
   if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
   if (n_first < 0 || n_count < 0 || n_first + n_count > c->P.n_wf) return fail(c, WSLDA_EINVAL, "densities: spinor range out of bounds");
-  if (!mask || (mask & ~WSLDA_D_ALL)) return fail(c, WSLDA_EINVAL, "densities: bad which_mask");
+  if (!mask || (mask & ~(WSLDA_D_ALL | WSLDA_D_BP))) return fail(c, WSLDA_EINVAL, "densities: bad which_mask");
   if (c->reduce_hook && accumulate && (mask & ~c->raw_local)) return fail(c, WSLDA_EINVAL, "densities: accumulate onto a block already summed over the ranks");
   c->raw_local |= mask;
   cudaStream_t st = S(stream);
@@ -321,7 +323,7 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
     if (!mask) return cuda_check(c, "densities");
   }
   // without gradient fields no scratch is involved: the whole range is one "chunk" (one k_density launch)
-  const int64_t step = (mask & (WSLDA_D_TAU | WSLDA_D_J)) ? c->P.chunk_n : (n_count > 0 ? n_count : 1);
+  const int64_t step = (mask & (WSLDA_D_TAU | WSLDA_D_J | WSLDA_D_BP)) ? c->P.chunk_n : (n_count > 0 ? n_count : 1);
   for (int64_t n0 = n_first; n0 < n_first + n_count; n0 += step) {
     const int64_t cnt = (n_first + n_count - n0 < step) ? n_first + n_count - n0 : step;
     dens_chunk(c, (const cplx*)psi_ + 2 * n0 * c->P.M, nullptr, n0, cnt, mask, (accumulate || n0 > n_first) ? 1 : 0, st);
@@ -337,18 +339,37 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
 // dirty groups are reduced as maximal contiguous runs (one hook call for rho + nu inside a step).
 static void reduce_densities(wslda_ctx* c, cudaStream_t st) {
   if (c->reduce_hook) {
-    static const unsigned grp[4] = {WSLDA_D_RHO, WSLDA_D_NU, WSLDA_D_TAU, WSLDA_D_J};
-    static const int first[5] = {DP_RHO_A, DP_NU_RE, DP_TAU_A, DP_JA0, DP_COUNT};
+    static const unsigned grp[5] = {WSLDA_D_RHO, WSLDA_D_NU, WSLDA_D_TAU, WSLDA_D_J, WSLDA_D_BP};
+    static const int first[6] = {DP_RHO_A, DP_NU_RE, DP_TAU_A, DP_JA0, DP_BP_RE, DP_COUNT};
     int g = 0;
-    while (g < 4) {
+    while (g < 5) {
       if (!(c->raw_local & grp[g])) { ++g; continue; }
       int h = g;
-      while (h + 1 < 4 && (c->raw_local & grp[h + 1])) ++h;
+      while (h + 1 < 5 && (c->raw_local & grp[h + 1])) ++h;
       c->reduce_hook(c->reduce_user, c->raw + (int64_t)first[g] * c->P.M, (int64_t)(first[h + 1] - first[g]) * c->P.M, (void*)st);
       g = h + 1;
     }
   }
   c->raw_local = 0;
+}
+
+static wslda_status observables(wslda_ctx* c, double* obs_dev, const double* ref_dev, double tol_n, double tol_e, cudaStream_t st,
+                                const char* where);
+// Eqs. 66-70 on top of the potentials just built: N from the observables kernel, div j_sigma by six
+// field derivatives (one per spin and held axis, Nyquist rule of an odd derivative), then the pointwise k_qf.
+static void quantum_friction(wslda_ctx* c, const FuncParams& fp, cudaStream_t st) {
+  const int64_t M = c->P.M;
+  observables(c, nullptr, nullptr, 0.0, 0.0, st, "quantum friction");
+  cplx* in = c->scr[5];
+  cplx* out = c->scr[6];
+  for (int d = 0; d < c->P.nd; ++d) {
+    LAUNCH(c, k_j_to_cplx, nb(M, 256), 256, 0, st, c->raw, d, c->f.spin_symmetric, in, M);
+    DerivArgs a; memset(&a, 0, sizeof a);
+    a.src = in; a.src_comp0 = 0; a.ncomp = 2; a.out[1 + d] = out;
+    deriv(c, a, st);
+    LAUNCH(c, k_real_acc, nb(2 * M, 256), 256, 0, st, c->qf_divj, out, 2 * M, d == 0 ? 1 : 0);
+  }
+  LAUNCH(c, k_qf, nb(M, 256), 256, 0, st, fp, c->raw, c->qf_divj, c->obs_out, c->V_a, c->V_b, c->U_a, c->U_b, c->delta, M);
 }
 
 // fresh: the block was just rebuilt from this rank's spinors (every call inside a step)
@@ -359,7 +380,8 @@ static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
   const int64_t M = c->P.M;
   FuncParams fp;
   fp.func_id = c->f.func_id; fp.force_a1 = c->f.force_a1; fp.spin_symmetric = c->f.spin_symmetric;
-  fp.current_terms = c->f.current_terms;
+  fp.current_terms = c->f.current_terms; fp.quantum_friction = c->f.quantum_friction;
+  fp.qf_alpha = c->f.qf_alpha; fp.qf_beta = c->f.qf_beta; fp.qf_gamma = c->f.qf_gamma; fp.qf_rho0 = c->f.qf_rho0; fp.qf_nreq = c->f.qf_nreq;
   fp.four_pi_as = c->f.four_pi_as; fp.C = c->f.C; fp.E_cut = c->f.E_cut; fp.rho_floor = c->f.rho_floor;
   fp.mu_a = c->mu_a; fp.mu_b = c->mu_b;
   const int frozen = c->f.lambda_mode == 1 && c->lambda_valid;
@@ -367,6 +389,7 @@ static void potentials(wslda_ctx* c, cudaStream_t st, bool fresh) {
          c->V_b, c->U_a, c->U_b, c->lambda, c->geff, c->delta, M, c->cur_A, c->cur_v, c->cur_W);
   c->lambda_valid = 1;
   if (c->f.kin_form == WSLDA_KIN_SYM40 && c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1) update_lap_alpha(c, st);
+  if (c->f.quantum_friction) quantum_friction(c, fp, st);
 }
 
 // observables from the density block as it stands (Eqs. 33a-g); ref != null adds the device-side conservation check

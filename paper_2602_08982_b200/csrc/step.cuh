@@ -18,6 +18,7 @@ static unsigned step_mask(const wslda_ctx* c) {
   unsigned m = WSLDA_D_RHO | WSLDA_D_NU;
   if (c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1 && !c->f.spin_symmetric) m |= WSLDA_D_TAU;
   if (c->f.current_terms && c->f.func_id == WSLDA_FUNC_ASLDA && !c->f.force_a1) m |= WSLDA_D_J;     // A_sigma follows j
+  if (c->f.quantum_friction) m |= WSLDA_D_J | WSLDA_D_BP;                                          // div j (Eq. 66), B' (Eq. 68)
   return m;
 }
 static inline int64_t chunk_len(const wslda_ctx* c, int64_t n0) {

@@ -783,3 +783,53 @@ def test_watchdog_passes_a_conserving_run_and_stops_a_violating_one():
         g.get_field("rho_a")
     with pytest.raises(ws.WsldaError):
         g.abm_step(phi, hist, w.dt)
+
+
+# ---- NEXT-3: quantum friction (Eqs. 66-70), general path --------------------------------------------
+@pytest.mark.parametrize("shape,dx", [((8, 4, 8), (1.0, 0.9, 1.1)), ((16, 8), (1.0, 1.2)), ((32,), (0.8,)), ((32, 16, 16), (1.0, 1.0, 0.9))])
+@pytest.mark.parametrize("sym", [0, 1])
+def test_kinetic_anomalous_density_matches_oracle(shape, dx, sym):
+    """B' of Eq. 68 (mask WSLDA_D_BP) on on-chip and multi-pass lattices, with transverse modes and multiplicities,
+    overwritten and accumulated over batches."""
+    n_wf = 7 if np.prod(shape) > 4096 else 19
+    w = generic(shape, dx, n_wf, 1, n_modes=3, spin_symmetric=sym)
+    psi = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    o.densities(psi)
+    dev = to_gpu(psi)
+    g.densities(dev, which=ws.D_BP | ws.D_NU)
+    assert relerr(to_np(g.get_field("bp")), o.get_field("bp")) < TOL_D
+    assert relerr(to_np(g.get_field("nu")), o.get_field("nu")) < TOL_D
+    g.densities(dev, n_first=0, n_count=3, which=ws.D_BP)
+    g.densities(dev, n_first=3, n_count=n_wf - 3, which=ws.D_BP, accumulate=1)
+    assert relerr(to_np(g.get_field("bp")), o.get_field("bp")) < TOL_D
+
+
+@pytest.mark.parametrize("case", ["bdg", "aslda_polarised", "slda_symmetric_32"])
+def test_quantum_friction_steps_match_oracle(case):
+    """Dissipative self-consistent steps: V^(d) from div j, Delta^(d) from the phases of nu and B' and from N - N_req,
+    rebuilt at both stages of Alg. 2 and in the Taylor starter."""
+    if case == "slda_symmetric_32":
+        w = wl.cfg4(n_side=32, n_wf=6, kin_form=1, n_steps=2)          # a Ny = Nz = 32 lattice: the fused kernels step aside
+        steps = 2
+    else:
+        w = wl.cfg4(n_side=8, n_wf=24, kin_form=1, n_steps=4)
+        steps = 4
+        if case == "bdg":
+            w.func_id, w.kin_form, w.four_pi_as = 1, 0, -3.0
+        else:
+            w.spin_symmetric = 0; w.w_a = 0.6 * np.asarray(w.w_b)
+    w.friction = dict(qf_alpha=6.0, qf_beta=5.0, qf_gamma=0.1, qf_rho0=0.03, qf_nreq=1.7)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, steps, selfstart=1)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("rho_a", "nu", "bp", "ja_x", "delta", "V_a", "U_b"):
+        ref = o.get_field(f)
+        assert np.abs(ref).max() > 0
+        assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f
+    w0 = wl.cfg4(n_side=8, n_wf=24, kin_form=1, n_steps=4)             # friction is not a rounding matter
+    if case == "aslda_polarised":
+        w0.spin_symmetric = 0; w0.w_a = 0.6 * np.asarray(w0.w_b)
+        o0 = make_oracle(w0); o0.densities(psi0); o0.update_potentials()
+        o1 = make_oracle(w); o1.densities(psi0); o1.update_potentials()
+        assert relerr(o1.get_field("delta"), o0.get_field("delta")) > 1e-3

@@ -360,6 +360,9 @@ def context_kwargs(w: "Workload", over=None) -> dict:
               normalize=w.normalize, four_pi_as=w.four_pi_as, E_cut=w.E_cut, lambda_mode=w.lambda_mode)
     if getattr(w, "current_terms", 0):
         kw["current_terms"] = 1
+    if getattr(w, "friction", None):                      # dict(qf_alpha=..., qf_beta=..., qf_gamma=..., qf_rho0=..., qf_nreq=...)
+        kw["quantum_friction"] = 1
+        kw.update(w.friction)
     kw.update(over or {})
     return kw
 
