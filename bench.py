@@ -315,6 +315,12 @@ def run_gpu(args):
                    "attributed_ms_per_step": round(v[4] / prof_steps, 4), "share": round(v[4] / tot_ms, 4)} for k, v in kern}
     del hist, phi
     torch.cuda.empty_cache()
+    cmp_cufft = None
+    if rank == 0 and not args.no_cufft and not args.shard:
+        try:
+            cmp_cufft = cufft_compare(w, g)
+        except RuntimeError as e:                          # out of memory for the library's temporaries: report, do not fail
+            cmp_cufft = {"error": str(e)[:200]}
 
     # ---- end to end: the same step through wslda_abm_step_host (pinned HOST buffers, copies inside the timed region)
     e2e = None
@@ -367,10 +373,63 @@ def run_gpu(args):
                           "l2": "inputs larger than L2 (no flush)" if (1 + w.history) * w.n_wf * 32 * w.M > 4e8
                                 else "working set near L2 size: numbers are L2-assisted"},
                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof,
-               "kernels": kernels, "cpu_baseline": cpu, "finite": finite}
+               "kernels": kernels, "cpu_baseline": cpu, "cufft_compare": cmp_cufft, "finite": finite}
         print(json.dumps(out))
     if world > 1 or args.shard:
         dist.destroy_process_group()
+
+
+def cufft_compare(w, g, n_cmp=256, reps=3):
+    """H psi by library transforms as an outside yardstick ("cuFFT-based H psi is timed as a second
+    comparison only"): torch.fft (cuFFT) forward / inverse 3-D transforms of w and alpha w plus the pointwise BdG mix in
+    torch ops, against wslda_apply_h on the same spinors.  Same operator (Eq. 40 / Eq. 14 per w.kin_form); fields
+    read back from the context.  Not part of the product path."""
+    import torch
+    if w.mode != 3 or w.kin_form == 2:
+        return None
+    n = min(w.n_wf, n_cmp)
+    shape = (w.n_wf, 2) + w.shape
+    psi = torch.empty(shape, dtype=torch.complex128, device="cuda")
+    wl.spinors_device(w, 0, w.n_wf, psi)
+    F = {k: g.get_field(k) for k in ("alpha_a", "alpha_b", "U_a", "U_b", "delta", "lap_alpha_a", "lap_alpha_b")}
+    ks = [torch.as_tensor(wl.kgrid(w.dims[d], w.dx[d]), device="cuda") for d in range(3)]
+    k2 = ks[0][:, None, None] ** 2 + ks[1][None, :, None] ** 2 + ks[2][None, None, :] ** 2
+    mu = w.mu
+
+    def lap(x):
+        return torch.fft.ifftn(-k2 * torch.fft.fftn(x, dim=(-3, -2, -1)), dim=(-3, -2, -1))
+
+    def hpsi(p):
+        u, v = p[:, 0], p[:, 1]
+        if w.kin_form == 1:
+            ku = -0.25 * (lap(F["alpha_a"] * u) + F["alpha_a"] * lap(u) - F["lap_alpha_a"] * u)
+            kv = -0.25 * (lap(F["alpha_b"] * v) + F["alpha_b"] * lap(v) - F["lap_alpha_b"] * v)
+        else:
+            ku, kv = -0.5 * lap(u), -0.5 * lap(v)
+        hu = ku + (F["U_a"] - mu[0]) * u + F["delta"] * v
+        hv = torch.conj(F["delta"]) * u - (kv + (F["U_b"] - mu[1]) * v)
+        return torch.stack([hu, hv], 1)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    sub = psi[:n]
+    ref = hpsi(sub)                                         # warm-up (cuFFT plans) + cross-check
+    out = torch.empty_like(psi)
+    eps = torch.zeros(w.n_wf, dtype=torch.float64, device="cuda")
+    g.apply_h(psi, out, eps, 0, n)
+    err = float((out[:n] - ref).abs().max() / ref.abs().max())
+    t = {}
+    for name, fn in (("cufft", lambda: hpsi(sub)), ("wslda", lambda: g.apply_h(psi, out, eps, 0, n))):
+        e0, e1 = ev(), ev()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record(); e1.synchronize()
+        t[name] = e0.elapsed_time(e1) / reps
+    del psi, out, ref
+    torch.cuda.empty_cache()
+    return {"what": "H psi on %d spinors: torch.fft (cuFFT) transforms + torch pointwise ops vs wslda_apply_h" % n,
+            "cufft_spinors_per_s": n / (t["cufft"] * 1e-3), "wslda_spinors_per_s": n / (t["wslda"] * 1e-3),
+            "speedup": t["cufft"] / t["wslda"], "max_rel_difference": err}
 
 
 def run_sweep(args):
@@ -462,6 +521,7 @@ def main():
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT-based H psi comparison leg")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: resident batches streamed over --sweep-total wavefunctions, pieces timed separately")
     ap.add_argument("--sweep-batches", default="512,1024,2048")
