@@ -367,7 +367,7 @@ def run_gpu(args):
                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
                "dtype": "c128", "data": "synthetic",
                "config": {"workload": desc, "name": w.name, "n_wf_per_gpu": w.n_wf, "M": w.M, "mode": w.mode,
-                          "kin_form": w.kin_form, "func_id": w.func_id, "ab_am": [w.ab_order, w.am_order], "dt": w.dt,
+                          "tuning": args.tuning or "defaults", "kin_form": w.kin_form, "func_id": w.func_id, "ab_am": [w.ab_order, w.am_order], "dt": w.dt,
                           "resident_bytes": (1 + w.history) * w.n_wf * 32 * w.M, "parallelism": (f"spinor index sharded x{world}, one NCCL all-reduce of the density block per density build"
                                           if args.shard else f"replicas x{world}"),
                           "l2": "inputs larger than L2 (no flush)" if (1 + w.history) * w.n_wf * 32 * w.M > 4e8
@@ -522,6 +522,7 @@ def main():
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT-based H psi comparison leg")
+    ap.add_argument("--tuning", default="", help="wslda_set_tuning fields, e.g. enable_tma_stage=1,tma_group=8 (kernel selection only)")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: resident batches streamed over --sweep-total wavefunctions, pieces timed separately")
     ap.add_argument("--sweep-batches", default="512,1024,2048")
@@ -529,6 +530,10 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.tuning:
+        import paper_2602_08982_b200 as ws
+        ws.build()
+        ws.set_tuning(**{k: (float(v) if "." in v else int(v)) for k, v in (kv.split("=") for kv in args.tuning.split(","))})
     if args.sweep:
         return run_sweep(args)
     run_gpu(args)
