@@ -227,6 +227,30 @@ int wslda_profile_report(wslda_ctx*, char* buf, size_t buf_bytes);
  * Needs no context; allocates and frees 8 bytes of device memory; synchronises.  flops_per_s: host.  sm_count: host,
  * nullable. */
 wslda_status wslda_fp64_probe(double* flops_per_s, double* sm_count);
+/* Allocation-free gradient densities, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops): tau_sigma = sum_n cw^sigma_n |grad w_n|^2 (Eqs. 7c-d) and
+ * j_a = -sum_n cw^a_n Im[u_n grad u_n^*], j_b = +sum_n cw^b_n Im[v_n grad v_n^*] (Eqs. 7f-g) of n_wf
+ * spinors on a cubic periodic lattice of side 32 or 64 (full 3-D; spectral first derivative of Eq. 26 with the Nyquist mode
+ * dropped).  Needs no context and no workspace: the partial planes of the axis-by-axis kernel live in a
+ * file-scope device array of wslda_static_scratch_bytes() = 24 MiB that every GPU loading the library holds until exit.
+ * No cudaMalloc / cudaFree / allocating library call is made, on the first call or later (the first call on a device looks
+ * up the array's device address and sets a kernel attribute).  ALL calls on a device share that array: two calls that may
+ * overlap on the GPU (different streams without an ordering between them, concurrent host threads) race; calls on one
+ * stream are safe.  The array keeps the last call's contents; nothing in it has to start at zero.
+ *   psi   device, complex128 [n_wf][2][n_side][n_side][n_side] (z fastest), read only
+ *   cw_a, cw_b  device, double [n_wf]: c_n w^a_n and c_n w^b_n -- the prefactor of Eqs. 29-30 (1 in full 3-D) times the
+ *         weight of Eq. 7 / Eq. 8
+ *   dx    host, 3 lattice spacings
+ *   tau   device, double [2][M] (a, b), M = n_side^3; nullable.   j: device, double [2][3][M] (a: x, y, z; b: x, y, z); nullable
+ * Asynchronous on `stream`; outputs are overwritten (no accumulate).  Sums run over n in increasing order inside
+ * min(n_wf, 8 | 1) groups (32^3 | 64^3) added in index order: bit-reproducible.  Errors (message through
+ * wslda_last_error(NULL)): WSLDA_EINVAL for null pointers, n_side beyond WSLDA_STATIC_MAX_SIDE or not 32 / 64, n_wf outside
+ * [1, WSLDA_STATIC_MAX_SPINORS], non-positive dx; WSLDA_ECUDA when there is no device or a launch fails. */
+#define WSLDA_STATIC_MAX_SIDE 64
+#define WSLDA_STATIC_MAX_SPINORS 65536
+size_t wslda_static_scratch_bytes(void);
+wslda_status wslda_gradient_densities_static(const void* psi, const double* cw_a, const double* cw_b, int64_t n_wf, int n_side,
+                                             const double dx[3], double* tau, double* j, void* cuda_stream);
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 int64_t wslda_launch_count(const wslda_ctx*);
 const char* wslda_last_error(const wslda_ctx*);

@@ -55,6 +55,35 @@ def fp64_probe():
     return f.value, int(n.value)
 
 
+STATIC_MAX_SIDE, STATIC_MAX_SPINORS = 64, 65536
+
+
+def gradient_densities_static(psi, cw_a, cw_b, dx, tau, j):
+    """wslda_gradient_densities_static: tau [2][M] and j [2][3][M] of the spinors psi [n][2][N][N][N] (N = 32 | 64) on
+    the current torch stream, with the kernel's scratch in the library's static device array: the call allocates nothing
+    (the caller passes the outputs).  Calls that overlap on the GPU race on that array."""
+    import torch
+    for t, dt, name in ((psi, torch.complex128, "psi"), (cw_a, torch.float64, "cw_a"), (cw_b, torch.float64, "cw_b"),
+                        (tau, torch.float64, "tau"), (j, torch.float64, "j")):
+        if t is None and name in ("tau", "j"):
+            continue
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise WsldaError(f"gradient_densities_static: {name} must be a contiguous CUDA tensor of {dt}")
+    if psi.dim() != 5 or psi.shape[1] != 2 or not (psi.shape[2] == psi.shape[3] == psi.shape[4]):
+        raise WsldaError("gradient_densities_static: psi must be [n][2][N][N][N]")
+    n, N = int(psi.shape[0]), int(psi.shape[2])
+    M = N ** 3
+    if cw_a.numel() < n or cw_b.numel() < n or (tau is not None and tau.numel() < 2 * M) or (j is not None and j.numel() < 6 * M):
+        raise WsldaError("gradient_densities_static: a weight or output tensor is too small")
+    d3 = (C.c_double * 3)(*[float(v) for v in dx])
+    rc = lib().wslda_gradient_densities_static(psi.data_ptr(), cw_a.data_ptr(), cw_b.data_ptr(), n, N, d3,
+                                               tau.data_ptr() if tau is not None else None,
+                                               j.data_ptr() if j is not None else None,
+                                               C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc:
+        raise WsldaError(f"gradient_densities_static failed ({rc}): {lib().wslda_last_error(None).decode()}")
+
+
 def set_tuning(**kw):
     """Process-wide kernel selection / tile sizes for contexts created afterwards (wslda_set_tuning); no arguments
     restores the defaults."""
@@ -79,7 +108,8 @@ SYMBOLS = ["wslda_workspace_bytes", "wslda_ctx_create", "wslda_ctx_destroy", "ws
            "wslda_apply_h", "wslda_densities", "wslda_update_potentials", "wslda_history_length", "wslda_abm_init",
            "wslda_abm_step", "wslda_abm_step_host", "wslda_launch_count", "wslda_last_error", "wslda_profile",
            "wslda_profile_report", "wslda_set_reduce_hook", "wslda_set_tuning", "wslda_set_external_velocity",
-           "wslda_energy", "wslda_watchdog", "wslda_fp64_probe"]
+           "wslda_energy", "wslda_watchdog", "wslda_fp64_probe", "wslda_static_scratch_bytes",
+           "wslda_gradient_densities_static"]
 OBS = ["N_a", "N_b", "E_kin", "E_pot", "E_pair", "E_pot_ext", "E_pair_ext", "E_total", "E_curr", "E_vel_ext"]
 REDUCE_HOOK = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
@@ -116,6 +146,10 @@ def lib():
         L.wslda_set_tuning.argtypes = [C.c_void_p]
         L.wslda_set_external_velocity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_fp64_probe.argtypes = [C.c_void_p, C.c_void_p]
+        L.wslda_static_scratch_bytes.restype = C.c_size_t
+        L.wslda_static_scratch_bytes.argtypes = []
+        L.wslda_gradient_densities_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int,
+                                                      C.POINTER(C.c_double), C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.wslda_watchdog.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.wslda_profile.argtypes = [C.c_void_p, C.c_int]
