@@ -43,7 +43,7 @@ class Tuning(C.Structure):
                 ("fused_chunk", C.c_int), ("fused_streams", C.c_int), ("group", C.c_int), ("p_planes", C.c_int),
                 ("x_rows", C.c_int), ("persistent_ctas", C.c_int), ("onchip_ctas", C.c_int), ("chunk_mb", C.c_double),
                 ("fft_radix", C.c_int), ("spin_limit", C.c_int), ("tma_group", C.c_int), ("tma_block", C.c_int),
-                ("tma_ring", C.c_int), ("tma_lag", C.c_int)]
+                ("tma_ring", C.c_int), ("tma_lag", C.c_int), ("dmma_stage", C.c_int), ("dmma_ctas", C.c_int)]
 
 
 def fp64_probe():

@@ -13,6 +13,7 @@
 #include "mega3d.cuh"
 #include "mega3s.cuh"
 #include "mega3t.cuh"
+#include "mega3m.cuh"
 #include "mega64.cuh"
 #include "gdens.cuh"
 #include "kernels.cuh"
@@ -133,7 +134,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * (P.N[0] < 64 ? 64 : P.N[0]) * 8);   // mega3t: 64 partial sums per spinor
     P.mega_acc_bytes = align_up((size_t)F3_RING * 4 * M * 8);
     P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)5 * n_wf * sizeof(int));      // done[4][G <= n_wf] + one arrival counter per spinor
-    P.mega_pack_bytes = align_up((size_t)M * 48);
+    P.mega_pack_bytes = align_up((size_t)M * 48) + 16384;            // + the folded derivative matrices of mega3m.cuh
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
   P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms && !f->quantum_friction;
@@ -188,6 +189,7 @@ struct wslda_ctx {
   int mega_grid;
   int sep_pm, sep_em;              // mega3s.cuh: x-planes per P item, row pairs per XE item
   int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
+  int dm3, dm3_grid; double* m_mat;   // 32^3 Eq. 40: matrix-form (DMMA) stage kernel (mega3m.cuh), its grid, the folded matrices
   int t3, t3_gs, t3_r, t3_ring, t3_lag, t3_grid;    // 32^3 Eq. 40: warp-specialised TMA-fed stage kernel (mega3t.cuh): spinors per group, per heavy super-item
   T3Maps t3_maps;                  // tensor maps of the arrays the library owns (QL ring, alpha); psi is encoded per launch
   int spin_limit;                  // bound of the device-side dependency waits (polls of 200 ns)
@@ -427,6 +429,33 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
       if (!ok) { cudaGetLastError(); c->t3 = 0; }            // no TMA encoder / not enough shared memory: the mega3s kernels serve
     }
     if (g_tune.persistent_ctas > 0) c->mega_grid = g_tune.persistent_ctas;
+    // matrix-form stage kernel (mega3m.cuh): Ce, Co per axis (z, y, x) from the k^2 tables of Eq. 25 (Nyquist kept)
+    c->m_mat = (double*)((char*)c->m_pack + align_up((size_t)M * 48));
+    c->dm3 = P.sep && f->kin_form == WSLDA_KIN_SYM40 && !c->t3 && g_tune.dmma_stage >= F3M_DEFAULT_ON;
+    if (c->dm3) {
+      std::vector<double> mat(3 * 2 * 256);
+      for (int ax = 0; ax < 3; ++ax) {
+        const double* k2 = c->hk2[2 - ax];
+        double cc[32];
+        for (int m = 0; m < 32; ++m) { double t = 0.0; for (int q = 0; q < 32; ++q) t -= k2[q] * cos(2.0 * PI * ((q * m) & 31) / 32.0); cc[m] = t / 32.0; }
+        for (int i = 0; i < 16; ++i)
+          for (int k = 0; k < 16; ++k) {
+            const int m = (i - k) & 31;
+            mat[(ax * 2 + 0) * 256 + i * 16 + k] = 0.5 * (cc[m] + cc[(m + 16) & 31]);
+            mat[(ax * 2 + 1) * 256 + i * 16 + k] = 0.5 * (cc[m] - cc[(m + 16) & 31]);
+          }
+      }
+      cudaMemcpy(c->m_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
+      int occ3 = 0, want = g_tune.dmma_ctas > 0 ? g_tune.dmma_ctas : F3M_OCC, got = want;
+      bool ok = true;
+#define WS_DM3_ATTR(K) do { ok = ok && cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, F3M_BUF_BYTES) == cudaSuccess; \
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ3, K, 128, F3M_BUF_BYTES); if (occ3 < got) got = occ3; } while (0)
+      WS_DM3_ATTR(k_f3m_mega<F3_APPLY>); WS_DM3_ATTR(k_f3m_mega<F3_CORR>); WS_DM3_ATTR(k_f3m_mega<F3_RHS>);
+#undef WS_DM3_ATTR
+      if (!ok || got < 1) { cudaGetLastError(); c->dm3 = 0; }
+      c->dm3_grid = got * sms;
+      if (g_tune.persistent_ctas > 0) c->dm3_grid = g_tune.persistent_ctas;
+    }
   }
   if (P.f6) {
     char* b = base + P.off_f6;

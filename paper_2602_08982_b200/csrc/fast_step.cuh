@@ -95,6 +95,17 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
     cudaMemcpyAsync(c->err_host, &A.sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);      // read at the next API call
     return;
   }
+  if (c->dm3 && sym) {                       // 32^3 Eq. 40: matrix-form line derivatives on DMMA (mega3m.cuh)
+    F3MMega A;
+    A.m = a; A.pm = c->sep_pm; A.em = c->sep_em; A.mat = c->m_mat;
+    const int ITs = a.gs * 32 / A.pm + a.gs * 32 / A.em + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
+    const long tot = (long)(a.G + 2) * ITs;
+    const int gr = (int)(tot < c->dm3_grid ? tot : c->dm3_grid);
+    void (*km)(F3MMega) = mode == F3_APPLY ? k_f3m_mega<F3_APPLY> : mode == F3_CORR ? k_f3m_mega<F3_CORR> : k_f3m_mega<F3_RHS>;
+    LAUNCHN(c, mode == F3_APPLY ? "k_f3m_mega_apply" : mode == F3_CORR ? "k_f3m_mega_corr" : "k_f3m_mega_rhs", km, gr, 128, F3M_BUF_BYTES, st, A);
+    cudaMemcpyAsync(c->err_host, &c->m_sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);
+    return;
+  }
   if (c->sep3) {                             // 32^3: axis-by-axis Laplacian, two passes (mega3s.cuh)
     F3SMega A;
     A.m = a; A.pm = c->sep_pm; A.em = c->sep_em;

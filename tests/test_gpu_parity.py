@@ -292,7 +292,33 @@ def test_tma_stage_kernel_32cubed(tuning, nwf, group, block, ring, lag):
     assert "k_t3_mega_corr" in names and "k_t3_mega_rhs" in names and "k_f3s_mega_corr" not in names
 
 
-@pytest.mark.parametrize("which", ["mega3s_32", "mega3d_16", "mega64", "tma_32"])
+@pytest.mark.parametrize("nwf,pm,em,ctas", [(10, 4, 2, 3), (37, 1, 1, 2), (7, 8, 4, 1)])
+def test_dmma_stage_kernel_32cubed(tuning, nwf, pm, em, ctas):
+    """The matrix-form (Eq. 28b) 32^3 Eq. 40 stage kernel on FP64 tensor instructions (mega3m.cuh, dmma_stage): H psi with
+    eps_n, a sub-range, self-consistent steps with ragged groups and more groups than ring slots; the kernels really ran."""
+    tuning(dmma_stage=1, dmma_ctas=ctas, p_planes=pm, x_rows=em, group=(5 if nwf > 30 else 0), fused_chunk=3, fused_streams=3)
+    w = wl.cfg4(n_side=32, n_wf=nwf, kin_form=1, n_steps=3)
+    psi0 = w.spinors()
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi0)
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    h2, _ = g.apply_h(to_gpu(psi0), n_first=1, n_count=3)
+    h2 = to_np(h2)
+    assert relerr(h2[1:4], ref[1:4]) < TOL_H and not h2[:1].any() and not h2[4:].any()
+    pg, po, fg, fo, o, g = run_both(w, psi0, w.n_steps)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("delta", "U_a", "rho_a", "nu"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names and "k_f3s_mega_corr" not in names
+
+
+@pytest.mark.parametrize("which", ["mega3s_32", "mega3d_16", "mega64", "tma_32", "dmma_32"])
 def test_persistent_kernels_bit_reproducible(tuning, which):
     """The ticketed persistent kernels hand items to whichever CTA is free, but every sum is taken in a fixed order
     (partial sums per item, densities per ring slot in group order): two runs give identical bits."""
@@ -302,6 +328,8 @@ def test_persistent_kernels_bit_reproducible(tuning, which):
         tuning(group=3); w = generic((16, 32, 32), (1.0, 1.0, 1.0), 11, 1, func_id=2, dt=0.004)
     elif which == "mega64":
         w = wl.cfg4(n_side=64, n_wf=5, kin_form=1, n_steps=2)
+    elif which == "dmma_32":
+        tuning(dmma_stage=1, group=5); w = wl.cfg4(n_side=32, n_wf=23, kin_form=1, n_steps=3)
     else:
         tuning(enable_tma_stage=1, tma_group=4, tma_ring=6, tma_lag=2); w = wl.cfg4(n_side=32, n_wf=13, kin_form=1, n_steps=3)
     psi0 = w.spinors() if w.kidx is not None else spinors(w)
