@@ -26,7 +26,7 @@
 #define F3M_AL_BYTES (F3_N * F3M_APITCH * 8)
 #define F3M_BUF_BYTES (2 * F3M_PSI_BYTES + 2 * F3M_AL_BYTES)
 #ifndef F3M_DEFAULT_ON
-#define F3M_DEFAULT_ON 1                                  // wslda_tuning.dmma_stage >= this selects the kernel (1: opt-in, 0: default)
+#define F3M_DEFAULT_ON 0                                  // wslda_tuning.dmma_stage >= this selects the kernel (1: opt-in, 0: default)
 #endif
 #ifndef F3M_OCC
 #define F3M_OCC 3

@@ -247,7 +247,7 @@ def test_fast3d_multikernel_fallback(tuning):
 def test_axis_by_axis_stage_kernel_32cubed(tuning, sep, pm, em):
     """The default 32^3 Eq. 40 stage kernels (mega3s.cuh: Laplacian axis by axis) for several item sizes, ragged groups
     of 3 spinors, and the three-pass kernels they replace (disable_axis_split): H psi and self-consistent steps."""
-    tuning(disable_axis_split=int(sep == "0"), p_planes=pm, x_rows=em, **SMALL)
+    tuning(disable_axis_split=int(sep == "0"), dmma_stage=-1, p_planes=pm, x_rows=em, **SMALL)
     w = wl.cfg4(n_side=32, n_wf=10, kin_form=1, n_steps=3)
     psi0 = w.spinors()
     o, g = make_oracle(w), make_gpu(w)
@@ -323,7 +323,7 @@ def test_persistent_kernels_bit_reproducible(tuning, which):
     """The ticketed persistent kernels hand items to whichever CTA is free, but every sum is taken in a fixed order
     (partial sums per item, densities per ring slot in group order): two runs give identical bits."""
     if which == "mega3s_32":
-        tuning(group=5); w = wl.cfg4(n_side=32, n_wf=23, kin_form=1, n_steps=3)
+        tuning(group=5, dmma_stage=-1); w = wl.cfg4(n_side=32, n_wf=23, kin_form=1, n_steps=3)
     elif which == "mega3d_16":
         tuning(group=3); w = generic((16, 32, 32), (1.0, 1.0, 1.0), 11, 1, func_id=2, dt=0.004)
     elif which == "mega64":
