@@ -308,17 +308,29 @@ __global__ void __launch_bounds__(128) k_f3_fin2(F3Fin2 a) {
 
 // densities of scale_n * psi for the spinors of a chunk (stage 1: the normalised predictor)
 struct F3DensOnly { const cplx* psi; const double* scale; int cnt; int64_t M; F3Dens d; };
-__global__ void __launch_bounds__(64) k_f3_dens(F3DensOnly a) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= a.M) return;
+// 64 lattice points per CTA, the chunk's spinors dealt round-robin to four thread groups (more loads in flight: the kernel
+// is bound by L2 latency, not by arithmetic); the four partial sums are added in a fixed order
+__global__ void __launch_bounds__(256) k_f3_dens(F3DensOnly a) {
+  __shared__ double part[3][4][64];
+  const int p = threadIdx.x & 63, q = threadIdx.x >> 6;
+  const int64_t i = (int64_t)blockIdx.x * 64 + p;                 // M is a multiple of 1024 on this path
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll 8
-  for (int n = 0; n < a.cnt; ++n) {
+#pragma unroll 4
+  for (int n = q; n < a.cnt; n += 4) {
     const double s = a.scale ? a.scale[n] : 1.0;
     const cplx u = cscale(a.psi[(int64_t)(2 * n) * a.M + i], s), v = cscale(a.psi[(int64_t)(2 * n + 1) * a.M + i], s);
     f3_dens_add(acc, u, v, a.d.cpref[n], a.d.w_a[n], a.d.w_b[n]);
   }
-  f3_dens_store(a.d, a.M, i, acc);
+  if (q) {
+#pragma unroll
+    for (int f = 0; f < 4; ++f) part[q - 1][f][p] = acc[f];
+  }
+  __syncthreads();
+  if (q == 0) {
+#pragma unroll
+    for (int f = 0; f < 4; ++f) acc[f] = (acc[f] + part[0][f][p]) + (part[1][f][p] + part[2][f][p]);
+    f3_dens_store(a.d, a.M, i, acc);
+  }
 }
 
 // raw[f] = sum over the per-stream accumulators in stream order (planes rho_a, rho_b, nu_re, nu_im)

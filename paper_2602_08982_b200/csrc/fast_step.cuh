@@ -290,7 +290,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
         d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
         d.d = f3_dens_args(c, q, n0, k < ns);
         WORK(c, 0, 0);
-        LAUNCH(c, k_f3_dens, nb(P.M, 64), 64, 0, st, d);
+        LAUNCH(c, k_f3_dens, nb(P.M, 64), 256, 0, st, d);
       }
     }
     f3_join(c, s);
@@ -323,7 +323,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
     F3DensOnly d;
     d.psi = s.phi + 2 * n0 * P.M; d.scale = c->f.normalize ? c->scale + n0 : nullptr; d.cnt = cnt; d.M = P.M;
     d.d = f3_dens_args(c, q, n0, k < ns);
-    LAUNCH(c, k_f3_dens, nb(P.M, 64), 64, 0, st, d);
+    LAUNCH(c, k_f3_dens, nb(P.M, 64), 256, 0, st, d);
   }
   f3_join(c, s);
   f3_dens_final(c, used, s.user);

@@ -28,6 +28,9 @@
 #ifndef F3M_DEFAULT_ON
 #define F3M_DEFAULT_ON 0                                  // wslda_tuning.dmma_stage >= this selects the kernel (1: opt-in, 0: default)
 #endif
+#ifndef F3M_PREFETCH
+#define F3M_PREFETCH 1                                   // XE items: L2 prefetch of the Q / C_part rows behind the tile loads (+2-3 %)
+#endif
 #ifndef F3M_OCC
 #define F3M_OCC 3
 #endif
@@ -209,6 +212,18 @@ __device__ __forceinline__ void f3m_body_xe(const F3MMega& A, const F3Pol& pol, 
     f3m_load<true>(a, n, y, buf);
     f3m_cp_commit();
     double e = 0.0, xx = 0.0, xpr = 0.0, xpi = 0.0, pp = 0.0;
+#if F3M_PREFETCH
+    // the rows of Q (and C_part) this CTA's epilogue reads: 32 x-rows of 512 bytes per component; one 128-byte line per thread
+    {
+      const int xr = threadIdx.x >> 2, seg = threadIdx.x & 3;
+      const size_t i = (size_t)y * F3_N + (size_t)xr * F3_PLANE + seg * 8;
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        f3_pf(a.spec0 + (ring + c) * M + i);
+        if (MODE == F3_CORR) f3_pf(a.cpart + (size_t)(2 * n + c) * M + i);
+      }
+    }
+#endif
     f3m_cp_wait<0>();
     __syncthreads();
 #pragma unroll 1
