@@ -156,7 +156,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS, cap = M <= 512 ? 296 : 148; P.oc_grid = (int)(nb_ < cap ? nb_ : cap); }
   if (g_tune.onchip_ctas > 0 && g_tune.onchip_ctas < P.oc_grid) P.oc_grid = g_tune.onchip_ctas;
   P.off_oc = o; P.oc_dpart_bytes = 0;
-  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes; }
+  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes + 65536; }   // + folded derivative matrices
   P.total = o;
   return 0;
 }
@@ -183,6 +183,7 @@ struct wslda_ctx {
   F3Sync* m_sync;
   cplx* m_pack;
   double* oc_dpart;
+  double* oc_mat; int oc_dm;       // on-chip 64 x 64: the Laplacian in matrix form on DMMA (onchip_step.cuh), its folded matrices
   cplx *s_spec0, *s_spec1, *s_X, *s_pack;   // 64^3 rings
   double *s_part, *s_acc, *s_partn;
   F3Sync* s_sync;
@@ -471,6 +472,25 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaFuncSetAttribute(k_f6_mega<F3_RHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * F6_TILE * 16);
   }
   if (P.oc) c->oc_dpart = (double*)(base + P.off_oc);
+  c->oc_dm = 0; c->oc_mat = nullptr;
+  if (P.oc && P.nd == 2 && P.N[0] == 64 && P.N[1] == 64 && g_tune.dmma_stage >= 0) {
+    // second-derivative matrices of Eq. 28b per axis, folded once: [axis][Ce | Co][32][32] (Nyquist mode kept: even derivative)
+    c->oc_mat = (double*)(base + P.off_oc + P.oc_dpart_bytes);
+    std::vector<double> mat(2 * 2 * 1024);
+    for (int ax = 0; ax < 2; ++ax) {
+      const double* k2 = c->hk2[ax];
+      double cc[64];
+      for (int m = 0; m < 64; ++m) { double t = 0.0; for (int q = 0; q < 64; ++q) t -= k2[q] * cos(2.0 * PI * ((q * m) & 63) / 64.0); cc[m] = t / 64.0; }
+      for (int i = 0; i < 32; ++i)
+        for (int k = 0; k < 32; ++k) {
+          const int m = (i - k) & 63;
+          mat[(ax * 2 + 0) * 1024 + i * 32 + k] = 0.5 * (cc[m] + cc[(m + 32) & 63]);
+          mat[(ax * 2 + 1) * 1024 + i * 32 + k] = 0.5 * (cc[m] - cc[(m + 32) & 63]);
+        }
+    }
+    cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
+    c->oc_dm = 1;
+  }
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
   cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);
   const int T = 256;

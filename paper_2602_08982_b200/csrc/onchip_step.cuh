@@ -31,6 +31,8 @@ struct OCArgs {
   double* dpart;               // [gridDim.x][4][slots], slots = max(M, 256)
   int64_t n;
   int S;
+  int dm;                      // 64 x 64: Laplacian in matrix form on DMMA (storage index swizzled: oc_ix)
+  const double* mat;           // [axis][Ce | Co][32][32]
 };
 
 // per-spinor sums of E[s][i] over the lattice: warp w takes spinors w, w + 8, ...; fixed order
@@ -54,6 +56,67 @@ __device__ __forceinline__ void oc_dens_acc(double (&acc)[MAXPT][4], int w, int 
 
 // MAXPT = compile-time bound on the lattice points per thread, max(1, M / blockDim.x): 2 (256 threads, M <= 512,
 // two CTAs per SM) or 8 (512 threads for M up to 4096, one CTA per SM)
+// ---- 64 x 64 (quasi-2D, configs[2]): the Laplacian in the matrix form of Eq. 28b on FP64 tensor
+// instructions.  d^2 along an axis is a real symmetric circulant; folded once (e = w[k] + w[k+32], o = w[k] - w[k+32]) it is
+// two 32 x 32 real matrices Ce, Co with out[i] +- out[i+32] = Ce e +- Co o.  A warp owns rows {8 rb ..} u {32 + 8 rb ..} by
+// columns {8 cb ..} u {32 + 8 cb ..} (16 warps = 16 blocks), contracts the tile along its rows (matrix = A operand) and along
+// its columns (matrix = B operand) straight from shared memory, and keeps its 16 x 16 results in accumulator fragments until
+// every warp has read the tile; then the tile is overwritten in place.  No transform passes, no spectrum, two barriers.
+// The tile's 16-byte elements are stored at oc_ix(i): column ^ f(row), conflict-free for both fragment footprints.
+__device__ __forceinline__ int oc_ix(int i, int dm) { return dm ? i ^ ((((i >> 6) & 1) << 2) | ((i >> 6) & 2)) : i; }
+__device__ __forceinline__ void oc_dmma(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int rb, int cb, double (&out)[2][2][2][2]) {   // [re | im][h][zi][j]
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const double* mx = mat + (8 * rb + g) * 32 + t;               // rows of Cx (A operand): + eo * 1024 + 4 kb
+  const double* my = mat + 2048 + (8 * cb + g) * 32 + t;        // columns of Cy = its rows (symmetric) (B operand)
+#pragma unroll
+  for (int zi = 0; zi < 2; ++zi) {                              // contraction along the rows: (d_x^2 w)[i][z]
+    const int z = 8 * cb + 32 * zi + g;
+    double acc[2][2][2] = {};                                   // [re | im][E | O][j]
+#pragma unroll
+    for (int kb = 0; kb < 8; ++kb) {
+      const int x1 = 4 * kb + t;
+      const cplx w1 = T[oc_ix(x1 * 64 + z, 1)], w2 = T[oc_ix((x1 + 32) * 64 + z, 1)];
+      const double me = __ldg(mx + 4 * kb), mo = __ldg(mx + 1024 + 4 * kb);
+      oc_dmma(acc[0][0][0], acc[0][0][1], me, w1.x + w2.x); oc_dmma(acc[0][1][0], acc[0][1][1], mo, w1.x - w2.x);
+      oc_dmma(acc[1][0][0], acc[1][0][1], me, w1.y + w2.y); oc_dmma(acc[1][1][0], acc[1][1][1], mo, w1.y - w2.y);
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) { out[p][0][zi][j] = acc[p][0][j] + acc[p][1][j]; out[p][1][zi][j] = acc[p][0][j] - acc[p][1][j]; }
+  }
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {                                 // contraction along the columns: (d_y^2 w)[x][i]
+    const int x = 8 * rb + 32 * h + g;
+    double acc[2][2][2] = {};
+#pragma unroll
+    for (int kb = 0; kb < 8; ++kb) {
+      const int y1 = 4 * kb + t;
+      const cplx w1 = T[oc_ix(x * 64 + y1, 1)], w2 = T[oc_ix(x * 64 + y1 + 32, 1)];
+      const double me = __ldg(my + 4 * kb), mo = __ldg(my + 1024 + 4 * kb);
+      oc_dmma(acc[0][0][0], acc[0][0][1], w1.x + w2.x, me); oc_dmma(acc[0][1][0], acc[0][1][1], w1.x - w2.x, mo);
+      oc_dmma(acc[1][0][0], acc[1][0][1], w1.y + w2.y, me); oc_dmma(acc[1][1][0], acc[1][1][1], w1.y - w2.y, mo);
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) { out[p][h][0][j] += acc[p][0][j] + acc[p][1][j]; out[p][h][1][j] += acc[p][0][j] - acc[p][1][j]; }
+  }
+}
+__device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const double (&out)[2][2][2][2]) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+#pragma unroll
+  for (int h = 0; h < 2; ++h)
+#pragma unroll
+    for (int zi = 0; zi < 2; ++zi)
+#pragma unroll
+      for (int j = 0; j < 2; ++j)
+        T[oc_ix((8 * rb + 32 * h + g) * 64 + 8 * cb + 32 * zi + 2 * t + j, 1)] = make_double2(out[0][h][zi][j], out[1][h][zi][j]);
+}
+
 template <int MODE, int MAXPT>
 __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_stage(OCArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -91,23 +154,34 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       if (w < PT * nsp_full) {
         const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
         if (a.scale && sp < cnt) { const double sc = a.scale[n0 + sp]; ru[w] = cscale(ru[w], sc); rv[w] = cscale(rv[w], sc); }
-        F[(2 * sp) * M + i] = ru[w]; F[(2 * sp + 1) * M + i] = rv[w];
+        F[(2 * sp) * M + oc_ix(i, a.dm)] = ru[w]; F[(2 * sp + 1) * M + oc_ix(i, a.dm)] = rv[w];
       }
     }
     __syncthreads();
-    const int G = 2 * S;
-    if (L.nd > 2) fft_axis<false>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
-    if (L.nd > 1) fft_axis<false>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
-    fft_axis<false>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
-    for (int idx = tid; idx < used; idx += NT) {
-      const int i = idx & (M - 1);
-      const int j2 = i & (L.N[2] - 1), j1 = (i >> L.lg[2]) & (L.N[1] - 1), j0 = i >> (L.lg[1] + L.lg[2]);
-      F[idx] = cscale(F[idx], kfactor(L, 0, j0, j1, j2).x);          // -k^2 / M at the stored (digit-reversed) position
+    if (a.dm) {                                                 // 64 x 64, 512 threads: lap u, lap v in place, matrix form on DMMA
+      const int wp = tid >> 5, rb = wp & 3, cb = wp >> 2;
+      for (int q = 0; q < 2 * cnt; ++q) {
+        double lap[2][2][2][2];
+        oc_lap64(F + (size_t)q * M, a.mat, rb, cb, lap);
+        __syncthreads();
+        oc_lap64_store(F + (size_t)q * M, rb, cb, lap);
+      }
+      __syncthreads();
+    } else {
+      const int G = 2 * S;
+      if (L.nd > 2) fft_axis<false>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
+      if (L.nd > 1) fft_axis<false>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
+      fft_axis<false>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
+      for (int idx = tid; idx < used; idx += NT) {
+        const int i = idx & (M - 1);
+        const int j2 = i & (L.N[2] - 1), j1 = (i >> L.lg[2]) & (L.N[1] - 1), j0 = i >> (L.lg[1] + L.lg[2]);
+        F[idx] = cscale(F[idx], kfactor(L, 0, j0, j1, j2).x);          // -k^2 / M at the stored (digit-reversed) position
+      }
+      __syncthreads();
+      fft_axis<true>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
+      if (L.nd > 1) fft_axis<true>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
+      if (L.nd > 2) fft_axis<true>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
     }
-    __syncthreads();
-    fft_axis<true>(F, G, L.lg[0], L.lg[1] + L.lg[2], L.tw[0]);
-    if (L.nd > 1) fft_axis<true>(F, G << L.lg[0], L.lg[1], L.lg[2], L.tw[1]);
-    if (L.nd > 2) fft_axis<true>(F, G << (L.lg[0] + L.lg[1]), L.lg[2], 0, L.tw[2]);
     // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order).  CORR leaves
     // X = C_part - i kappa H psi in F (phi_new = X + i kappa eps psi once eps_n is known): C_part is consumed here,
     // four slots at a time so that its loads are in flight together without holding 16 more values in registers.
@@ -134,7 +208,8 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
             const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b, kp2 = a.kperp2[n];
             const cplx u = ru[w], v = rv[w];
-            const cplx lu = F[(2 * sp) * M + i], lv = F[(2 * sp + 1) * M + i];
+            const int is = oc_ix(i, a.dm);
+            const cplx lu = F[(2 * sp) * M + is], lv = F[(2 * sp + 1) * M + is];
             const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
             const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
             const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                    // Eqs. 5, 15
@@ -143,10 +218,10 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             if (MODE == OC_APPLY) {
               a.out[(size_t)(2 * n) * M + i] = Hu; a.out[(size_t)(2 * n + 1) * M + i] = Hv;
             } else if (MODE == OC_RHS) {
-              F[(2 * sp) * M + i] = Hu; F[(2 * sp + 1) * M + i] = Hv;
+              F[(2 * sp) * M + is] = Hu; F[(2 * sp + 1) * M + is] = Hv;
             } else {
-              F[(2 * sp) * M + i] = make_double2(cu[r].x + a.kappa * Hu.y, cu[r].y - a.kappa * Hu.x);
-              F[(2 * sp + 1) * M + i] = make_double2(cv[r].x + a.kappa * Hv.y, cv[r].y - a.kappa * Hv.x);
+              F[(2 * sp) * M + is] = make_double2(cu[r].x + a.kappa * Hu.y, cu[r].y - a.kappa * Hu.x);
+              F[(2 * sp + 1) * M + is] = make_double2(cv[r].x + a.kappa * Hv.y, cv[r].y - a.kappa * Hv.x);
             }
           }
         }
@@ -171,7 +246,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const int64_t n = n0 + sp;
             const double e = s_eps[sp];
             const cplx u = ru[w], v = rv[w];
-            const cplx Hu = F[(2 * sp) * M + i], Hv = F[(2 * sp + 1) * M + i];
+            const cplx Hu = F[(2 * sp) * M + oc_ix(i, a.dm)], Hv = F[(2 * sp + 1) * M + oc_ix(i, a.dm)];
             if (MODE == OC_RHS) {
               const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
               a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
@@ -353,7 +428,7 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   a.out = out; a.cpart = cpart; a.kappa = kappa; a.dV = c->dV;
   a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.eps_out = eps_user;
   a.do_dens = do_dens; a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.dpart = c->oc_dpart;
-  a.n = n; a.S = P.ocS;
+  a.n = n; a.S = P.ocS; a.dm = c->oc_dm; a.mat = c->oc_mat;
   const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
   if (!g_oc_attr_done) {
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
