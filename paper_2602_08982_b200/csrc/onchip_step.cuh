@@ -45,8 +45,23 @@ __device__ __forceinline__ void oc_reduce(const double* E, int cnt, int lgM, dou
     if (lane == 0) out_s[s] = v;
   }
 }
+// one spinor of 4096 points, 16 warps: every warp sums a slice of 256, warp 0 adds the 16 slices in index order.
+// Contains the barrier between the two levels; `scratch` = 16 doubles of shared memory.
+__device__ __forceinline__ void oc_reduce1(const double* E, double* scratch, double* out_s) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double v = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) v += E[warp * 256 + k * 32 + lane];
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if (lane == 0) scratch[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    double t = lane < 16 ? scratch[lane] : 0.0;
+    for (int o = 8; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) out_s[0] = t;
+  }
+}
 
-// acc[w mod PT] += (a0..a3) with a register-resident accumulator array: the index is resolved by predication
 template <int MAXPT>
 __device__ __forceinline__ void oc_dens_acc(double (&acc)[MAXPT][4], int w, int PT, double a0, double a1, double a2, double a3) {
 #pragma unroll
@@ -117,23 +132,24 @@ __device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const do
         T[oc_ix((8 * rb + 32 * h + g) * 64 + 8 * cb + 32 * zi + 2 * t + j, 1)] = make_double2(out[0][h][zi][j], out[1][h][zi][j]);
 }
 
-template <int MODE, int MAXPT>
+template <int MODE, int MAXPT, bool DM = false>
 __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_stage(OCArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Lat& L = a.L;
-  const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x, NT = blockDim.x;
+  // the 64 x 64 matrix-form kernel (DM) is one spinor of 4096 points per batch on 512 threads: compile-time slot geometry
+  const int lgM = DM ? 12 : L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = DM ? 1 : a.S, tid = threadIdx.x, NT = DM ? 512 : blockDim.x;
   cplx* F = reinterpret_cast<cplx*>(smem_raw);                       // [S][2][M]
   double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);       // [S][M]
-  __shared__ double s_eps[OC_MAXS], s_sn[OC_MAXS];
+  __shared__ double s_eps[OC_MAXS], s_sn[OC_MAXS], s_red[16];
   // slots of this thread: lattice points i(kk) = (tid + 256 kk) & (M - 1), kk < PT; spinors s0, s0 + SSTEP, ...
-  const int PT = M >= NT ? M / NT : 1;
-  const int SSTEP = M >= NT ? 1 : NT / M, s0 = M >= NT ? 0 : tid >> lgM;
+  const int PT = DM ? 8 : M >= NT ? M / NT : 1;
+  const int SSTEP = DM ? 1 : M >= NT ? 1 : NT / M, s0 = DM ? 0 : M >= NT ? 0 : tid >> lgM;
   double acc[MAXPT][4];
 #pragma unroll
   for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
   // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP), at most OC_SLOTS of them; the spinor
   // values of the slots stay in registers from the load to the last phase (psi is read from HBM exactly once)
-  const int nsp_full = S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
+  const int nsp_full = DM ? 1 : S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
   const int64_t n_batches = (a.n + S - 1) / S;
   for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const int64_t n0 = b * S;
@@ -154,17 +170,29 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       if (w < PT * nsp_full) {
         const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
         if (a.scale && sp < cnt) { const double sc = a.scale[n0 + sp]; ru[w] = cscale(ru[w], sc); rv[w] = cscale(rv[w], sc); }
-        F[(2 * sp) * M + oc_ix(i, a.dm)] = ru[w]; F[(2 * sp + 1) * M + oc_ix(i, a.dm)] = rv[w];
+        F[(2 * sp) * M + oc_ix(i, DM)] = ru[w]; F[(2 * sp + 1) * M + oc_ix(i, DM)] = rv[w];
       }
     }
     __syncthreads();
-    if (a.dm) {                                                 // 64 x 64, 512 threads: lap u, lap v in place, matrix form on DMMA
+    if (DM) {                                                   // 64 x 64, 512 threads: lap u, lap v in place, matrix form on DMMA
       const int wp = tid >> 5, rb = wp & 3, cb = wp >> 2;
       for (int q = 0; q < 2 * cnt; ++q) {
         double lap[2][2][2][2];
         oc_lap64(F + (size_t)q * M, a.mat, rb, cb, lap);
         __syncthreads();
         oc_lap64_store(F + (size_t)q * M, rb, cb, lap);
+      }
+      // the spinor values are read again (L2) instead of being held in 64 registers across the matrix products
+#pragma unroll
+      for (int w = 0; w < OC_SLOTS; ++w) {
+        ru[w] = rv[w] = make_double2(0.0, 0.0);                 // (dead across the products on every path)
+        if (w < PT * nsp_full) {
+          const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+          if (sp < cnt) {
+            const double sc = a.scale ? a.scale[n0 + sp] : 1.0;
+            ru[w] = cscale(__ldcg(src + (size_t)(2 * sp) * M + i), sc); rv[w] = cscale(__ldcg(src + (size_t)(2 * sp + 1) * M + i), sc);
+          }
+        }
       }
       __syncthreads();
     } else {
@@ -208,7 +236,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
             const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b, kp2 = a.kperp2[n];
             const cplx u = ru[w], v = rv[w];
-            const int is = oc_ix(i, a.dm);
+            const int is = oc_ix(i, DM);
             const cplx lu = F[(2 * sp) * M + is], lv = F[(2 * sp + 1) * M + is];
             const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
             const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
@@ -228,7 +256,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       }
     }
     __syncthreads();
-    oc_reduce(E, cnt, lgM, s_eps);
+    if (DM) oc_reduce1(E, s_red, s_eps); else oc_reduce(E, cnt, lgM, s_eps);
     __syncthreads();
     if (tid < cnt) {
       const double e_true = a.dV * s_eps[tid];
@@ -246,7 +274,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const int64_t n = n0 + sp;
             const double e = s_eps[sp];
             const cplx u = ru[w], v = rv[w];
-            const cplx Hu = F[(2 * sp) * M + oc_ix(i, a.dm)], Hv = F[(2 * sp + 1) * M + oc_ix(i, a.dm)];
+            const cplx Hu = F[(2 * sp) * M + oc_ix(i, DM)], Hv = F[(2 * sp + 1) * M + oc_ix(i, DM)];
             if (MODE == OC_RHS) {
               const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
               a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
@@ -263,7 +291,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     }
     if (MODE == OC_CORR) {
       __syncthreads();
-      oc_reduce(E, cnt, lgM, s_sn);
+      if (DM) oc_reduce1(E, s_red, s_sn); else oc_reduce(E, cnt, lgM, s_sn);
       __syncthreads();
       if (tid < cnt) s_sn[tid] = a.normalize ? 1.0 / sqrt(a.dV * s_sn[tid]) : 1.0;
       __syncthreads();
@@ -316,7 +344,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
   const int lgM = L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = a.S, tid = threadIdx.x, NT = blockDim.x;
   cplx* F = reinterpret_cast<cplx*>(smem_raw);
   double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);
-  __shared__ double s_sn[OC_MAXS];
+  __shared__ double s_sn[OC_MAXS], s_red[16];
   const int PT = M >= NT ? M / NT : 1;
   const int SSTEP = M >= NT ? 1 : NT / M, s0 = M >= NT ? 0 : tid >> lgM;
   double acc[MAXPT][4];
@@ -366,7 +394,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       }
     }
     __syncthreads();
-    oc_reduce(E, cnt, lgM, s_sn);
+    if (M == 4096 && NT == 512) oc_reduce1(E, s_red, s_sn); else oc_reduce(E, cnt, lgM, s_sn);     // S = 1: all 16 warps
     __syncthreads();
     if (tid < cnt) s_sn[tid] = a.normalize ? 1.0 / sqrt(a.dV * s_sn[tid]) : 1.0;
     __syncthreads();
@@ -437,6 +465,9 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     g_oc_attr_done = true;
   }
   const bool small = P.M <= 512;
@@ -447,6 +478,7 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   WORK(c, 32.0 * P.M * n * (mode == OC_CORR ? 3.0 : 2.0), 5.0 * P.M * lgM * 2.0 * 2.0 * n);
   void (*k)(OCArgs);
   if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
+  else if (c->oc_dm) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, true> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, true> : k_onchip_stage<OC_RHS, 8, true>;
   else k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8> : k_onchip_stage<OC_RHS, 8>;
   LAUNCHN(c, mode == OC_APPLY ? "k_onchip_apply" : mode == OC_CORR ? "k_onchip_corr" : "k_onchip_rhs", k, grid, NT, smem, st, a);
   if (mode == OC_CORR && do_dens) {
