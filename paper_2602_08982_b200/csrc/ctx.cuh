@@ -491,6 +491,25 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
     c->oc_dm = 1;
   }
+  if (P.oc && P.nd == 1 && P.N[0] == 128 && P.ocS * 2 <= 32 && g_tune.dmma_stage >= 0) {
+    // lines of 128 points: [Ce | Co][64][64]
+    c->oc_mat = (double*)(base + P.off_oc + P.oc_dpart_bytes);
+    std::vector<double> mat(2 * 4096);
+    const double* k2 = c->hk2[0];              // (only the first 64 entries are kept on the host: rebuild the table)
+    double kk2[128];
+    for (int q = 0; q < 128; ++q) { const double len = 128 * c->dx[0]; const double k = (q < 64) ? 2.0 * PI * q / len : 2.0 * PI * (q - 128) / len; kk2[q] = k * k; }
+    (void)k2;
+    double cc[128];
+    for (int m = 0; m < 128; ++m) { double t = 0.0; for (int q = 0; q < 128; ++q) t -= kk2[q] * cos(2.0 * PI * ((q * m) & 127) / 128.0); cc[m] = t / 128.0; }
+    for (int i = 0; i < 64; ++i)
+      for (int k = 0; k < 64; ++k) {
+        const int m = (i - k) & 127;
+        mat[i * 64 + k] = 0.5 * (cc[m] + cc[(m + 64) & 127]);
+        mat[4096 + i * 64 + k] = 0.5 * (cc[m] - cc[(m + 64) & 127]);
+      }
+    cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
+    c->oc_dm = 2;
+  }
   // defaults: zero fields, alpha = 1, w_a = 0, w_b = 1, one mode k_perp = 0 with multiplicity 1, scale = 1
   cudaMemset(base + P.off_perwf, 0, P.off_part - P.off_perwf);
   const int T = 256;

@@ -78,7 +78,10 @@ __device__ __forceinline__ void oc_dens_acc(double (&acc)[MAXPT][4], int w, int 
 // its columns (matrix = B operand) straight from shared memory, and keeps its 16 x 16 results in accumulator fragments until
 // every warp has read the tile; then the tile is overwritten in place.  No transform passes, no spectrum, two barriers.
 // The tile's 16-byte elements are stored at oc_ix(i): column ^ f(row), conflict-free for both fragment footprints.
-__device__ __forceinline__ int oc_ix(int i, int dm) { return dm ? i ^ ((((i >> 6) & 1) << 2) | ((i >> 6) & 2)) : i; }
+// (DM = 1: 64 x 64 tile, column ^ f(row); DM = 2: lines of 128 points, point ^ 4 on odd lines; DM = 0: natural order)
+__device__ __forceinline__ int oc_ix(int line, int i, int dm) {
+  return dm == 1 ? i ^ ((((i >> 6) & 1) << 2) | ((i >> 6) & 2)) : dm == 2 ? i ^ ((line & 1) << 2) : i;
+}
 __device__ __forceinline__ void oc_dmma(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
@@ -93,7 +96,7 @@ __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int r
 #pragma unroll
     for (int kb = 0; kb < 8; ++kb) {
       const int x1 = 4 * kb + t;
-      const cplx w1 = T[oc_ix(x1 * 64 + z, 1)], w2 = T[oc_ix((x1 + 32) * 64 + z, 1)];
+      const cplx w1 = T[oc_ix(0, x1 * 64 + z, 1)], w2 = T[oc_ix(0, (x1 + 32) * 64 + z, 1)];
       const double me = __ldg(mx + 4 * kb), mo = __ldg(mx + 1024 + 4 * kb);
       oc_dmma(acc[0][0][0], acc[0][0][1], me, w1.x + w2.x); oc_dmma(acc[0][1][0], acc[0][1][1], mo, w1.x - w2.x);
       oc_dmma(acc[1][0][0], acc[1][0][1], me, w1.y + w2.y); oc_dmma(acc[1][1][0], acc[1][1][1], mo, w1.y - w2.y);
@@ -110,7 +113,7 @@ __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int r
 #pragma unroll
     for (int kb = 0; kb < 8; ++kb) {
       const int y1 = 4 * kb + t;
-      const cplx w1 = T[oc_ix(x * 64 + y1, 1)], w2 = T[oc_ix(x * 64 + y1 + 32, 1)];
+      const cplx w1 = T[oc_ix(0, x * 64 + y1, 1)], w2 = T[oc_ix(0, x * 64 + y1 + 32, 1)];
       const double me = __ldg(my + 4 * kb), mo = __ldg(my + 1024 + 4 * kb);
       oc_dmma(acc[0][0][0], acc[0][0][1], w1.x + w2.x, me); oc_dmma(acc[0][1][0], acc[0][1][1], w1.x - w2.x, mo);
       oc_dmma(acc[1][0][0], acc[1][0][1], w1.y + w2.y, me); oc_dmma(acc[1][1][0], acc[1][1][1], w1.y - w2.y, mo);
@@ -129,27 +132,69 @@ __device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const do
     for (int zi = 0; zi < 2; ++zi)
 #pragma unroll
       for (int j = 0; j < 2; ++j)
-        T[oc_ix((8 * rb + 32 * h + g) * 64 + 8 * cb + 32 * zi + 2 * t + j, 1)] = make_double2(out[0][h][zi][j], out[1][h][zi][j]);
+        T[oc_ix(0, (8 * rb + 32 * h + g) * 64 + 8 * cb + 32 * zi + 2 * t + j, 1)] = make_double2(out[0][h][zi][j], out[1][h][zi][j]);
 }
 
-template <int MODE, int MAXPT, bool DM = false>
+// ---- lines of 128 points (quasi-1D, configs[1]): d^2 as the folded matrices Ce, Co (64 x 64) of Eq. 28b.  The batch is a
+// matrix [lines][128]: the lines are the rows of the A operand, the matrix is the B operand.  Warp = (block of 8 lines, half
+// of the 64 folded columns): 4 x 16 k-blocks, results in fragments until every warp has read its lines, then in place.
+// Element i of line l is stored at oc_ix(l, i, 2).  Contains its two barriers.
+__device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
+  const bool active = 8 * lb < lines;                           // (whole warp)
+  const cplx* T = F + line * 128;
+  const int sw = (line & 1) << 2;
+  double acc[4][2][2][2] = {};                                  // [column block][re | im][E | O][j]
+  if (active) {
+#pragma unroll 4
+    for (int kb = 0; kb < 16; ++kb) {
+      const int k1 = (4 * kb + t) ^ sw;
+      const cplx w1 = T[k1], w2 = T[k1 + 64];
+      const double er = w1.x + w2.x, orr = w1.x - w2.x, ei = w1.y + w2.y, oi = w1.y - w2.y;
+#pragma unroll
+      for (int cb = 0; cb < 4; ++cb) {
+        const double* m = mat + (8 * (4 * ch + cb) + g) * 64 + 4 * kb + t;       // symmetric: column = row
+        const double me = __ldg(m), mo = __ldg(m + 4096);
+        oc_dmma(acc[cb][0][0][0], acc[cb][0][0][1], er, me); oc_dmma(acc[cb][0][1][0], acc[cb][0][1][1], orr, mo);
+        oc_dmma(acc[cb][1][0][0], acc[cb][1][0][1], ei, me); oc_dmma(acc[cb][1][1][0], acc[cb][1][1][1], oi, mo);
+      }
+    }
+  }
+  __syncthreads();
+  if (active) {
+    cplx* W = F + line * 128;
+#pragma unroll
+    for (int cb = 0; cb < 4; ++cb)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int i = 8 * (4 * ch + cb) + 2 * t + j;
+        W[i ^ sw] = make_double2(acc[cb][0][0][j] + acc[cb][0][1][j], acc[cb][1][0][j] + acc[cb][1][1][j]);
+        W[(i ^ sw) + 64] = make_double2(acc[cb][0][0][j] - acc[cb][0][1][j], acc[cb][1][0][j] - acc[cb][1][1][j]);
+      }
+  }
+  __syncthreads();
+}
+
+template <int MODE, int MAXPT, int DM = 0>
 __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_stage(OCArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Lat& L = a.L;
   // the 64 x 64 matrix-form kernel (DM) is one spinor of 4096 points per batch on 512 threads: compile-time slot geometry
-  const int lgM = DM ? 12 : L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = DM ? 1 : a.S, tid = threadIdx.x, NT = DM ? 512 : blockDim.x;
+  const int lgM = DM == 1 ? 12 : DM == 2 ? 7 : L.lg[0] + L.lg[1] + L.lg[2], M = 1 << lgM, S = DM == 1 ? 1 : a.S, tid = threadIdx.x;
+  const int NT = DM == 1 ? 512 : DM == 2 ? 256 : blockDim.x;
   cplx* F = reinterpret_cast<cplx*>(smem_raw);                       // [S][2][M]
   double* E = reinterpret_cast<double*>(F + (size_t)S * 2 * M);       // [S][M]
   __shared__ double s_eps[OC_MAXS], s_sn[OC_MAXS], s_red[16];
   // slots of this thread: lattice points i(kk) = (tid + 256 kk) & (M - 1), kk < PT; spinors s0, s0 + SSTEP, ...
-  const int PT = DM ? 8 : M >= NT ? M / NT : 1;
-  const int SSTEP = DM ? 1 : M >= NT ? 1 : NT / M, s0 = DM ? 0 : M >= NT ? 0 : tid >> lgM;
+  const int PT = DM == 1 ? 8 : DM == 2 ? 1 : M >= NT ? M / NT : 1;
+  const int SSTEP = DM == 1 ? 1 : DM == 2 ? 2 : M >= NT ? 1 : NT / M, s0 = DM == 1 ? 0 : DM == 2 ? tid >> 7 : M >= NT ? 0 : tid >> lgM;
   double acc[MAXPT][4];
 #pragma unroll
   for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
   // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP), at most OC_SLOTS of them; the spinor
   // values of the slots stay in registers from the load to the last phase (psi is read from HBM exactly once)
-  const int nsp_full = DM ? 1 : S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
+  const int nsp_full = DM == 1 ? 1 : S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
   const int64_t n_batches = (a.n + S - 1) / S;
   for (int64_t b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const int64_t n0 = b * S;
@@ -170,11 +215,26 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       if (w < PT * nsp_full) {
         const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
         if (a.scale && sp < cnt) { const double sc = a.scale[n0 + sp]; ru[w] = cscale(ru[w], sc); rv[w] = cscale(rv[w], sc); }
-        F[(2 * sp) * M + oc_ix(i, DM)] = ru[w]; F[(2 * sp + 1) * M + oc_ix(i, DM)] = rv[w];
+        F[(2 * sp) * M + oc_ix(0, i, DM)] = ru[w]; F[(2 * sp + 1) * M + oc_ix(1, i, DM)] = rv[w];
       }
     }
     __syncthreads();
-    if (DM) {                                                   // 64 x 64, 512 threads: lap u, lap v in place, matrix form on DMMA
+    if (DM == 2) {                                              // lines of 128 points, 256 threads: d^2 in matrix form on DMMA
+      oc_lap128(F, a.mat, 2 * cnt);
+      // the spinor values are read again (L2) instead of being held in registers across the matrix products
+#pragma unroll
+      for (int w = 0; w < OC_SLOTS; ++w) {
+        ru[w] = rv[w] = make_double2(0.0, 0.0);
+        if (w < PT * nsp_full) {
+          const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
+          if (sp < cnt) {
+            const double sc = a.scale ? a.scale[n0 + sp] : 1.0;
+            ru[w] = cscale(__ldcg(src + (size_t)(2 * sp) * M + i), sc); rv[w] = cscale(__ldcg(src + (size_t)(2 * sp + 1) * M + i), sc);
+          }
+        }
+      }
+      __syncthreads();
+    } else if (DM == 1) {                                       // 64 x 64, 512 threads: lap u, lap v in place, matrix form on DMMA
       const int wp = tid >> 5, rb = wp & 3, cb = wp >> 2;
       for (int q = 0; q < 2 * cnt; ++q) {
         double lap[2][2][2][2];
@@ -236,8 +296,8 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const cplx D = cadd(a.F.delta[i], a.F.dext[i]);
             const double pa = a.F.U_a[i] - a.F.mu_a, pb = a.F.U_b[i] - a.F.mu_b, kp2 = a.kperp2[n];
             const cplx u = ru[w], v = rv[w];
-            const int is = oc_ix(i, DM);
-            const cplx lu = F[(2 * sp) * M + is], lv = F[(2 * sp + 1) * M + is];
+            const int is = oc_ix(0, i, DM), it = oc_ix(1, i, DM);
+            const cplx lu = F[(2 * sp) * M + is], lv = F[(2 * sp + 1) * M + it];
             const cplx Ku = make_double2(-0.5 * lu.x + 0.5 * kp2 * u.x, -0.5 * lu.y + 0.5 * kp2 * u.y);   // Eq. 14
             const cplx Kv = make_double2(-0.5 * lv.x + 0.5 * kp2 * v.x, -0.5 * lv.y + 0.5 * kp2 * v.y);
             const cplx Hu = cadd(Ku, cadd(cscale(u, pa), cmul(D, v)));                                    // Eqs. 5, 15
@@ -246,17 +306,17 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             if (MODE == OC_APPLY) {
               a.out[(size_t)(2 * n) * M + i] = Hu; a.out[(size_t)(2 * n + 1) * M + i] = Hv;
             } else if (MODE == OC_RHS) {
-              F[(2 * sp) * M + is] = Hu; F[(2 * sp + 1) * M + is] = Hv;
+              F[(2 * sp) * M + is] = Hu; F[(2 * sp + 1) * M + it] = Hv;
             } else {
               F[(2 * sp) * M + is] = make_double2(cu[r].x + a.kappa * Hu.y, cu[r].y - a.kappa * Hu.x);
-              F[(2 * sp + 1) * M + is] = make_double2(cv[r].x + a.kappa * Hv.y, cv[r].y - a.kappa * Hv.x);
+              F[(2 * sp + 1) * M + it] = make_double2(cv[r].x + a.kappa * Hv.y, cv[r].y - a.kappa * Hv.x);
             }
           }
         }
       }
     }
     __syncthreads();
-    if (DM) oc_reduce1(E, s_red, s_eps); else oc_reduce(E, cnt, lgM, s_eps);
+    if (DM == 1) oc_reduce1(E, s_red, s_eps); else oc_reduce(E, cnt, lgM, s_eps);
     __syncthreads();
     if (tid < cnt) {
       const double e_true = a.dV * s_eps[tid];
@@ -274,7 +334,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const int64_t n = n0 + sp;
             const double e = s_eps[sp];
             const cplx u = ru[w], v = rv[w];
-            const cplx Hu = F[(2 * sp) * M + oc_ix(i, DM)], Hv = F[(2 * sp + 1) * M + oc_ix(i, DM)];
+            const cplx Hu = F[(2 * sp) * M + oc_ix(0, i, DM)], Hv = F[(2 * sp + 1) * M + oc_ix(1, i, DM)];
             if (MODE == OC_RHS) {
               const cplx fu = make_double2(Hu.y - e * u.y, -(Hu.x - e * u.x)), fv = make_double2(Hv.y - e * v.y, -(Hv.x - e * v.x));
               a.out[(size_t)(2 * n) * M + i] = fu; a.out[(size_t)(2 * n + 1) * M + i] = fv;
@@ -291,7 +351,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     }
     if (MODE == OC_CORR) {
       __syncthreads();
-      if (DM) oc_reduce1(E, s_red, s_sn); else oc_reduce(E, cnt, lgM, s_sn);
+      if (DM == 1) oc_reduce1(E, s_red, s_sn); else oc_reduce(E, cnt, lgM, s_sn);
       __syncthreads();
       if (tid < cnt) s_sn[tid] = a.normalize ? 1.0 / sqrt(a.dV * s_sn[tid]) : 1.0;
       __syncthreads();
@@ -465,9 +525,12 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     g_oc_attr_done = true;
   }
   const bool small = P.M <= 512;
@@ -477,8 +540,9 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   const double lgM = (double)(P.lg[0] + P.lg[1] + P.lg[2]);
   WORK(c, 32.0 * P.M * n * (mode == OC_CORR ? 3.0 : 2.0), 5.0 * P.M * lgM * 2.0 * 2.0 * n);
   void (*k)(OCArgs);
-  if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
-  else if (c->oc_dm) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, true> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, true> : k_onchip_stage<OC_RHS, 8, true>;
+  if (small && c->oc_dm == 2) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2, 2> : k_onchip_stage<OC_RHS, 2, 2>;
+  else if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
+  else if (c->oc_dm == 1) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, 1> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, 1> : k_onchip_stage<OC_RHS, 8, 1>;
   else k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8> : k_onchip_stage<OC_RHS, 8>;
   LAUNCHN(c, mode == OC_APPLY ? "k_onchip_apply" : mode == OC_CORR ? "k_onchip_corr" : "k_onchip_rhs", k, grid, NT, smem, st, a);
   if (mode == OC_CORR && do_dens) {
