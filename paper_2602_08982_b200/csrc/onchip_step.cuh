@@ -417,12 +417,13 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP); two slots per round so that 2 x 2 x (1 + m)
     // independent 16-byte loads are in flight before the first use
     const int nsp = cnt > s0 ? (cnt - s0 + SSTEP - 1) / SSTEP : 0, W = PT * nsp;
-    for (int w0 = 0; w0 < W; w0 += 2) {
-      cplx ph[2][2], fh[2][2][5];
-      size_t off[2][2];
-      int si[2], ii[2];
+    constexpr int R = MAXPT <= 2 ? 2 : 1;                      // slots per round (MAXPT = 8: 64 registers hold the density accumulators)
+    for (int w0 = 0; w0 < W; w0 += R) {
+      cplx ph[R][2], fh[R][2][5];
+      size_t off[R][2];
+      int si[R], ii[R];
 #pragma unroll
-      for (int r = 0; r < 2; ++r) {
+      for (int r = 0; r < R; ++r) {
         const int w = w0 + r < W ? w0 + r : W - 1;               // the tail repeats the last slot (harmless: same values)
         ii[r] = (tid + NT * (w % PT)) & (M - 1); si[r] = s0 + (w / PT) * SSTEP;
 #pragma unroll
@@ -435,7 +436,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
         }
       }
 #pragma unroll
-      for (int r = 0; r < 2; ++r) {
+      for (int r = 0; r < R; ++r) {
         if (w0 + r >= W) break;
         double nrm = 0.0;
 #pragma unroll
