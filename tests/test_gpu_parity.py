@@ -694,6 +694,53 @@ def test_density_allreduce_through_nccl_single_rank():
             dist.destroy_process_group()
 
 
+@pytest.mark.parametrize("case", ["fused32", "mega3d16", "onchip", "general"])
+def test_reduce_hook_fires_on_the_callers_stream_with_complete_sums(case, tuning):
+    """The density block handed to the hook is complete when the hook's work runs: the hook is given the
+    CALLER's stream -- never one of the library-owned stage-1 streams --, twice per self-consistent step; a copy of the block
+    enqueued there by the hook equals the block after a full device synchronisation (nothing writes it after the last hook),
+    and a hook that only copies leaves the step bit-identical to an unhooked one."""
+    import torch
+    if case == "fused32":
+        tuning(fused_chunk=3, fused_streams=3); w = wl.cfg4(n_side=32, n_wf=11, kin_form=1, n_steps=2)
+    elif case == "mega3d16":
+        tuning(fused_chunk=2, fused_streams=3, group=3); w = generic((16, 32, 32), (1.0, 1.0, 1.0), 7, 1, func_id=2, dt=0.004)
+    elif case == "onchip":
+        w = generic((64, 64), (1.0, 1.0), 6, 0, func_id=2, dt=0.004)
+    else:
+        w = generic((16, 8, 8), (1.0, 1.0, 1.0), 9, 2, func_id=2, dt=0.004)
+    psi0 = w.spinors() if getattr(w, "kidx", None) is not None else spinors(w)
+    final = {}
+    for hooked in (True, False):
+        g = make_gpu(w)
+        s = torch.cuda.Stream()
+        calls = []
+        if hooked:
+            def hook(block, stream, calls=calls):
+                with torch.cuda.stream(torch.cuda.ExternalStream(stream)):
+                    calls.append((stream, block, block.clone()))
+            g.set_reduce_hook(hook)
+        phi = to_gpu(psi0)
+        hist = [torch.zeros_like(phi) for _ in range(g.m)]
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            hist = g.abm_init(phi, hist, w.dt, 0)
+            n0 = len(calls)
+            hist = g.abm_step(phi, hist, w.dt)
+        torch.cuda.synchronize()
+        if hooked:
+            step_calls = calls[n0:]
+            assert len(step_calls) == 2, len(step_calls)                 # after the predictor's and after the corrector's densities
+            for stream, block, snap in step_calls:
+                assert stream == s.cuda_stream                            # the caller's stream, not a library-owned one
+                assert block.numel() % g.M == 0 and 4 <= block.numel() // g.M <= 14
+            stream, block, snap = step_calls[-1]
+            assert torch.equal(snap, block) and float(block.abs().max()) > 0.0
+        final[hooked] = (to_np(phi).copy(), to_np(g.get_field("rho_a")).copy(), to_np(g.get_field("nu")).copy())
+    for a, b in zip(final[True], final[False]):
+        assert np.array_equal(a, b)
+
+
 # ---- NEXT-1: current / velocity coupling (Eq. 4c PAPER.md:140, Eqs. 9b-c PAPER.md:199-205), general path ---------------
 def _with_currents(w, seed, amp=0.2):
     M = int(np.prod(w.shape))
