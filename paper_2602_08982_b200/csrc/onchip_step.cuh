@@ -189,9 +189,12 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
   // slots of this thread: lattice points i(kk) = (tid + 256 kk) & (M - 1), kk < PT; spinors s0, s0 + SSTEP, ...
   const int PT = DM == 1 ? 8 : DM == 2 ? 1 : M >= NT ? M / NT : 1;
   const int SSTEP = DM == 1 ? 1 : DM == 2 ? 2 : M >= NT ? 1 : NT / M, s0 = DM == 1 ? 0 : DM == 2 ? tid >> 7 : M >= NT ? 0 : tid >> lgM;
-  double acc[MAXPT][4];
+  // 4096 points (DM = 1): the 64 registers of per-thread density accumulators do not fit beside the spinor values (the
+  // corrector spilled 488 bytes per thread): the densities of phi_new are taken by one streaming pass afterwards (oc_launch)
+  constexpr bool NODENS = DM == 1;
+  double acc[NODENS ? 1 : MAXPT][4];
 #pragma unroll
-  for (int kk = 0; kk < MAXPT; ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
+  for (int kk = 0; kk < (NODENS ? 1 : MAXPT); ++kk) { acc[kk][0] = acc[kk][1] = acc[kk][2] = acc[kk][3] = 0.0; }
   // work slots of this thread: w -> (kk = w % PT, s = s0 + (w / PT) * SSTEP), at most OC_SLOTS of them; the spinor
   // values of the slots stay in registers from the load to the last phase (psi is read from HBM exactly once)
   const int nsp_full = DM == 1 ? 1 : S > s0 ? (S - s0 + SSTEP - 1) / SSTEP : 0;
@@ -365,9 +368,9 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
             const double sn = s_sn[sp];
             const cplx u = cscale(ru[w], sn), v = cscale(rv[w], sn);
             a.out[(size_t)(2 * n) * M + i] = u; a.out[(size_t)(2 * n + 1) * M + i] = v;
-            if (a.do_dens) {
+            if (!NODENS && a.do_dens) {
               const double cp = a.cpref[n], wa = a.w_a[n], wb = a.w_b[n], wn = 0.5 * cp * (wb - wa);
-              oc_dens_acc<MAXPT>(acc, w, PT, cp * wa * cabs2(u), cp * wb * cabs2(v), wn * (u.x * v.x + u.y * v.y), wn * (u.y * v.x - u.x * v.y));
+              oc_dens_acc<(NODENS ? 1 : MAXPT)>(acc, w, PT, cp * wa * cabs2(u), cp * wb * cabs2(v), wn * (u.x * v.x + u.y * v.y), wn * (u.y * v.x - u.x * v.y));
             }
           }
         }
@@ -375,11 +378,11 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     }
     __syncthreads();
   }
-  if (MODE == OC_CORR && a.do_dens) {
+  if (!NODENS && MODE == OC_CORR && a.do_dens) {
     const int slots = PT * NT;
     double* dp = a.dpart + (size_t)blockIdx.x * 4 * slots;
 #pragma unroll
-    for (int kk = 0; kk < MAXPT; ++kk)
+    for (int kk = 0; kk < (NODENS ? 1 : MAXPT); ++kk)
       if (kk < PT)
 #pragma unroll
         for (int f = 0; f < 4; ++f) dp[f * slots + tid + NT * kk] = acc[kk][f];
@@ -547,8 +550,12 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   else k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8> : k_onchip_stage<OC_RHS, 8>;
   LAUNCHN(c, mode == OC_APPLY ? "k_onchip_apply" : mode == OC_CORR ? "k_onchip_corr" : "k_onchip_rhs", k, grid, NT, smem, st, a);
   if (mode == OC_CORR && do_dens) {
-    const int slots = (int)(P.M > NT ? P.M : NT);
-    LAUNCH(c, k_oc_dens_final, nb(4 * P.M * 32, 256), 256, 0, st, c->oc_dpart, grid, slots, P.M, c->raw);
+    if (c->oc_dm == 1) {                                     // 64 x 64: one streaming pass over the normalised phi_new
+      dens_chunk(c, out, nullptr, n0, n, WSLDA_D_RHO | WSLDA_D_NU, 0, st);
+    } else {
+      const int slots = (int)(P.M > NT ? P.M : NT);
+      LAUNCH(c, k_oc_dens_final, nb(4 * P.M * 32, 256), 256, 0, st, c->oc_dpart, grid, slots, P.M, c->raw);
+    }
   }
 }
 
