@@ -276,12 +276,13 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order).  CORR leaves
     // X = C_part - i kappa H psi in F (phi_new = X + i kappa eps psi once eps_n is known): C_part is consumed here,
     // four slots at a time so that its loads are in flight together without holding 16 more values in registers.
+    constexpr int WB = DM == 1 ? 2 : 4;                         // slots per batch of loads (4096 points: register budget)
 #pragma unroll
-    for (int w0 = 0; w0 < OC_SLOTS; w0 += 4) {
-      cplx cu[4], cv[4];
+    for (int w0 = 0; w0 < OC_SLOTS; w0 += WB) {
+      cplx cu[WB], cv[WB];
       if (MODE == OC_CORR) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < WB; ++r) {
           const int w = w0 + r;
           if (w < PT * nsp_full) {
             const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
@@ -290,7 +291,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
         }
       }
 #pragma unroll
-      for (int r = 0; r < 4; ++r) {
+      for (int r = 0; r < WB; ++r) {
         const int w = w0 + r;
         if (w < PT * nsp_full) {
           const int i = (tid + NT * (w % PT)) & (M - 1), sp = s0 + (w / PT) * SSTEP;
