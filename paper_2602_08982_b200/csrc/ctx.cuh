@@ -488,6 +488,15 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
           mat[(ax * 2 + 1) * 1024 + i * 32 + k] = 0.5 * (cc[m] - cc[(m + 32) & 63]);
         }
     }
+    {   // fragment order: [axis][Ce | Co][block of 8 rows][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t]: a warp's load is 256 contiguous bytes
+      std::vector<double> fr(mat.size());
+      for (int ae = 0; ae < 4; ++ae)
+        for (int blk = 0; blk < 4; ++blk)
+          for (int kb = 0; kb < 8; ++kb)
+            for (int lane = 0; lane < 32; ++lane)
+              fr[ae * 1024 + (blk * 8 + kb) * 32 + lane] = mat[ae * 1024 + (8 * blk + (lane >> 2)) * 32 + 4 * kb + (lane & 3)];
+      mat.swap(fr);
+    }
     cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
     c->oc_dm = 1;
   }
@@ -507,6 +516,15 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
         mat[i * 64 + k] = 0.5 * (cc[m] + cc[(m + 64) & 127]);
         mat[4096 + i * 64 + k] = 0.5 * (cc[m] - cc[(m + 64) & 127]);
       }
+    {   // fragment order: [Ce | Co][block of 8 columns][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t]
+      std::vector<double> fr(mat.size());
+      for (int eo = 0; eo < 2; ++eo)
+        for (int blk = 0; blk < 8; ++blk)
+          for (int kb = 0; kb < 16; ++kb)
+            for (int lane = 0; lane < 32; ++lane)
+              fr[eo * 4096 + (blk * 16 + kb) * 32 + lane] = mat[eo * 4096 + (8 * blk + (lane >> 2)) * 64 + 4 * kb + (lane & 3)];
+      mat.swap(fr);
+    }
     cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
     c->oc_dm = 2;
   }

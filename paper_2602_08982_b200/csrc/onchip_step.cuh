@@ -87,8 +87,9 @@ __device__ __forceinline__ void oc_dmma(double& c0, double& c1, double a, double
 }
 __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int rb, int cb, double (&out)[2][2][2][2]) {   // [re | im][h][zi][j]
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  const double* mx = mat + (8 * rb + g) * 32 + t;               // rows of Cx (A operand): + eo * 1024 + 4 kb
-  const double* my = mat + 2048 + (8 * cb + g) * 32 + t;        // columns of Cy = its rows (symmetric) (B operand)
+  // matrices in fragment order (ctx.cuh): [axis][Ce | Co][block][k-block][lane]
+  const double* mx = mat + rb * 256 + lane;                     // rows of Cx (A operand): + eo * 1024 + 32 kb
+  const double* my = mat + 2048 + cb * 256 + lane;              // columns of Cy = its rows (symmetric) (B operand)
 #pragma unroll
   for (int zi = 0; zi < 2; ++zi) {                              // contraction along the rows: (d_x^2 w)[i][z]
     const int z = 8 * cb + 32 * zi + g;
@@ -97,7 +98,7 @@ __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int r
     for (int kb = 0; kb < 8; ++kb) {
       const int x1 = 4 * kb + t;
       const cplx w1 = T[oc_ix(0, x1 * 64 + z, 1)], w2 = T[oc_ix(0, (x1 + 32) * 64 + z, 1)];
-      const double me = __ldg(mx + 4 * kb), mo = __ldg(mx + 1024 + 4 * kb);
+      const double me = __ldg(mx + 32 * kb), mo = __ldg(mx + 1024 + 32 * kb);
       oc_dmma(acc[0][0][0], acc[0][0][1], me, w1.x + w2.x); oc_dmma(acc[0][1][0], acc[0][1][1], mo, w1.x - w2.x);
       oc_dmma(acc[1][0][0], acc[1][0][1], me, w1.y + w2.y); oc_dmma(acc[1][1][0], acc[1][1][1], mo, w1.y - w2.y);
     }
@@ -114,7 +115,7 @@ __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int r
     for (int kb = 0; kb < 8; ++kb) {
       const int y1 = 4 * kb + t;
       const cplx w1 = T[oc_ix(0, x * 64 + y1, 1)], w2 = T[oc_ix(0, x * 64 + y1 + 32, 1)];
-      const double me = __ldg(my + 4 * kb), mo = __ldg(my + 1024 + 4 * kb);
+      const double me = __ldg(my + 32 * kb), mo = __ldg(my + 1024 + 32 * kb);
       oc_dmma(acc[0][0][0], acc[0][0][1], w1.x + w2.x, me); oc_dmma(acc[0][1][0], acc[0][1][1], w1.x - w2.x, mo);
       oc_dmma(acc[1][0][0], acc[1][0][1], w1.y + w2.y, me); oc_dmma(acc[1][1][0], acc[1][1][1], w1.y - w2.y, mo);
     }
@@ -154,7 +155,7 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
       const double er = w1.x + w2.x, orr = w1.x - w2.x, ei = w1.y + w2.y, oi = w1.y - w2.y;
 #pragma unroll
       for (int cb = 0; cb < 4; ++cb) {
-        const double* m = mat + (8 * (4 * ch + cb) + g) * 64 + 4 * kb + t;       // symmetric: column = row
+        const double* m = mat + ((4 * ch + cb) * 16 + kb) * 32 + lane;           // fragment order (ctx.cuh); symmetric: column = row
         const double me = __ldg(m), mo = __ldg(m + 4096);
         oc_dmma(acc[cb][0][0][0], acc[cb][0][0][1], er, me); oc_dmma(acc[cb][0][1][0], acc[cb][0][1][1], orr, mo);
         oc_dmma(acc[cb][1][0][0], acc[cb][1][0][1], ei, me); oc_dmma(acc[cb][1][1][0], acc[cb][1][1][1], oi, mo);
