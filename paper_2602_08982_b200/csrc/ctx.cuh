@@ -446,6 +446,15 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
             mat[(ax * 2 + 1) * 256 + i * 16 + k] = 0.5 * (cc[m] - cc[(m + 16) & 31]);
           }
       }
+      {   // fragment order: [axis][Ce | Co][block of 8 rows][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t] (256 contiguous bytes per warp load)
+        std::vector<double> fr(mat.size());
+        for (int ae = 0; ae < 6; ++ae)
+          for (int blk = 0; blk < 2; ++blk)
+            for (int kb = 0; kb < 4; ++kb)
+              for (int lane = 0; lane < 32; ++lane)
+                fr[ae * 256 + (blk * 4 + kb) * 32 + lane] = mat[ae * 256 + (8 * blk + (lane >> 2)) * 16 + 4 * kb + (lane & 3)];
+        mat.swap(fr);
+      }
       cudaMemcpy(c->m_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
       int occ3 = 0, want = g_tune.dmma_ctas > 0 ? g_tune.dmma_ctas : F3M_OCC, got = want;
       bool ok = true;

@@ -95,8 +95,8 @@ __device__ __forceinline__ void f3m_task_p(const cplx* T, const double* AL, cons
   for (int eo = 0; eo < 2; ++eo)
 #pragma unroll
     for (int kb = 0; kb < 4; ++kb) {
-      mA[eo][kb] = mat[(1 * 2 + eo) * 256 + (8 * rb + g) * 16 + 4 * kb + t];
-      mB[eo][kb] = mat[(0 * 2 + eo) * 256 + (8 * cb + g) * 16 + 4 * kb + t];
+      mA[eo][kb] = mat[(1 * 2 + eo) * 256 + (rb * 4 + kb) * 32 + lane];         // fragment order (ctx.cuh): [axis][Ce | Co][block][k-block][lane]
+      mB[eo][kb] = mat[(0 * 2 + eo) * 256 + (cb * 4 + kb) * 32 + lane];
     }
   double out[2][2][2][2][2];                            // [field w | alpha w][re | im][row half][col half][j]
   // d_y^2: A = Ce / Co rows, B = folded data W[k = y][n = z]
@@ -201,7 +201,7 @@ __device__ __forceinline__ void f3m_body_xe(const F3MMega& A, const F3Pol& pol, 
 #pragma unroll
   for (int eo = 0; eo < 2; ++eo)
 #pragma unroll
-    for (int kb = 0; kb < 4; ++kb) mA[eo][kb] = A.mat[(2 * 2 + eo) * 256 + (8 * rb + gq) * 16 + 4 * kb + t];
+    for (int kb = 0; kb < 4; ++kb) mA[eo][kb] = A.mat[(2 * 2 + eo) * 256 + (rb * 4 + kb) * 32 + lane];
   const cplx* Tu = reinterpret_cast<const cplx*>(buf);
   const cplx* Tv = reinterpret_cast<const cplx*>(buf + F3M_PSI_BYTES);
   const double* ALa = reinterpret_cast<const double*>(buf + 2 * F3M_PSI_BYTES);
