@@ -110,8 +110,9 @@ typedef struct {
                                a wait that runs out makes every later call return WSLDA_ECUDA                       */
   int tma_group, tma_block, tma_ring, tma_lag;   /* mega3t: spinors per group (8), per block (2), ring depth in blocks (20),
                                ticks between the P, X, E items of a block (5)                                       */
-  int dmma_stage;           /* 32^3, Eq. 40: line derivatives in the matrix form of Eq. 28b on FP64 tensor instructions
-                               (mega3m); 0 = library default (on), 1 = on, -1 = off: the register-FFT kernel mega3s                                     */
+  int dmma_stage;           /* line derivatives in the matrix form of Eq. 28b on FP64 tensor instructions: the 32^3 Eq. 40
+                               stage kernels (mega3m) and the on-chip stage kernels for lines of 128 points and 64 x 64
+                               lattices; 0 = library default (on), 1 = on, -1 = off: register / shared-memory FFT kernels */
   int dmma_ctas;            /* mega3m: resident CTAs per SM (default 3)                                             */
 } wslda_tuning;
 wslda_status wslda_set_tuning(const wslda_tuning* t);
