@@ -510,30 +510,27 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->oc_dm = 1;
   }
   if (P.oc && P.nd == 1 && P.N[0] == 128 && P.ocS * 2 <= 32 && g_tune.dmma_stage >= 0) {
-    // lines of 128 points: [Ce | Co][64][64]
+    // lines of 128 points, folded twice (onchip_step.cuh oc_lap128): Co [64][64], Cee, Ceo [32][32], in fragment order
     c->oc_mat = (double*)(base + P.off_oc + P.oc_dpart_bytes);
-    std::vector<double> mat(2 * 4096);
-    const double* k2 = c->hk2[0];              // (only the first 64 entries are kept on the host: rebuild the table)
-    double kk2[128];
+    double kk2[128], cc[128], ce[64];
     for (int q = 0; q < 128; ++q) { const double len = 128 * c->dx[0]; const double k = (q < 64) ? 2.0 * PI * q / len : 2.0 * PI * (q - 128) / len; kk2[q] = k * k; }
-    (void)k2;
-    double cc[128];
     for (int m = 0; m < 128; ++m) { double t = 0.0; for (int q = 0; q < 128; ++q) t -= kk2[q] * cos(2.0 * PI * ((q * m) & 127) / 128.0); cc[m] = t / 128.0; }
-    for (int i = 0; i < 64; ++i)
-      for (int k = 0; k < 64; ++k) {
-        const int m = (i - k) & 127;
-        mat[i * 64 + k] = 0.5 * (cc[m] + cc[(m + 64) & 127]);
-        mat[4096 + i * 64 + k] = 0.5 * (cc[m] - cc[(m + 64) & 127]);
-      }
-    {   // fragment order: [Ce | Co][block of 8 columns][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t]
-      std::vector<double> fr(mat.size());
-      for (int eo = 0; eo < 2; ++eo)
-        for (int blk = 0; blk < 8; ++blk)
-          for (int kb = 0; kb < 16; ++kb)
-            for (int lane = 0; lane < 32; ++lane)
-              fr[eo * 4096 + (blk * 16 + kb) * 32 + lane] = mat[eo * 4096 + (8 * blk + (lane >> 2)) * 64 + 4 * kb + (lane & 3)];
-      mat.swap(fr);
-    }
+    for (int m = 0; m < 64; ++m) ce[m] = 0.5 * (cc[m] + cc[m + 64]);        // the even part's circulant (period 64), 1/2 of the first fold
+    std::vector<double> mat(4096 + 2 * 1024);
+    // fragment order: [block of 8 columns][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t] (symmetric matrices: column = row)
+    for (int blk = 0; blk < 8; ++blk)
+      for (int kb = 0; kb < 16; ++kb)
+        for (int lane = 0; lane < 32; ++lane) {
+          const int i = 8 * blk + (lane >> 2), k = 4 * kb + (lane & 3), m = (i - k) & 127;
+          mat[(blk * 16 + kb) * 32 + lane] = 0.5 * (cc[m] - cc[(m + 64) & 127]);
+        }
+    for (int blk = 0; blk < 4; ++blk)
+      for (int kb = 0; kb < 8; ++kb)
+        for (int lane = 0; lane < 32; ++lane) {
+          const int i = 8 * blk + (lane >> 2), k = 4 * kb + (lane & 3), m = (i - k) & 63;
+          mat[4096 + (blk * 8 + kb) * 32 + lane] = 0.5 * (ce[m] + ce[(m + 32) & 63]);
+          mat[5120 + (blk * 8 + kb) * 32 + lane] = 0.5 * (ce[m] - ce[(m + 32) & 63]);
+        }
     cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
     c->oc_dm = 2;
   }

@@ -137,28 +137,41 @@ __device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const do
 }
 
 // ---- lines of 128 points (quasi-1D, configs[1]): d^2 as the folded matrices Ce, Co (64 x 64) of Eq. 28b.  The batch is a
-// matrix [lines][128]: the lines are the rows of the A operand, the matrix is the B operand.  Warp = (block of 8 lines, half
-// of the 64 folded columns): 4 x 16 k-blocks, results in fragments until every warp has read its lines, then in place.
+// matrix [lines][128]: the lines are the rows of the A operand, the matrices are the B operand.  Warp = (block of 8 lines, half
+// of the folded columns), results in fragments until every warp has read its lines, then in place.
 // Element i of line l is stored at oc_ix(l, i, 2).  Contains its two barriers.
 __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines) {
+  // two folds: e = w[k] + w[k+64], o = w[k] - w[k+64] (k < 64); the even part is again a symmetric circulant (period 64):
+  // ee = e[k] + e[k+32], eo = e[k] - e[k+32] (k < 32).  O = Co o (64 x 64), EE = Cee ee, EO = Ceo eo (32 x 32);
+  // E[i] = EE[i] + EO[i], E[i+32] = EE[i] - EO[i] (i < 32); out[i] = E[i] + O[i], out[i+64] = E[i] - O[i] (i < 64):
+  // 6144 instead of 8192 multiply-adds per real line.  mat (fragment order, ctx.cuh): Co [8 blocks][16 kb][32],
+  // then Cee, Ceo [4 blocks][8 kb][32] each.
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
   const bool active = 8 * lb < lines;                           // (whole warp)
   const cplx* T = F + line * 128;
   const int sw = (line & 1) << 2;
-  double acc[4][2][2][2] = {};                                  // [column block][re | im][E | O][j]
+  double aO[4][2][2] = {}, aE[2][2][2][2] = {};                 // O: [b, b+1, b+4, b+5][re | im][j]; E: [b, b+1][EE | EO][re | im][j]
+  const int b0 = 2 * ch;                                        // this warp's column blocks of the twice-folded part: b0, b0 + 1
   if (active) {
-#pragma unroll 4
-    for (int kb = 0; kb < 16; ++kb) {
+#pragma unroll 2
+    for (int kb = 0; kb < 8; ++kb) {
       const int k1 = (4 * kb + t) ^ sw;
-      const cplx w1 = T[k1], w2 = T[k1 + 64];
-      const double er = w1.x + w2.x, orr = w1.x - w2.x, ei = w1.y + w2.y, oi = w1.y - w2.y;
+      const cplx w0 = T[k1], w1 = T[k1 + 32], w2 = T[k1 + 64], w3 = T[k1 + 96];
+      const cplx e0 = cadd(w0, w2), e1 = cadd(w1, w3), o0 = csub(w0, w2), o1 = csub(w1, w3);   // e[k], e[k+32], o[k], o[k+32]
+      const cplx ee = cadd(e0, e1), eo = csub(e0, e1);
 #pragma unroll
-      for (int cb = 0; cb < 4; ++cb) {
-        const double* m = mat + ((4 * ch + cb) * 16 + kb) * 32 + lane;           // fragment order (ctx.cuh); symmetric: column = row
-        const double me = __ldg(m), mo = __ldg(m + 4096);
-        oc_dmma(acc[cb][0][0][0], acc[cb][0][0][1], er, me); oc_dmma(acc[cb][0][1][0], acc[cb][0][1][1], orr, mo);
-        oc_dmma(acc[cb][1][0][0], acc[cb][1][0][1], ei, me); oc_dmma(acc[cb][1][1][0], acc[cb][1][1][1], oi, mo);
+      for (int q = 0; q < 4; ++q) {                             // O part: column blocks b0, b0 + 1, b0 + 4, b0 + 5; k-blocks kb and kb + 8
+        const int cbb = b0 + (q & 1) + 4 * (q >> 1);
+        const double m0 = __ldg(mat + (cbb * 16 + kb) * 32 + lane), m1 = __ldg(mat + (cbb * 16 + kb + 8) * 32 + lane);
+        oc_dmma(aO[q][0][0], aO[q][0][1], o0.x, m0); oc_dmma(aO[q][1][0], aO[q][1][1], o0.y, m0);
+        oc_dmma(aO[q][0][0], aO[q][0][1], o1.x, m1); oc_dmma(aO[q][1][0], aO[q][1][1], o1.y, m1);
+      }
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {                             // EE, EO: column blocks b0, b0 + 1 of 4; k-block kb of 8
+        const double mee = __ldg(mat + 4096 + ((b0 + q) * 8 + kb) * 32 + lane), meo = __ldg(mat + 5120 + ((b0 + q) * 8 + kb) * 32 + lane);
+        oc_dmma(aE[q][0][0][0], aE[q][0][0][1], ee.x, mee); oc_dmma(aE[q][0][1][0], aE[q][0][1][1], ee.y, mee);
+        oc_dmma(aE[q][1][0][0], aE[q][1][0][1], eo.x, meo); oc_dmma(aE[q][1][1][0], aE[q][1][1][1], eo.y, meo);
       }
     }
   }
@@ -166,12 +179,15 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
   if (active) {
     cplx* W = F + line * 128;
 #pragma unroll
-    for (int cb = 0; cb < 4; ++cb)
+    for (int q = 0; q < 2; ++q)
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int i = 8 * (4 * ch + cb) + 2 * t + j;
-        W[i ^ sw] = make_double2(acc[cb][0][0][j] + acc[cb][0][1][j], acc[cb][1][0][j] + acc[cb][1][1][j]);
-        W[(i ^ sw) + 64] = make_double2(acc[cb][0][0][j] - acc[cb][0][1][j], acc[cb][1][0][j] - acc[cb][1][1][j]);
+        const int i = (8 * (b0 + q) + 2 * t + j) ^ sw;            // i < 32
+        const cplx EE = make_double2(aE[q][0][0][j], aE[q][0][1][j]), EO = make_double2(aE[q][1][0][j], aE[q][1][1][j]);
+        const cplx Elo = cadd(EE, EO), Ehi = csub(EE, EO);       // E[i], E[i + 32]
+        const cplx Olo = make_double2(aO[q][0][j], aO[q][1][j]), Ohi = make_double2(aO[q + 2][0][j], aO[q + 2][1][j]);   // O[i], O[i + 32]
+        W[i] = cadd(Elo, Olo); W[i + 64] = csub(Elo, Olo);
+        W[i + 32] = cadd(Ehi, Ohi); W[i + 96] = csub(Ehi, Ohi);
       }
   }
   __syncthreads();
