@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     // ---- phase 1: H psi and the integrand of eps_n (F now holds lap u, lap v in natural order).  CORR leaves
     // X = C_part - i kappa H psi in F (phi_new = X + i kappa eps psi once eps_n is known): C_part is consumed here,
     // four slots at a time so that its loads are in flight together without holding 16 more values in registers.
-    constexpr int WB = DM == 1 ? 2 : 4;                         // slots per batch of loads (4096 points: register budget)
+    constexpr int WB = DM ? 2 : 4;                              // slots per batch of loads (4096 points: register budget)
 #pragma unroll
     for (int w0 = 0; w0 < OC_SLOTS; w0 += WB) {
       cplx cu[WB], cv[WB];
