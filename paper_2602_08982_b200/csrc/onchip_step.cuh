@@ -149,7 +149,8 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
   const bool active = 8 * lb < lines;                           // (whole warp)
-  const cplx* T = F + line * 128;
+  const bool lv = line < lines;                                 // a ragged last batch: lines beyond it are neither read nor written
+  const cplx* T = F + (lv ? line : 0) * 128;
   const int sw = (line & 1) << 2;
   double aO[4][2][2] = {}, aE[2][2][2][2] = {};                 // O: [b, b+1, b+4, b+5][re | im][j]; E: [b, b+1][EE | EO][re | im][j]
   const int b0 = 2 * ch;                                        // this warp's column blocks of the twice-folded part: b0, b0 + 1
@@ -157,7 +158,8 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
 #pragma unroll 2
     for (int kb = 0; kb < 8; ++kb) {
       const int k1 = (4 * kb + t) ^ sw;
-      const cplx w0 = T[k1], w1 = T[k1 + 32], w2 = T[k1 + 64], w3 = T[k1 + 96];
+      const cplx zero = make_double2(0.0, 0.0);
+      const cplx w0 = lv ? T[k1] : zero, w1 = lv ? T[k1 + 32] : zero, w2 = lv ? T[k1 + 64] : zero, w3 = lv ? T[k1 + 96] : zero;
       const cplx e0 = cadd(w0, w2), e1 = cadd(w1, w3), o0 = csub(w0, w2), o1 = csub(w1, w3);   // e[k], e[k+32], o[k], o[k+32]
       const cplx ee = cadd(e0, e1), eo = csub(e0, e1);
 #pragma unroll
@@ -176,7 +178,7 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
     }
   }
   __syncthreads();
-  if (active) {
+  if (active && lv) {
     cplx* W = F + line * 128;
 #pragma unroll
     for (int q = 0; q < 2; ++q)

@@ -318,6 +318,34 @@ def test_dmma_stage_kernel_32cubed(tuning, nwf, pm, em, ctas):
     assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names and "k_f3s_mega_corr" not in names
 
 
+@pytest.mark.parametrize("shape,dx,nwf", [((128,), (0.9,), 5), ((128,), (1.0,), 19), ((128,), (1.1,), 37), ((64, 64), (1.0, 0.9), 3)])
+@pytest.mark.parametrize("dmma", [0, -1])
+def test_onchip_matrix_form_cores_with_ragged_batches(tuning, shape, dx, nwf, dmma):
+    """The on-chip stage kernels with the matrix-form (Eq. 28b, DMMA) core and with the FFT core (dmma_stage = -1) on the two
+    shapes the matrix form covers, with batches that do not fill the CTA (lines of 128: 16 spinors per batch): H psi with
+    eps_n, a sub-range, self-consistent steps; the kernels really ran."""
+    tuning(dmma_stage=dmma)
+    w = generic(shape, dx, nwf, 0, func_id=2, force_a1=1, n_modes=3, dt=0.004)     # SLDA with alpha = 1: the step rebuilds rho and nu only
+    psi0 = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi0)
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    h2, _ = g.apply_h(to_gpu(psi0), n_first=1, n_count=2)
+    h2 = to_np(h2)
+    assert relerr(h2[1:3], ref[1:3]) < TOL_H and not h2[:1].any() and not h2[3:].any()
+    pg, po, fg, fo, o, g = run_both(w, psi0, 3)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("delta", "U_a", "rho_a", "rho_b", "nu"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_onchip_corr" in names and "k_onchip_rhs" in names and "k_onchip_pred" in names
+
+
 @pytest.mark.parametrize("which", ["mega3s_32", "mega3d_16", "mega64", "tma_32", "dmma_32"])
 def test_persistent_kernels_bit_reproducible(tuning, which):
     """The ticketed persistent kernels hand items to whichever CTA is free, but every sum is taken in a fixed order
