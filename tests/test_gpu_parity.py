@@ -318,6 +318,22 @@ def test_dmma_stage_kernel_32cubed(tuning, nwf, pm, em, ctas):
     assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names and "k_f3s_mega_corr" not in names
 
 
+def test_dmma_stage_kernel_anisotropic_spacings(tuning):
+    """mega3m with three different lattice spacings (each axis has its own folded matrices: a swapped pair would pass every
+    isotropic test) and fixed random fields with alpha_a != alpha_b: H psi, eps_n and ABM steps against the oracle."""
+    tuning(dmma_stage=1)
+    w = generic((32, 32, 32), (1.0, 0.85, 1.2), 9, 1, func_id=0, dt=0.004)
+    psi0 = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    ref, eref = o.apply_h(psi0)
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    pg, po, fg, fo, o, g = run_both(w, psi0, 3)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    names = _kernels_of(g, lambda: g.apply_h(to_gpu(psi0)))
+    assert "k_f3m_mega_apply" in names
+
+
 @pytest.mark.parametrize("shape,dx,nwf", [((128,), (0.9,), 5), ((128,), (1.0,), 19), ((128,), (1.1,), 37), ((64, 64), (1.0, 0.9), 3)])
 @pytest.mark.parametrize("dmma", [0, -1])
 def test_onchip_matrix_form_cores_with_ragged_batches(tuning, shape, dx, nwf, dmma):
