@@ -30,7 +30,7 @@ METRIC = "qp_wavefunction_time_steps_per_s"
 UNIT = "spinor-steps/s"
 
 
-def make_workload(name, n_wf=None):
+def make_workload(name, n_wf=None, kin_form=None):
     if name == "cfg1":
         return wl.cfg1(n_wf), "configs[0]: 3D BdG 8^3, fixed potentials, AB4AM4"
     if name == "cfg2":
@@ -40,6 +40,9 @@ def make_workload(name, n_wf=None):
         w = wl.cfg3()
         return w, "configs[2]: quasi-2D SLDA vortex 64^2 x 16 kz, self-consistent, AB4AM5"
     if name == "cfg4":
+        if kin_form in (0, 2):           # the other discretisations of the kinetic term on the same workload (comparison lines)
+            form = {0: "Eq.14 Laplacian operator (alpha treated as 1 in the kinetic term)", 2: "DIVGRAD operator (3 gradient + 3 divergence transforms; general path)"}[kin_form]
+            return wl.cfg4(n_wf=n_wf, kin_form=kin_form), f"configs[3] variant: 3D SLDA 32^3 trap, {form}, self-consistent, AB4AM5"
         return wl.cfg4(n_wf=n_wf), "configs[3]: 3D SLDA 32^3 trap, general-alpha Eq.40 operator, self-consistent, AB4AM5"
     if name == "cfg5":
         return wl.cfg5(n_wf=n_wf or 2048), "configs[4]: 3D ASLDA-like 64^3, h_a != h_b, fixed smooth potentials, AB4AM5"
@@ -162,7 +165,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w, desc = make_workload(args.config, args.n_wf)
+    w, desc = make_workload(args.config, args.n_wf, args.kin_form)
     import oracle as orc
     orc.build()
     cal, _ = time_oracle(w, budget_s=4.0, steps=1)                 # calibration: spinor-steps/s
@@ -227,7 +230,7 @@ def run_gpu(args):
         dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29655", rank=0, world_size=1,
                                 device_id=torch.device("cuda", local))
     ws.build()
-    w, desc = make_workload(args.config, args.n_wf)
+    w, desc = make_workload(args.config, args.n_wf, args.kin_form)
     w_full, n_lo = w, 0
     if args.shard:                                     # shard the spinor index, all-reduce the densities
         n_lo, n_hi = wl.shard_range(w_full.n_wf, rank, world)
@@ -517,6 +520,8 @@ def main():
     ap.add_argument("--impl", default="wslda", choices=["wslda", "reference"])
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--n-wf", type=int, default=None)
+    ap.add_argument("--kin-form", type=int, default=None, choices=[0, 1, 2],
+                    help="cfg4 only: time another discretisation of the kinetic term (0 Eq. 14, 2 DIVGRAD) instead of Eq. 40")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
