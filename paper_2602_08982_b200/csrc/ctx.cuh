@@ -149,7 +149,9 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
-  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->current_terms && !f->quantum_friction;
+  // (the current / velocity coupling is fused only where the matrix-form core exists for it: 64 x 64)
+  P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->quantum_friction &&
+         (!f->current_terms || (mode == 2 && P.N[0] == 64 && P.N[1] == 64 && g_tune.dmma_stage >= 0));
   if (g_tune.disable_onchip) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
   { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
@@ -497,9 +499,26 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
           mat[(ax * 2 + 1) * 1024 + i * 32 + k] = 0.5 * (cc[m] - cc[(m + 32) & 63]);
         }
     }
+    // first-derivative matrices for the current / velocity coupling (odd derivative: Nyquist mode dropped), same folding
+    mat.resize(2 * 2 * 1024 * 2);
+    for (int ax = 0; ax < 2; ++ax) {
+      const double len = 64 * c->dx[ax];
+      double cc[64];
+      for (int m = 0; m < 64; ++m) {
+        double t = 0.0;
+        for (int q = 1; q < 64; ++q) { if (q == 32) continue; const double k = q < 32 ? 2.0 * PI * q / len : 2.0 * PI * (q - 64) / len; t -= k * sin(2.0 * PI * ((q * m) & 63) / 64.0); }
+        cc[m] = t / 64.0;
+      }
+      for (int i = 0; i < 32; ++i)
+        for (int k = 0; k < 32; ++k) {
+          const int m = (i - k) & 63;
+          mat[4096 + (ax * 2 + 0) * 1024 + i * 32 + k] = 0.5 * (cc[m] + cc[(m + 32) & 63]);
+          mat[4096 + (ax * 2 + 1) * 1024 + i * 32 + k] = 0.5 * (cc[m] - cc[(m + 32) & 63]);
+        }
+    }
     {   // fragment order: [axis][Ce | Co][block of 8 rows][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t]: a warp's load is 256 contiguous bytes
       std::vector<double> fr(mat.size());
-      for (int ae = 0; ae < 4; ++ae)
+      for (int ae = 0; ae < 8; ++ae)
         for (int blk = 0; blk < 4; ++blk)
           for (int kb = 0; kb < 8; ++kb)
             for (int lane = 0; lane < 32; ++lane)

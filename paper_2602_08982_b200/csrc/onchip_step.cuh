@@ -32,6 +32,7 @@ struct OCArgs {
   int64_t n;
   int S;
   int dm;                      // 64 x 64: Laplacian in matrix form on DMMA (storage index swizzled: oc_ix)
+  const double* curW;          // current / velocity coupling (DM = 1 only): W_sigma,d = A_sigma,d - v_ext,sigma,d, [2][3][M]; nullable
   const double* mat;           // [axis][Ce | Co][32][32]
 };
 
@@ -125,6 +126,69 @@ __device__ __forceinline__ void oc_lap64(const cplx* T, const double* mat, int r
       for (int j = 0; j < 2; ++j) { out[p][h][0][j] += acc[p][0][j] + acc[p][1][j]; out[p][h][1][j] += acc[p][0][j] - acc[p][1][j]; }
   }
 }
+// The current / velocity coupling of Eq. 4c in the Hermitian form of DESIGN R27 on the same tile: adds
+//   rot * [ W_x (D_x w) + D_x (W_x w) + W_y (D_y w) + D_y (W_y w) ]
+// to `out`, D_d the spectral FIRST derivative as a folded circulant (odd derivative: Nyquist mode dropped),
+// W_d real fields [64][64] in global memory (L1 / L2).  rot = +i (sgn = +1: component u, so that -1/2 out carries
+// -(i/2){W, grad} u) or -i (sgn = -1: component v, whose coupling enters -h_b^* with the opposite sign).
+__device__ __forceinline__ void oc_cur64(const cplx* T, const double* mat1, const double* Wx, const double* Wy, int rb, int cb, double sgn,
+                                         double (&out)[2][2][2][2]) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const double* mx = mat1 + rb * 256 + lane;
+  const double* my = mat1 + 2048 + cb * 256 + lane;
+#pragma unroll
+  for (int zi = 0; zi < 2; ++zi) {                              // along the rows: D_x
+    const int z = 8 * cb + 32 * zi + g;
+    double aG[2][2][2] = {}, aH[2][2][2] = {};                  // [re | im][E | O][j]: D_x w and D_x (W_x w)
+#pragma unroll
+    for (int kb = 0; kb < 8; ++kb) {
+      const int x1 = 4 * kb + t;
+      const cplx w1 = T[oc_ix(0, x1 * 64 + z, 1)], w2 = T[oc_ix(0, (x1 + 32) * 64 + z, 1)];
+      const cplx h1 = cscale(w1, __ldg(Wx + x1 * 64 + z)), h2 = cscale(w2, __ldg(Wx + (x1 + 32) * 64 + z));
+      const double me = __ldg(mx + 32 * kb), mo = __ldg(mx + 1024 + 32 * kb);
+      oc_dmma(aG[0][0][0], aG[0][0][1], me, w1.x + w2.x); oc_dmma(aG[0][1][0], aG[0][1][1], mo, w1.x - w2.x);
+      oc_dmma(aG[1][0][0], aG[1][0][1], me, w1.y + w2.y); oc_dmma(aG[1][1][0], aG[1][1][1], mo, w1.y - w2.y);
+      oc_dmma(aH[0][0][0], aH[0][0][1], me, h1.x + h2.x); oc_dmma(aH[0][1][0], aH[0][1][1], mo, h1.x - h2.x);
+      oc_dmma(aH[1][0][0], aH[1][0][1], me, h1.y + h2.y); oc_dmma(aH[1][1][0], aH[1][1][1], mo, h1.y - h2.y);
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const double sg = h ? -1.0 : 1.0;
+        const double wv = __ldg(Wx + (8 * rb + 32 * h + g) * 64 + 8 * cb + 32 * zi + 2 * t + j);
+        const double tr = wv * (aG[0][0][j] + sg * aG[0][1][j]) + (aH[0][0][j] + sg * aH[0][1][j]);
+        const double ti = wv * (aG[1][0][j] + sg * aG[1][1][j]) + (aH[1][0][j] + sg * aH[1][1][j]);
+        out[0][h][zi][j] -= sgn * ti; out[1][h][zi][j] += sgn * tr;                 // (+-i) (tr + i ti)
+      }
+  }
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {                                 // along the columns: D_y
+    const int x = 8 * rb + 32 * h + g;
+    double aG[2][2][2] = {}, aH[2][2][2] = {};
+#pragma unroll
+    for (int kb = 0; kb < 8; ++kb) {
+      const int y1 = 4 * kb + t;
+      const cplx w1 = T[oc_ix(0, x * 64 + y1, 1)], w2 = T[oc_ix(0, x * 64 + y1 + 32, 1)];
+      const cplx h1 = cscale(w1, __ldg(Wy + x * 64 + y1)), h2 = cscale(w2, __ldg(Wy + x * 64 + y1 + 32));
+      const double me = __ldg(my + 32 * kb), mo = __ldg(my + 1024 + 32 * kb);
+      oc_dmma(aG[0][0][0], aG[0][0][1], w1.x + w2.x, me); oc_dmma(aG[0][1][0], aG[0][1][1], w1.x - w2.x, mo);
+      oc_dmma(aG[1][0][0], aG[1][0][1], w1.y + w2.y, me); oc_dmma(aG[1][1][0], aG[1][1][1], w1.y - w2.y, mo);
+      oc_dmma(aH[0][0][0], aH[0][0][1], h1.x + h2.x, me); oc_dmma(aH[0][1][0], aH[0][1][1], h1.x - h2.x, mo);
+      oc_dmma(aH[1][0][0], aH[1][0][1], h1.y + h2.y, me); oc_dmma(aH[1][1][0], aH[1][1][1], h1.y - h2.y, mo);
+    }
+#pragma unroll
+    for (int zi = 0; zi < 2; ++zi)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const double sg = zi ? -1.0 : 1.0;
+        const double wv = __ldg(Wy + x * 64 + 8 * cb + 32 * zi + 2 * t + j);
+        const double tr = wv * (aG[0][0][j] + sg * aG[0][1][j]) + (aH[0][0][j] + sg * aH[0][1][j]);
+        const double ti = wv * (aG[1][0][j] + sg * aG[1][1][j]) + (aH[1][0][j] + sg * aH[1][1][j]);
+        out[0][h][zi][j] -= sgn * ti; out[1][h][zi][j] += sgn * tr;
+      }
+  }
+}
 __device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const double (&out)[2][2][2][2]) {
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
 #pragma unroll
@@ -195,7 +259,7 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
   __syncthreads();
 }
 
-template <int MODE, int MAXPT, int DM = 0>
+template <int MODE, int MAXPT, int DM = 0, bool CUR = false>
 __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_onchip_stage(OCArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Lat& L = a.L;
@@ -261,6 +325,10 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
       for (int q = 0; q < 2 * cnt; ++q) {
         double lap[2][2][2][2];
         oc_lap64(F + (size_t)q * M, a.mat, rb, cb, lap);
+        if (CUR) {                                              // lap - 2 (+-) cur(w): the stage's K = -1/2 (.) then carries the coupling
+          const double* W = a.curW + (size_t)(q & 1) * 3 * M;
+          oc_cur64(F + (size_t)q * M, a.mat + 4096, W, W + M, rb, cb, (q & 1) ? -1.0 : 1.0, lap);
+        }
         __syncthreads();
         oc_lap64_store(F + (size_t)q * M, rb, cb, lap);
       }
@@ -540,7 +608,7 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   a.out = out; a.cpart = cpart; a.kappa = kappa; a.dV = c->dV;
   a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.eps_out = eps_user;
   a.do_dens = do_dens; a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.dpart = c->oc_dpart;
-  a.n = n; a.S = P.ocS; a.dm = c->oc_dm; a.mat = c->oc_mat;
+  a.n = n; a.S = P.ocS; a.dm = c->oc_dm; a.mat = c->oc_mat; a.curW = (c->f.current_terms && c->oc_dm == 1) ? c->cur_W : nullptr;
   const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
   if (!g_oc_attr_done) {
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -552,6 +620,9 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -566,6 +637,7 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   void (*k)(OCArgs);
   if (small && c->oc_dm == 2) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2, 2> : k_onchip_stage<OC_RHS, 2, 2>;
   else if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
+  else if (c->oc_dm == 1 && a.curW) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, 1, true> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, 1, true> : k_onchip_stage<OC_RHS, 8, 1, true>;
   else if (c->oc_dm == 1) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, 1> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, 1> : k_onchip_stage<OC_RHS, 8, 1>;
   else k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8> : k_onchip_stage<OC_RHS, 8>;
   LAUNCHN(c, mode == OC_APPLY ? "k_onchip_apply" : mode == OC_CORR ? "k_onchip_corr" : "k_onchip_rhs", k, grid, NT, smem, st, a);
