@@ -166,6 +166,12 @@ def run_reference(args):
     if rank != 0:
         return
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "velocity", 0.0):
+        Mv, ndv = int(np.prod(w.shape)), len(w.shape)
+        vv = args.velocity * wl.normal(977, 0, 6 * Mv).reshape(2, 3, *w.shape)
+        w.current_terms = 1
+        w.vel = (vv[0, :ndv], vv[1, :ndv])
+        desc += f" + external velocity fields (amplitude {args.velocity}) through the coupling of Eq. 4c"
     import oracle as orc
     orc.build()
     cal, _ = time_oracle(w, budget_s=4.0, steps=1)                 # calibration: spinor-steps/s
@@ -231,6 +237,12 @@ def run_gpu(args):
                                 device_id=torch.device("cuda", local))
     ws.build()
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "velocity", 0.0):
+        Mv, ndv = int(np.prod(w.shape)), len(w.shape)
+        vv = args.velocity * wl.normal(977, 0, 6 * Mv).reshape(2, 3, *w.shape)
+        w.current_terms = 1
+        w.vel = (vv[0, :ndv], vv[1, :ndv])
+        desc += f" + external velocity fields (amplitude {args.velocity}) through the coupling of Eq. 4c"
     w_full, n_lo = w, 0
     if args.shard:                                     # shard the spinor index, all-reduce the densities
         n_lo, n_hi = wl.shard_range(w_full.n_wf, rank, world)
@@ -522,6 +534,8 @@ def main():
     ap.add_argument("--n-wf", type=int, default=None)
     ap.add_argument("--kin-form", type=int, default=None, choices=[0, 1, 2],
                     help="cfg4 only: time another discretisation of the kinetic term (0 Eq. 14, 2 DIVGRAD) instead of Eq. 40")
+    ap.add_argument("--velocity", type=float, default=0.0,
+                    help="add seeded external velocity fields of this amplitude (NEXT-1 current / velocity coupling, Eq. 4c) to the workload")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
