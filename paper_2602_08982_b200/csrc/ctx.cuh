@@ -149,16 +149,16 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.f6_partn_bytes = align_up((size_t)n_wf * P.nblk * 8);       // norm partials of a whole-batch predictor launch
     o += 3 * P.f6_ring_bytes + P.f6_part_bytes + P.f6_acc_bytes + P.f6_sync_bytes + P.f6_pack_bytes + P.f6_partn_bytes;
   }
-  // (the current / velocity coupling is fused only where the matrix-form core exists for it: 64 x 64)
+  // (the current / velocity coupling is fused only where the matrix-form core exists for it: 64 x 64 and lines of 128)
   P.oc = P.onchip && f->kin_form == WSLDA_KIN_LAPLACE && !f->quantum_friction &&
-         (!f->current_terms || (mode == 2 && P.N[0] == 64 && P.N[1] == 64 && g_tune.dmma_stage >= 0));
+         (!f->current_terms || (g_tune.dmma_stage >= 0 && ((mode == 2 && P.N[0] == 64 && P.N[1] == 64) || (mode == 1 && P.N[0] == 128))));
   if (g_tune.disable_onchip) P.oc = 0;
   // batch: 64 KB of spinors per CTA (two CTAs per SM) up to 512 points, one spinor per CTA above
   { int64_t S = (M <= 512 ? 4096 : 8192) / (2 * M); if (S < 1) S = 1; if (S > 64) S = 64; if (S > n_wf) S = n_wf; P.ocS = (int)S; }
   { int64_t nb_ = (n_wf + P.ocS - 1) / P.ocS, cap = M <= 512 ? 296 : 148; P.oc_grid = (int)(nb_ < cap ? nb_ : cap); }
   if (g_tune.onchip_ctas > 0 && g_tune.onchip_ctas < P.oc_grid) P.oc_grid = g_tune.onchip_ctas;
   P.off_oc = o; P.oc_dpart_bytes = 0;
-  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes + 65536; }   // + folded derivative matrices
+  if (P.oc) { P.oc_dpart_bytes = align_up((size_t)P.oc_grid * 4 * (M > 512 ? M : 512) * 8); o += P.oc_dpart_bytes + 131072; }   // + folded derivative matrices (second and first derivative)
   P.total = o;
   return 0;
 }
@@ -535,7 +535,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     for (int q = 0; q < 128; ++q) { const double len = 128 * c->dx[0]; const double k = (q < 64) ? 2.0 * PI * q / len : 2.0 * PI * (q - 128) / len; kk2[q] = k * k; }
     for (int m = 0; m < 128; ++m) { double t = 0.0; for (int q = 0; q < 128; ++q) t -= kk2[q] * cos(2.0 * PI * ((q * m) & 127) / 128.0); cc[m] = t / 128.0; }
     for (int m = 0; m < 64; ++m) ce[m] = 0.5 * (cc[m] + cc[m + 64]);        // the even part's circulant (period 64), 1/2 of the first fold
-    std::vector<double> mat(4096 + 2 * 1024);
+    std::vector<double> mat(4096 + 2 * 1024 + 2 * 4096);
     // fragment order: [block of 8 columns][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t] (symmetric matrices: column = row)
     for (int blk = 0; blk < 8; ++blk)
       for (int kb = 0; kb < 16; ++kb)
@@ -550,6 +550,22 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
           mat[4096 + (blk * 8 + kb) * 32 + lane] = 0.5 * (ce[m] + ce[(m + 32) & 63]);
           mat[5120 + (blk * 8 + kb) * 32 + lane] = 0.5 * (ce[m] - ce[(m + 32) & 63]);
         }
+    {   // first derivative (odd: Nyquist mode dropped), folded once: De, Do [8 blocks][16 kb][32] at 6144 and 10240
+      double d1[128];
+      const double len = 128 * c->dx[0];
+      for (int m = 0; m < 128; ++m) {
+        double t = 0.0;
+        for (int q = 1; q < 128; ++q) { if (q == 64) continue; const double k = q < 64 ? 2.0 * PI * q / len : 2.0 * PI * (q - 128) / len; t -= k * sin(2.0 * PI * ((q * m) & 127) / 128.0); }
+        d1[m] = t / 128.0;
+      }
+      for (int blk = 0; blk < 8; ++blk)
+        for (int kb = 0; kb < 16; ++kb)
+          for (int lane = 0; lane < 32; ++lane) {
+            const int i = 8 * blk + (lane >> 2), k = 4 * kb + (lane & 3), m = (i - k) & 127;
+            mat[6144 + (blk * 16 + kb) * 32 + lane] = 0.5 * (d1[m] + d1[(m + 64) & 127]);
+            mat[10240 + (blk * 16 + kb) * 32 + lane] = 0.5 * (d1[m] - d1[(m + 64) & 127]);
+          }
+    }
     cudaMemcpy(c->oc_mat, mat.data(), mat.size() * 8, cudaMemcpyHostToDevice);
     c->oc_dm = 2;
   }

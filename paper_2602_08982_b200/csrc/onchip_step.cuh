@@ -203,8 +203,8 @@ __device__ __forceinline__ void oc_lap64_store(cplx* T, int rb, int cb, const do
 // ---- lines of 128 points (quasi-1D, configs[1]): d^2 as the folded matrices Ce, Co (64 x 64) of Eq. 28b.  The batch is a
 // matrix [lines][128]: the lines are the rows of the A operand, the matrices are the B operand.  Warp = (block of 8 lines, half
 // of the folded columns), results in fragments until every warp has read its lines, then in place.
-// Element i of line l is stored at oc_ix(l, i, 2).  Contains its two barriers.
-__device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines) {
+// Element i of line l is stored at oc_ix(l, i, 2).  The results stay in registers (res) until oc_lap128_store.
+__device__ __forceinline__ void oc_lap128(const cplx* F, const double* mat, int lines, cplx (&res)[2][2][4]) {
   // two folds: e = w[k] + w[k+64], o = w[k] - w[k+64] (k < 64); the even part is again a symmetric circulant (period 64):
   // ee = e[k] + e[k+32], eo = e[k] - e[k+32] (k < 32).  O = Co o (64 x 64), EE = Cee ee, EO = Ceo eo (32 x 32);
   // E[i] = EE[i] + EO[i], E[i+32] = EE[i] - EO[i] (i < 32); out[i] = E[i] + O[i], out[i+64] = E[i] - O[i] (i < 64):
@@ -241,22 +241,79 @@ __device__ __forceinline__ void oc_lap128(cplx* F, const double* mat, int lines)
       }
     }
   }
-  __syncthreads();
-  if (active && lv) {
-    cplx* W = F + line * 128;
+  // results of this thread: points i, i + 32, i + 64, i + 96 for (q, j), i = 8 (b0 + q) + 2 t + j
 #pragma unroll
-    for (int q = 0; q < 2; ++q)
+  for (int q = 0; q < 2; ++q)
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const int i = (8 * (b0 + q) + 2 * t + j) ^ sw;            // i < 32
-        const cplx EE = make_double2(aE[q][0][0][j], aE[q][0][1][j]), EO = make_double2(aE[q][1][0][j], aE[q][1][1][j]);
-        const cplx Elo = cadd(EE, EO), Ehi = csub(EE, EO);       // E[i], E[i + 32]
-        const cplx Olo = make_double2(aO[q][0][j], aO[q][1][j]), Ohi = make_double2(aO[q + 2][0][j], aO[q + 2][1][j]);   // O[i], O[i + 32]
-        W[i] = cadd(Elo, Olo); W[i + 64] = csub(Elo, Olo);
-        W[i + 32] = cadd(Ehi, Ohi); W[i + 96] = csub(Ehi, Ohi);
+    for (int j = 0; j < 2; ++j) {
+      const cplx EE = make_double2(aE[q][0][0][j], aE[q][0][1][j]), EO = make_double2(aE[q][1][0][j], aE[q][1][1][j]);
+      const cplx Elo = cadd(EE, EO), Ehi = csub(EE, EO);       // E[i], E[i + 32]
+      const cplx Olo = make_double2(aO[q][0][j], aO[q][1][j]), Ohi = make_double2(aO[q + 2][0][j], aO[q + 2][1][j]);   // O[i], O[i + 32]
+      res[q][j][0] = cadd(Elo, Olo); res[q][j][2] = csub(Elo, Olo);
+      res[q][j][1] = cadd(Ehi, Ohi); res[q][j][3] = csub(Ehi, Ohi);
+    }
+}
+
+// The current / velocity coupling on lines of 128 points (one held axis): res += rot [ W (D w) + D (W w) ], D the first
+// derivative as a circulant folded once (De, Do 64 x 64, fragment order at mat1), W_sigma [128] in global memory;
+// rot = +i on the lines of u (even), -i on the lines of v (odd).  One column-block pair (q) at a time: 16 accumulators.
+__device__ __forceinline__ void oc_cur128(const cplx* F, const double* mat1, const double* curW, int lines, cplx (&res)[2][2][4]) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
+  if (8 * lb >= lines) return;                                  // (whole warp)
+  const bool lv = line < lines;
+  const cplx* T = F + (lv ? line : 0) * 128;
+  const int sw = (line & 1) << 2, b0 = 2 * ch;
+  const double* W = curW + (line & 1) * 3 * 128;                // W_a | W_b along the held axis (M = 128)
+  const double sgn = (line & 1) ? -1.0 : 1.0;
+  const cplx zero = make_double2(0.0, 0.0);
+#pragma unroll 1
+  for (int q = 0; q < 2; ++q) {
+    double aG[2][2][2][2] = {}, aH[2][2][2][2] = {};            // [columns i | i + 32][re | im][E | O][j]
+#pragma unroll 2
+    for (int kb = 0; kb < 16; ++kb) {
+      const int k = 4 * kb + t, k1 = k ^ sw;
+      const cplx w1 = lv ? T[k1] : zero, w2 = lv ? T[k1 + 64] : zero;
+      const cplx h1 = cscale(w1, __ldg(W + k)), h2 = cscale(w2, __ldg(W + k + 64));
+      const cplx ew = cadd(w1, w2), ow = csub(w1, w2), eh = cadd(h1, h2), oh = csub(h1, h2);
+#pragma unroll
+      for (int hi = 0; hi < 2; ++hi) {
+        const int cbb = b0 + q + 4 * hi;
+        const double me = __ldg(mat1 + (cbb * 16 + kb) * 32 + lane), mo = __ldg(mat1 + 4096 + (cbb * 16 + kb) * 32 + lane);
+        oc_dmma(aG[hi][0][0][0], aG[hi][0][0][1], ew.x, me); oc_dmma(aG[hi][0][1][0], aG[hi][0][1][1], ow.x, mo);
+        oc_dmma(aG[hi][1][0][0], aG[hi][1][0][1], ew.y, me); oc_dmma(aG[hi][1][1][0], aG[hi][1][1][1], ow.y, mo);
+        oc_dmma(aH[hi][0][0][0], aH[hi][0][0][1], eh.x, me); oc_dmma(aH[hi][0][1][0], aH[hi][0][1][1], oh.x, mo);
+        oc_dmma(aH[hi][1][0][0], aH[hi][1][0][1], eh.y, me); oc_dmma(aH[hi][1][1][0], aH[hi][1][1][1], oh.y, mo);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int p = 0; p < 4; ++p) {                             // point i + 32 p: columns block hi = p & 1, E + O (p < 2) or E - O
+        const int hi = p & 1, i = 8 * (b0 + q) + 2 * t + j + 32 * p;
+        const double sg = p < 2 ? 1.0 : -1.0, wv = __ldg(W + i);
+        const double tr = wv * (aG[hi][0][0][j] + sg * aG[hi][0][1][j]) + (aH[hi][0][0][j] + sg * aH[hi][0][1][j]);
+        const double ti = wv * (aG[hi][1][0][j] + sg * aG[hi][1][1][j]) + (aH[hi][1][0][j] + sg * aH[hi][1][1][j]);
+        res[q][j][p].x -= sgn * ti; res[q][j][p].y += sgn * tr;
       }
   }
-  __syncthreads();
+}
+
+// overwrite the lines in place (after every warp has read them: the caller's barrier)
+__device__ __forceinline__ void oc_lap128_store(cplx* F, int lines, const cplx (&res)[2][2][4]) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
+  if (8 * lb >= lines || line >= lines) return;
+  cplx* W = F + line * 128;
+  const int sw = (line & 1) << 2, b0 = 2 * ch;
+#pragma unroll
+  for (int q = 0; q < 2; ++q)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const int i = (8 * (b0 + q) + 2 * t + j) ^ sw;
+#pragma unroll
+      for (int p = 0; p < 4; ++p) W[i + 32 * p] = res[q][j][p];
+    }
 }
 
 template <int MODE, int MAXPT, int DM = 0, bool CUR = false>
@@ -306,7 +363,16 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     }
     __syncthreads();
     if (DM == 2) {                                              // lines of 128 points, 256 threads: d^2 in matrix form on DMMA
-      oc_lap128(F, a.mat, 2 * cnt);
+      {
+        cplx res[2][2][4];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) (&res[0][0][0])[i] = make_double2(0.0, 0.0);
+        oc_lap128(F, a.mat, 2 * cnt, res);
+        if (CUR) oc_cur128(F, a.mat + 6144, a.curW, 2 * cnt, res);
+        __syncthreads();
+        oc_lap128_store(F, 2 * cnt, res);
+        __syncthreads();
+      }
       // the spinor values are read again (L2) instead of being held in registers across the matrix products
 #pragma unroll
       for (int w = 0; w < OC_SLOTS; ++w) {
@@ -608,7 +674,7 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   a.out = out; a.cpart = cpart; a.kappa = kappa; a.dV = c->dV;
   a.use_shift = c->f.subtract_mean_energy; a.normalize = c->f.normalize; a.eps_out = eps_user;
   a.do_dens = do_dens; a.cpref = c->cpref + n0; a.w_a = c->w_a + n0; a.w_b = c->w_b + n0; a.dpart = c->oc_dpart;
-  a.n = n; a.S = P.ocS; a.dm = c->oc_dm; a.mat = c->oc_mat; a.curW = (c->f.current_terms && c->oc_dm == 1) ? c->cur_W : nullptr;
+  a.n = n; a.S = P.ocS; a.dm = c->oc_dm; a.mat = c->oc_mat; a.curW = (c->f.current_terms && c->oc_dm) ? c->cur_W : nullptr;
   const size_t smem = (size_t)P.ocS * 2 * P.M * 16 + (size_t)P.ocS * P.M * 8;
   if (!g_oc_attr_done) {
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -617,6 +683,9 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 2, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 2, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_APPLY, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_CORR, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(k_onchip_stage<OC_RHS, 2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -635,7 +704,8 @@ static void oc_launch(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, 
   const double lgM = (double)(P.lg[0] + P.lg[1] + P.lg[2]);
   WORK(c, 32.0 * P.M * n * (mode == OC_CORR ? 3.0 : 2.0), 5.0 * P.M * lgM * 2.0 * 2.0 * n);
   void (*k)(OCArgs);
-  if (small && c->oc_dm == 2) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2, 2> : k_onchip_stage<OC_RHS, 2, 2>;
+  if (small && c->oc_dm == 2 && a.curW) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2, 2, true> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2, 2, true> : k_onchip_stage<OC_RHS, 2, 2, true>;
+  else if (small && c->oc_dm == 2) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2, 2> : k_onchip_stage<OC_RHS, 2, 2>;
   else if (small) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 2> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 2> : k_onchip_stage<OC_RHS, 2>;
   else if (c->oc_dm == 1 && a.curW) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, 1, true> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, 1, true> : k_onchip_stage<OC_RHS, 8, 1, true>;
   else if (c->oc_dm == 1) k = mode == OC_APPLY ? k_onchip_stage<OC_APPLY, 8, 1> : mode == OC_CORR ? k_onchip_stage<OC_CORR, 8, 1> : k_onchip_stage<OC_RHS, 8, 1>;

@@ -812,13 +812,15 @@ def test_current_coupling_apply_h_matches_oracle(shape, dx, kin_form):
     assert relerr(make_oracle(w0).apply_h(psi)[0], ref) > 1e-3
 
 
+@pytest.mark.parametrize("shape,dx,nwf", [((64, 64), (1.0, 0.9), 5), ((128,), (0.9,), 19)])
 @pytest.mark.parametrize("func_id,force_a1", [(0, 0), (2, 1), (1, 0)])
-def test_current_coupling_on_the_fused_onchip_path_64x64(func_id, force_a1):
-    """NEXT-1 on a fused path: on 64 x 64 lattices the on-chip stage kernels take the coupling -(i/2){W, grad} inside their
-    matrix-form core (first-derivative matrices on DMMA; W = -v_ext whenever the step rebuilds rho and nu only: fixed fields,
-    SLDA with alpha = 1, BdG): H psi with eps_n and ABM steps against the oracle, and the on-chip kernels really ran."""
+def test_current_coupling_on_the_fused_onchip_paths(shape, dx, nwf, func_id, force_a1):
+    """NEXT-1 on fused paths: on 64 x 64 lattices and on lines of 128 points the on-chip stage kernels take the coupling
+    -(i/2){W, grad} inside their matrix-form core (first-derivative matrices on DMMA; W = -v_ext whenever the step rebuilds rho
+    and nu only: fixed fields, SLDA with alpha = 1, BdG): H psi with eps_n and ABM steps against the oracle (ragged batches on
+    the lines), and the on-chip kernels really ran."""
     kw = dict(four_pi_as=-3.0) if func_id == 1 else {}
-    w = _with_currents(generic((64, 64), (1.0, 0.9), 5, 0, func_id=func_id, force_a1=force_a1, n_modes=2, dt=0.004, **kw), 461, amp=0.3)
+    w = _with_currents(generic(shape, dx, nwf, 0, func_id=func_id, force_a1=force_a1, n_modes=2, dt=0.004, **kw), 461, amp=0.3)
     psi0 = spinors(w)
     o, g = make_oracle(w), make_gpu(w)
     if func_id:
@@ -828,7 +830,7 @@ def test_current_coupling_on_the_fused_onchip_path_64x64(func_id, force_a1):
     assert "k_onchip_apply" in names
     h, e = g.apply_h(to_gpu(psi0))
     assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
-    w0 = generic((64, 64), (1.0, 0.9), 5, 0, func_id=func_id, force_a1=force_a1, n_modes=2, dt=0.004, **kw)
+    w0 = generic(shape, dx, nwf, 0, func_id=func_id, force_a1=force_a1, n_modes=2, dt=0.004, **kw)
     o0 = make_oracle(w0)
     if func_id:
         o0.densities(psi0); o0.update_potentials()
