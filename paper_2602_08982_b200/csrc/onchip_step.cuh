@@ -222,8 +222,7 @@ __device__ __forceinline__ void oc_lap128(const cplx* F, const double* mat, int 
 #pragma unroll 2
     for (int kb = 0; kb < 8; ++kb) {
       const int k1 = (4 * kb + t) ^ sw;
-      const cplx zero = make_double2(0.0, 0.0);
-      const cplx w0 = lv ? T[k1] : zero, w1 = lv ? T[k1 + 32] : zero, w2 = lv ? T[k1 + 64] : zero, w3 = lv ? T[k1 + 96] : zero;
+      const cplx w0 = T[k1], w1 = T[k1 + 32], w2 = T[k1 + 64], w3 = T[k1 + 96];   // (a line beyond the batch reads line 0: its results are dropped)
       const cplx e0 = cadd(w0, w2), e1 = cadd(w1, w3), o0 = csub(w0, w2), o1 = csub(w1, w3);   // e[k], e[k+32], o[k], o[k+32]
       const cplx ee = cadd(e0, e1), eo = csub(e0, e1);
 #pragma unroll
@@ -266,14 +265,13 @@ __device__ __forceinline__ void oc_cur128(const cplx* F, const double* mat1, con
   const int sw = (line & 1) << 2, b0 = 2 * ch;
   const double* W = curW + (line & 1) * 3 * 128;                // W_a | W_b along the held axis (M = 128)
   const double sgn = (line & 1) ? -1.0 : 1.0;
-  const cplx zero = make_double2(0.0, 0.0);
 #pragma unroll 1
   for (int q = 0; q < 2; ++q) {
     double aG[2][2][2][2] = {}, aH[2][2][2][2] = {};            // [columns i | i + 32][re | im][E | O][j]
 #pragma unroll 2
     for (int kb = 0; kb < 16; ++kb) {
       const int k = 4 * kb + t, k1 = k ^ sw;
-      const cplx w1 = lv ? T[k1] : zero, w2 = lv ? T[k1 + 64] : zero;
+      const cplx w1 = T[k1], w2 = T[k1 + 64];
       const cplx h1 = cscale(w1, __ldg(W + k)), h2 = cscale(w2, __ldg(W + k + 64));
       const cplx ew = cadd(w1, w2), ow = csub(w1, w2), eh = cadd(h1, h2), oh = csub(h1, h2);
 #pragma unroll
@@ -314,6 +312,62 @@ __device__ __forceinline__ void oc_lap128_store(cplx* F, int lines, const cplx (
 #pragma unroll
       for (int p = 0; p < 4; ++p) W[i + 32 * p] = res[q][j][p];
     }
+}
+
+// the same products with the results written in place from the accumulators (contains its two barriers): the variant
+// without the coupling, which needs no result registers beside them
+__device__ __forceinline__ void oc_lap128_inplace(cplx* F, const double* mat, int lines) {
+  // two folds: e = w[k] + w[k+64], o = w[k] - w[k+64] (k < 64); the even part is again a symmetric circulant (period 64):
+  // ee = e[k] + e[k+32], eo = e[k] - e[k+32] (k < 32).  O = Co o (64 x 64), EE = Cee ee, EO = Ceo eo (32 x 32);
+  // E[i] = EE[i] + EO[i], E[i+32] = EE[i] - EO[i] (i < 32); out[i] = E[i] + O[i], out[i+64] = E[i] - O[i] (i < 64):
+  // 6144 instead of 8192 multiply-adds per real line.  mat (fragment order, ctx.cuh): Co [8 blocks][16 kb][32],
+  // then Cee, Ceo [4 blocks][8 kb][32] each.
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int lb = warp & 3, ch = warp >> 2, line = 8 * lb + g;
+  const bool active = 8 * lb < lines;                           // (whole warp)
+  const bool lv = line < lines;                                 // a ragged last batch: lines beyond it are neither read nor written
+  const cplx* T = F + (lv ? line : 0) * 128;
+  const int sw = (line & 1) << 2;
+  double aO[4][2][2] = {}, aE[2][2][2][2] = {};                 // O: [b, b+1, b+4, b+5][re | im][j]; E: [b, b+1][EE | EO][re | im][j]
+  const int b0 = 2 * ch;                                        // this warp's column blocks of the twice-folded part: b0, b0 + 1
+  if (active) {
+#pragma unroll 2
+    for (int kb = 0; kb < 8; ++kb) {
+      const int k1 = (4 * kb + t) ^ sw;
+      const cplx w0 = T[k1], w1 = T[k1 + 32], w2 = T[k1 + 64], w3 = T[k1 + 96];   // (a line beyond the batch reads line 0: its results are dropped)
+      const cplx e0 = cadd(w0, w2), e1 = cadd(w1, w3), o0 = csub(w0, w2), o1 = csub(w1, w3);   // e[k], e[k+32], o[k], o[k+32]
+      const cplx ee = cadd(e0, e1), eo = csub(e0, e1);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {                             // O part: column blocks b0, b0 + 1, b0 + 4, b0 + 5; k-blocks kb and kb + 8
+        const int cbb = b0 + (q & 1) + 4 * (q >> 1);
+        const double m0 = __ldg(mat + (cbb * 16 + kb) * 32 + lane), m1 = __ldg(mat + (cbb * 16 + kb + 8) * 32 + lane);
+        oc_dmma(aO[q][0][0], aO[q][0][1], o0.x, m0); oc_dmma(aO[q][1][0], aO[q][1][1], o0.y, m0);
+        oc_dmma(aO[q][0][0], aO[q][0][1], o1.x, m1); oc_dmma(aO[q][1][0], aO[q][1][1], o1.y, m1);
+      }
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {                             // EE, EO: column blocks b0, b0 + 1 of 4; k-block kb of 8
+        const double mee = __ldg(mat + 4096 + ((b0 + q) * 8 + kb) * 32 + lane), meo = __ldg(mat + 5120 + ((b0 + q) * 8 + kb) * 32 + lane);
+        oc_dmma(aE[q][0][0][0], aE[q][0][0][1], ee.x, mee); oc_dmma(aE[q][0][1][0], aE[q][0][1][1], ee.y, mee);
+        oc_dmma(aE[q][1][0][0], aE[q][1][0][1], eo.x, meo); oc_dmma(aE[q][1][1][0], aE[q][1][1][1], eo.y, meo);
+      }
+    }
+  }
+  __syncthreads();
+  if (active && lv) {
+    cplx* W = F + line * 128;
+#pragma unroll
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int i = (8 * (b0 + q) + 2 * t + j) ^ sw;            // i < 32
+        const cplx EE = make_double2(aE[q][0][0][j], aE[q][0][1][j]), EO = make_double2(aE[q][1][0][j], aE[q][1][1][j]);
+        const cplx Elo = cadd(EE, EO), Ehi = csub(EE, EO);       // E[i], E[i + 32]
+        const cplx Olo = make_double2(aO[q][0][j], aO[q][1][j]), Ohi = make_double2(aO[q + 2][0][j], aO[q + 2][1][j]);   // O[i], O[i + 32]
+        W[i] = cadd(Elo, Olo); W[i + 64] = csub(Elo, Olo);
+        W[i + 32] = cadd(Ehi, Ohi); W[i + 96] = csub(Ehi, Ohi);
+      }
+  }
+  __syncthreads();
 }
 
 template <int MODE, int MAXPT, int DM = 0, bool CUR = false>
@@ -363,15 +417,17 @@ __global__ void __launch_bounds__(MAXPT <= 2 ? 256 : 512, MAXPT <= 2 ? 2 : 1) k_
     }
     __syncthreads();
     if (DM == 2) {                                              // lines of 128 points, 256 threads: d^2 in matrix form on DMMA
-      {
+      if (CUR) {
         cplx res[2][2][4];
 #pragma unroll
         for (int i = 0; i < 16; ++i) (&res[0][0][0])[i] = make_double2(0.0, 0.0);
         oc_lap128(F, a.mat, 2 * cnt, res);
-        if (CUR) oc_cur128(F, a.mat + 6144, a.curW, 2 * cnt, res);
+        oc_cur128(F, a.mat + 6144, a.curW, 2 * cnt, res);
         __syncthreads();
         oc_lap128_store(F, 2 * cnt, res);
         __syncthreads();
+      } else {
+        oc_lap128_inplace(F, a.mat, 2 * cnt);
       }
       // the spinor values are read again (L2) instead of being held in registers across the matrix products
 #pragma unroll
