@@ -106,7 +106,10 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
   // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
-           f->kin_form != WSLDA_KIN_DIVGRAD && !f->current_terms && !f->quantum_friction;
+           f->kin_form != WSLDA_KIN_DIVGRAD && !f->quantum_friction &&
+           // the current / velocity coupling is fused only in the matrix-form 32^3 Eq. 40 stage kernels (mega3m.cuh)
+           (!f->current_terms || (P.N[0] == 32 && f->kin_form == WSLDA_KIN_SYM40 && g_tune.dmma_stage >= F3M_DEFAULT_ON &&
+                                  !g_tune.disable_persistent && !g_tune.disable_axis_split && !g_tune.enable_tma_stage));
   if (g_tune.disable_fused3d) P.fast = 0;
   P.fc = 32; P.ns = 3;
   if (g_tune.fused_chunk > 0) P.fc = g_tune.fused_chunk;
@@ -134,7 +137,7 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_part_bytes = align_up((size_t)F3_NPART * n_wf * (P.N[0] < 64 ? 64 : P.N[0]) * 8);   // mega3t: 64 partial sums per spinor
     P.mega_acc_bytes = align_up((size_t)F3_RING * 4 * M * 8);
     P.mega_sync_bytes = align_up(sizeof(F3Sync) + (size_t)5 * n_wf * sizeof(int));      // done[4][G <= n_wf] + one arrival counter per spinor
-    P.mega_pack_bytes = align_up((size_t)M * 48) + 16384;            // + the folded derivative matrices of mega3m.cuh
+    P.mega_pack_bytes = align_up((size_t)M * 48) + 32768;            // + the folded derivative matrices of mega3m.cuh (second and first derivative)
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
   P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms && !f->quantum_friction;
@@ -192,7 +195,7 @@ struct wslda_ctx {
   int mega_grid;
   int sep_pm, sep_em;              // mega3s.cuh: x-planes per P item, row pairs per XE item
   int sep3;                        // 32^3 Eq. 40: axis-by-axis Laplacian stage kernel (mega3s.cuh)
-  int dm3, dm3_grid; double* m_mat;   // 32^3 Eq. 40: matrix-form (DMMA) stage kernel (mega3m.cuh), its grid, the folded matrices
+  int dm3, dm3_grid, dm3_grid_cur; double* m_mat;   // 32^3 Eq. 40: matrix-form (DMMA) stage kernel (mega3m.cuh), its grid, the folded matrices
   int t3, t3_gs, t3_r, t3_ring, t3_lag, t3_grid;    // 32^3 Eq. 40: warp-specialised TMA-fed stage kernel (mega3t.cuh): spinors per group, per heavy super-item
   T3Maps t3_maps;                  // tensor maps of the arrays the library owns (QL ring, alpha); psi is encoded per launch
   int spin_limit;                  // bound of the device-side dependency waits (polls of 200 ns)
@@ -436,7 +439,7 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
     c->m_mat = (double*)((char*)c->m_pack + align_up((size_t)M * 48));
     c->dm3 = P.sep && f->kin_form == WSLDA_KIN_SYM40 && !c->t3 && g_tune.dmma_stage >= F3M_DEFAULT_ON;
     if (c->dm3) {
-      std::vector<double> mat(3 * 2 * 256);
+      std::vector<double> mat(2 * 3 * 2 * 256);                  // second derivative, then 2 x first derivative (CUR kernels)
       for (int ax = 0; ax < 3; ++ax) {
         const double* k2 = c->hk2[2 - ax];
         double cc[32];
@@ -448,9 +451,24 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
             mat[(ax * 2 + 1) * 256 + i * 16 + k] = 0.5 * (cc[m] - cc[(m + 16) & 31]);
           }
       }
+      for (int ax = 0; ax < 3; ++ax) {                          // 2 D_d (odd derivative: Nyquist mode dropped), folded once
+        const double len = 32 * c->dx[2 - ax];
+        double d1[32];
+        for (int m = 0; m < 32; ++m) {
+          double t = 0.0;
+          for (int q = 1; q < 32; ++q) { if (q == 16) continue; const double k = q < 16 ? 2.0 * PI * q / len : 2.0 * PI * (q - 32) / len; t -= k * sin(2.0 * PI * ((q * m) & 31) / 32.0); }
+          d1[m] = t / 32.0;
+        }
+        for (int i = 0; i < 16; ++i)
+          for (int k = 0; k < 16; ++k) {
+            const int m = (i - k) & 31;
+            mat[1536 + (ax * 2 + 0) * 256 + i * 16 + k] = d1[m] + d1[(m + 16) & 31];
+            mat[1536 + (ax * 2 + 1) * 256 + i * 16 + k] = d1[m] - d1[(m + 16) & 31];
+          }
+      }
       {   // fragment order: [axis][Ce | Co][block of 8 rows][k-block][lane = 4 g + t] = M[8 blk + g][4 kb + t] (256 contiguous bytes per warp load)
         std::vector<double> fr(mat.size());
-        for (int ae = 0; ae < 6; ++ae)
+        for (int ae = 0; ae < 12; ++ae)
           for (int blk = 0; blk < 2; ++blk)
             for (int kb = 0; kb < 4; ++kb)
               for (int lane = 0; lane < 32; ++lane)
@@ -463,8 +481,17 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
 #define WS_DM3_ATTR(K) do { ok = ok && cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, F3M_BUF_BYTES) == cudaSuccess; \
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ3, K, 128, F3M_BUF_BYTES); if (occ3 < got) got = occ3; } while (0)
       WS_DM3_ATTR(k_f3m_mega<F3_APPLY>); WS_DM3_ATTR(k_f3m_mega<F3_CORR>); WS_DM3_ATTR(k_f3m_mega<F3_RHS>);
+      int got_cur = 2;
+      if (f->current_terms) {
+        const int keep = got; got = 2;
+        WS_DM3_ATTR((k_f3m_mega<F3_APPLY, true>)); WS_DM3_ATTR((k_f3m_mega<F3_CORR, true>)); WS_DM3_ATTR((k_f3m_mega<F3_RHS, true>));
+        got_cur = got; got = keep;
+        if (got_cur < 1) ok = false;
+      }
+      c->dm3_grid_cur = got_cur * sms;
 #undef WS_DM3_ATTR
       if (!ok || got < 1) { cudaGetLastError(); c->dm3 = 0; }
+      if (!c->dm3 && f->current_terms) { snprintf(g_err, 256, "wslda_ctx_create: the fused 32^3 kernels with the current coupling could not be set up"); free(c); return WSLDA_ECUDA; }
       c->dm3_grid = got * sms;
       if (g_tune.persistent_ctas > 0) c->dm3_grid = g_tune.persistent_ctas;
     }

@@ -97,11 +97,14 @@ static void f3_mega(wslda_ctx* c, cudaStream_t st, int mode, const cplx* psi, co
   }
   if (c->dm3 && sym) {                       // 32^3 Eq. 40: matrix-form line derivatives on DMMA (mega3m.cuh)
     F3MMega A;
-    A.m = a; A.pm = c->sep_pm; A.em = c->sep_em; A.mat = c->m_mat;
+    A.m = a; A.pm = c->sep_pm; A.em = c->sep_em; A.mat = c->m_mat; A.mat1 = c->m_mat + 1536; A.curW = c->f.current_terms ? c->cur_W : nullptr;
     const int ITs = a.gs * 32 / A.pm + a.gs * 32 / A.em + (mode == F3_APPLY ? 0 : 32 * F3_DSPLIT);
     const long tot = (long)(a.G + 2) * ITs;
-    const int gr = (int)(tot < c->dm3_grid ? tot : c->dm3_grid);
+    const int cap = c->f.current_terms ? c->dm3_grid_cur : c->dm3_grid;
+    const int gr = (int)(tot < cap ? tot : cap);
     void (*km)(F3MMega) = mode == F3_APPLY ? k_f3m_mega<F3_APPLY> : mode == F3_CORR ? k_f3m_mega<F3_CORR> : k_f3m_mega<F3_RHS>;
+    if (c->f.current_terms)                                // the coupling of Eq. 4c inside the matrix-form kernels (own instantiation, 2 CTAs per SM)
+      km = mode == F3_APPLY ? k_f3m_mega<F3_APPLY, true> : mode == F3_CORR ? k_f3m_mega<F3_CORR, true> : k_f3m_mega<F3_RHS, true>;
     LAUNCHN(c, mode == F3_APPLY ? "k_f3m_mega_apply" : mode == F3_CORR ? "k_f3m_mega_corr" : "k_f3m_mega_rhs", km, gr, 128, F3M_BUF_BYTES, st, A);
     cudaMemcpyAsync(c->err_host, &c->m_sync->error, sizeof(int), cudaMemcpyDeviceToHost, st);
     return;

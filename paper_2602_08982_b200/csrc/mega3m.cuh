@@ -88,7 +88,11 @@ __device__ __forceinline__ void f3m_load(const F3Mega& a, int n, int idx, unsign
 }
 
 // one warp task of a P item; T, AL: this component's tiles; q: this component's plane of the Q ring
-__device__ __forceinline__ void f3m_task_p(const cplx* T, const double* AL, const double* mat, int rb, int cb, double s, cplx* q, uint64_t pol) {
+// CUR: the in-plane part of the current / velocity coupling (Eq. 4c, R27) rides on the alpha-w field's results: with the first-
+// derivative matrices stored as 2 D (mat1), -1/4 [.. + (+-i)(W_d (2 D_d w) + 2 D_d (W_d w))] = .. + (+-)(-(i/2)){W_d, d_d} w; sgn = +1 for u, -1 for v
+template <bool CUR = false>
+__device__ __forceinline__ void f3m_task_p(const cplx* T, const double* AL, const double* mat, int rb, int cb, double s, cplx* q, uint64_t pol,
+                                           const double* mat1 = nullptr, const double* Wy = nullptr, const double* Wz = nullptr, double sgn = 1.0) {
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   double mA[2][4], mB[2][4];                            // fragments of Ce, Co: rows of the y matrices (A operand), of the z matrices (B operand)
 #pragma unroll
@@ -120,6 +124,25 @@ __device__ __forceinline__ void f3m_task_p(const cplx* T, const double* AL, cons
           out[f][p][0][zi][j] = acc[f][p][0][j] + acc[f][p][1][j];
           out[f][p][1][zi][j] = acc[f][p][0][j] - acc[f][p][1][j];
         }
+    if (CUR) {                                              // W_y (2 D_y w) + 2 D_y (W_y w)
+#pragma unroll
+      for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = 0.0;
+#pragma unroll
+      for (int kb = 0; kb < 4; ++kb) {
+        const int y1 = 4 * kb + t, y2 = y1 + 16;
+        f3m_kblock<true>(acc, T[f3m_sw(y1, z)], T[f3m_sw(y2, z)], __ldg(Wy + y1 * F3_N + z), __ldg(Wy + y2 * F3_N + z),
+                         __ldg(mat1 + (1 * 2 + 0) * 256 + (rb * 4 + kb) * 32 + lane), __ldg(mat1 + (1 * 2 + 1) * 256 + (rb * 4 + kb) * 32 + lane));
+      }
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const double sg = h ? -1.0 : 1.0, wv = __ldg(Wy + (8 * rb + 16 * h + g) * F3_N + 8 * cb + 16 * zi + 2 * t + j);
+          const double tr = wv * (acc[0][0][0][j] + sg * acc[0][0][1][j]) + (acc[1][0][0][j] + sg * acc[1][0][1][j]);
+          const double ti = wv * (acc[0][1][0][j] + sg * acc[0][1][1][j]) + (acc[1][1][0][j] + sg * acc[1][1][1][j]);
+          out[1][0][h][zi][j] -= sgn * ti; out[1][1][h][zi][j] += sgn * tr;
+        }
+    }
   }
   // d_z^2: A = folded data W[m = y][k = z], B = Ce / Co columns
 #pragma unroll
@@ -142,6 +165,25 @@ __device__ __forceinline__ void f3m_task_p(const cplx* T, const double* AL, cons
           out[f][p][h][0][j] += acc[f][p][0][j] + acc[f][p][1][j];
           out[f][p][h][1][j] += acc[f][p][0][j] - acc[f][p][1][j];
         }
+    if (CUR) {                                              // W_z (2 D_z w) + 2 D_z (W_z w)
+#pragma unroll
+      for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = 0.0;
+#pragma unroll
+      for (int kb = 0; kb < 4; ++kb) {
+        const int z1 = 4 * kb + t, z2 = z1 + 16;
+        f3m_kblock<false>(acc, T[f3m_sw(y, z1)], T[f3m_sw(y, z2)], __ldg(Wz + y * F3_N + z1), __ldg(Wz + y * F3_N + z2),
+                          __ldg(mat1 + (0 * 2 + 0) * 256 + (cb * 4 + kb) * 32 + lane), __ldg(mat1 + (0 * 2 + 1) * 256 + (cb * 4 + kb) * 32 + lane));
+      }
+#pragma unroll
+      for (int zi = 0; zi < 2; ++zi)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const double sg = zi ? -1.0 : 1.0, wv = __ldg(Wz + y * F3_N + 8 * cb + 16 * zi + 2 * t + j);
+          const double tr = wv * (acc[0][0][0][j] + sg * acc[0][0][1][j]) + (acc[1][0][0][j] + sg * acc[1][0][1][j]);
+          const double ti = wv * (acc[0][1][0][j] + sg * acc[0][1][1][j]) + (acc[1][1][0][j] + sg * acc[1][1][1][j]);
+          out[1][0][h][zi][j] -= sgn * ti; out[1][1][h][zi][j] += sgn * tr;
+        }
+    }
   }
   // Q_c = s [ alpha (d_y^2 + d_z^2) w + (d_y^2 + d_z^2)(alpha w) ] at (y = 8 rb + 16 h + g, z = 8 cb + 16 zi + 2 t + j)
 #pragma unroll
@@ -159,9 +201,12 @@ struct F3MMega {
   F3Mega m;                      // spec0 = Q ring [R][gs][2][M]
   int pm, em;                    // x-planes per P item, y-rows per XE item
   const double* mat;             // [axis z, y, x][Ce | Co][16][16]
+  const double* mat1;            // CUR: the first-derivative matrices (2 D, folded), same layout
+  const double* curW;            // CUR: W_sigma,d = A_sigma,d - v_ext,sigma,d, [2][3][M]
 };
 
 // ---- P item: pm x-planes of one spinor -----------------------------------------------------------------------------
+template <bool CUR = false>
 __device__ __forceinline__ void f3m_body_p(const F3MMega& A, const F3Pol& pol, int g, int ip, unsigned char* buf) {
   const F3Mega& a = A.m;
   const int warp = threadIdx.x >> 5;
@@ -180,14 +225,19 @@ __device__ __forceinline__ void f3m_body_p(const F3MMega& A, const F3Pol& pol, i
     __syncthreads();
     cplx* q = a.spec0 + (((size_t)(g % F3_RING) * a.gs + nl) * 2 + c) * M + (size_t)ix * F3_PLANE;
 #pragma unroll 1
-    for (int cb = 0; cb < 2; ++cb) f3m_task_p(T, AL, A.mat, rb, cb, s, q, pol.keep);
+    for (int cb = 0; cb < 2; ++cb) {
+      if (CUR) {
+        const double* W = A.curW + (size_t)(c * 3) * M + (size_t)ix * F3_PLANE;       // W_c,x | + M: W_c,y | + 2 M: W_c,z of this plane
+        f3m_task_p<true>(T, AL, A.mat, rb, cb, s, q, pol.keep, A.mat1, W + M, W + 2 * M, c ? -1.0 : 1.0);
+      } else f3m_task_p(T, AL, A.mat, rb, cb, s, q, pol.keep);
+    }
     __syncthreads();
   }
 }
 
 // ---- XE item: em y-rows of one spinor.  A warp task is (rows {8 rb ..} u {16 + 8 rb ..} of x, 8 columns of z) for BOTH
 // components: d_x^2 of w and alpha w by DMMA, then the pointwise epilogue on the accumulator fragments ------------------
-template <int MODE>
+template <int MODE, bool CUR = false>
 __device__ __forceinline__ void f3m_body_xe(const F3MMega& A, const F3Pol& pol, int g, int ie, unsigned char* buf, double* red) {
   const F3Mega& a = A.m;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gq = lane >> 2, t = lane & 3;
@@ -269,6 +319,27 @@ __device__ __forceinline__ void f3m_body_xe(const F3MMega& A, const F3Pol& pol, 
             L[c][h][j] = make_double2(s * (aj * wr + vr), s * (aj * wi + vi));
           }
         }
+        if (CUR) {                                              // the x part of the coupling: W_x (2 D_x w) + 2 D_x (W_x w), rotated by +-i
+          const double* Wx = A.curW + (size_t)(c * 3) * M + (size_t)y * F3_N;          // + x * F3_PLANE + z
+#pragma unroll
+          for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = 0.0;
+#pragma unroll
+          for (int kb = 0; kb < 4; ++kb) {
+            const int x1 = 4 * kb + t, x2 = x1 + 16;
+            f3m_kblock<true>(acc, T[f3m_sw(x1, z)], T[f3m_sw(x2, z)], __ldg(Wx + (size_t)x1 * F3_PLANE + z), __ldg(Wx + (size_t)x2 * F3_PLANE + z),
+                             __ldg(A.mat1 + (2 * 2 + 0) * 256 + (rb * 4 + kb) * 32 + lane), __ldg(A.mat1 + (2 * 2 + 1) * 256 + (rb * 4 + kb) * 32 + lane));
+          }
+          const double sgn = c ? -1.0 : 1.0;
+#pragma unroll
+          for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              const double sg = h ? -1.0 : 1.0, wv = __ldg(Wx + (size_t)(8 * rb + 16 * h + gq) * F3_PLANE + 8 * cb + 2 * t + j);
+              const double tr = wv * (acc[0][0][0][j] + sg * acc[0][0][1][j]) + (acc[1][0][0][j] + sg * acc[1][0][1][j]);
+              const double ti = wv * (acc[0][1][0][j] + sg * acc[0][1][1][j]) + (acc[1][1][0][j] + sg * acc[1][1][1][j]);
+              L[c][h][j].x -= s * sgn * ti; L[c][h][j].y += s * sgn * tr;
+            }
+        }
       }
       // pointwise epilogue at (x = 8 rb + 16 h + gq, z = 8 cb + 2 t + j): Eqs. 5, 15, 40; the stage combination
 #pragma unroll
@@ -320,8 +391,8 @@ __device__ __forceinline__ void f3m_body_xe(const F3MMega& A, const F3Pol& pol, 
 }
 
 // tick t: P(t), XE(t-1), D(t-2): the dispatch of k_f3s_mega (mega3s.cuh) with the matrix-form bodies
-template <int MODE>
-__global__ void __launch_bounds__(128, F3M_OCC) k_f3m_mega(F3MMega A) {
+template <int MODE, bool CUR = false>
+__global__ void __launch_bounds__(128, CUR ? 2 : F3M_OCC) k_f3m_mega(F3MMega A) {
   extern __shared__ __align__(128) unsigned char f3m_buf[];
   __shared__ int s_item[2];
   __shared__ double s_eps[32], s_sn[32], red[4 * F3_NPART];
@@ -345,7 +416,7 @@ __global__ void __launch_bounds__(128, F3M_OCC) k_f3m_mega(F3MMega A) {
       const int g = tick;
       if (g < G) {
         if (g >= F3_RING) f3_wait(&done[G + g - F3_RING], nE, a.sync);                 // the Q slot is free
-        f3m_body_p(A, pol, g, r, f3m_buf);
+        f3m_body_p<CUR>(A, pol, g, r, f3m_buf);
         f3_signal(&done[g], &a.sync->next, t1); drew = true;
       }
     } else if (r < nP + nE) {
@@ -353,7 +424,7 @@ __global__ void __launch_bounds__(128, F3M_OCC) k_f3m_mega(F3MMega A) {
       if (g >= 0 && g < G) {
         f3_wait(&done[g], nP, a.sync);
         if (MODE != F3_APPLY && g >= F3_RING) f3_wait(&done[2 * G + g - F3_RING], nD, a.sync);   // the X slot is free
-        f3m_body_xe<MODE>(A, pol, g, r - nP, f3m_buf, red);
+        f3m_body_xe<MODE, CUR>(A, pol, g, r - nP, f3m_buf, red);
         f3_signal(&done[G + g], &a.sync->next, t1); drew = true;
       }
     } else {

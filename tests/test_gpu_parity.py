@@ -845,6 +845,39 @@ def test_current_coupling_on_the_fused_onchip_paths(shape, dx, nwf, func_id, for
     assert "k_onchip_corr" in names and "k_onchip_rhs" in names
 
 
+@pytest.mark.parametrize("func_id,force_a1,nwf", [(0, 0, 9), (2, 1, 37), (1, 0, 5)])
+def test_current_coupling_on_the_fused_32cubed_path(tuning, func_id, force_a1, nwf):
+    """NEXT-1 on the persistent 32^3 Eq. 40 kernels: the matrix-form stage kernels (mega3m.cuh, own instantiation) take the
+    coupling -(i/2){W, grad}: its y and z parts ride on the alpha-w field of the P items, its x part on the XE items' x-derivative
+    (2 D_d matrices on DMMA).  Fixed random fields with alpha_a != alpha_b, SLDA with alpha = 1, BdG; three lattice spacings;
+    ragged groups; H psi with eps_n and ABM steps against the oracle; the fused kernels really ran."""
+    tuning(group=(5 if nwf > 30 else 0), fused_chunk=3, fused_streams=3)
+    kw = dict(four_pi_as=-3.0) if func_id == 1 else {}
+    mk = lambda: generic((32, 32, 32), (1.0, 0.85, 1.2), nwf, 1, func_id=func_id, force_a1=force_a1, dt=0.004, **kw)
+    w = _with_currents(mk(), 471, amp=0.3)
+    psi0 = spinors(w)
+    o, g = make_oracle(w), make_gpu(w)
+    if func_id:
+        o.densities(psi0); o.update_potentials(); g.densities(to_gpu(psi0)); g.update_potentials()
+    ref, eref = o.apply_h(psi0)
+    names = _kernels_of(g, lambda: g.apply_h(to_gpu(psi0)))
+    assert "k_f3m_mega_apply" in names
+    h, e = g.apply_h(to_gpu(psi0))
+    assert relerr(to_np(h), ref) < TOL_H and relerr(to_np(e), eref) < TOL_H
+    o0 = make_oracle(mk())
+    if func_id:
+        o0.densities(psi0); o0.update_potentials()
+    assert relerr(o0.apply_h(psi0)[0], ref) > 1e-3                     # the term is not a rounding matter
+    pg, po, fg, fo, o, g = run_both(w, psi0, 3)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names
+
+
 @pytest.mark.parametrize("case", ["aslda_polarised", "aslda_symmetric", "bdg_moving_frame", "fixed"])
 def test_current_coupling_selfconsistent_steps(case):
     """Self-consistent steps with the coupling: A_sigma = (1 - alpha_sigma) j_sigma / rho_sigma rebuilt at both stages of
