@@ -166,6 +166,9 @@ def run_reference(args):
     if rank != 0:
         return
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "force_a1", False):
+        w.force_a1 = 1
+        desc += " (alpha = 1: force_a1)"
     if getattr(args, "velocity", 0.0):
         Mv, ndv = int(np.prod(w.shape)), len(w.shape)
         vv = args.velocity * wl.normal(977, 0, 6 * Mv).reshape(2, 3, *w.shape)
@@ -237,6 +240,9 @@ def run_gpu(args):
                                 device_id=torch.device("cuda", local))
     ws.build()
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "force_a1", False):
+        w.force_a1 = 1
+        desc += " (alpha = 1: force_a1)"
     if getattr(args, "velocity", 0.0):
         Mv, ndv = int(np.prod(w.shape)), len(w.shape)
         vv = args.velocity * wl.normal(977, 0, 6 * Mv).reshape(2, 3, *w.shape)
@@ -536,6 +542,7 @@ def main():
                     help="cfg4 only: time another discretisation of the kinetic term (0 Eq. 14, 2 DIVGRAD) instead of Eq. 40")
     ap.add_argument("--velocity", type=float, default=0.0,
                     help="add seeded external velocity fields of this amplitude (NEXT-1 current / velocity coupling, Eq. 4c) to the workload")
+    ap.add_argument("--force-a1", action="store_true", help="SLDA with alpha = 1 (the functional's force_a1 switch) on the chosen workload")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
