@@ -61,8 +61,10 @@ typedef struct {
                                  with A_sigma = dE/dj_sigma = (1 - alpha_sigma) j_sigma / rho_sigma
                                  and the j-terms of Eqs. 9b-c in V_sigma.  The
                                 anticommutator is applied as W.grad + grad.(W .), both derivatives spectral with the
-                                Nyquist rule: exactly Hermitian.  Served by the general path (no fused kernels);
-                                wslda_abm_step then also rebuilds j at both stages.  0: h of Eq. 4c without it  */
+                                Nyquist rule: exactly Hermitian.  Fused into the matrix-form stage kernels (32^3 with the
+                                Eq. 40 operator, 64 x 64, lines of 128 points) whenever the step rebuilds rho and nu
+                                only (A_sigma = 0: fixed fields, alpha = 1, BdG); otherwise the general path serves it
+                                and wslda_abm_step also rebuilds j at both stages.  0: h of Eq. 4c without it       */
   int quantum_friction;      /* 1: the dissipative potentials of Eqs. 66-70 are added at every
                                 potential update: V_sigma += -(qf_alpha / qf_rho0) div j_sigma, Delta += Delta [qf_beta
                                 sin(arg nu - arg B') + i qf_gamma (N - qf_nreq) / qf_nreq].  General path; the step then
