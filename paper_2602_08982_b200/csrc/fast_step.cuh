@@ -270,8 +270,15 @@ static void f3_dens_final(wslda_ctx* c, int used, cudaStream_t st) {
   LAUNCH(c, k_f3_dens_final, nb(4 * M, 256), 256, 0, st, c->f_acc[0], used, (int64_t)(c->P.fast_stream_bytes / 8), M, c->raw);
 }
 
+// The fused step serves functionals that consume rho and nu only, and -- on cubic 32^3 lattices with the persistent
+// kernels -- tau and j as well (polarised ASLDA; A_sigma = (1 - alpha_sigma) j_sigma / rho_sigma): the gradient densities are
+// then taken axis by axis (gdens.cuh) after each stage.
 static bool f3_step_ok(const wslda_ctx* c) {
-  return c->P.fast && (c->f.func_id == WSLDA_FUNC_FIXED || step_mask(c) == (WSLDA_D_RHO | WSLDA_D_NU));
+  if (!c->P.fast) return false;
+  if (c->f.func_id == WSLDA_FUNC_FIXED) return true;
+  const unsigned m = step_mask(c);
+  if (m == (WSLDA_D_RHO | WSLDA_D_NU)) return true;
+  return !(m & ~(WSLDA_D_RHO | WSLDA_D_NU | WSLDA_D_TAU | WSLDA_D_J)) && c->P.mega && gdens_ok(c);
 }
 
 static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
@@ -297,12 +304,18 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
       }
     }
     f3_join(c, s);
-    if (!fixed) { f3_dens_final(c, used, s.user); potentials(c, s.user); }
+    const unsigned gm = fixed ? 0u : step_mask(c) & (WSLDA_D_TAU | WSLDA_D_J);      // gradient densities the functional consumes
+    if (!fixed) {
+      f3_dens_final(c, used, s.user);
+      if (gm) gdens(c, s.phi, 0, n_wf, gm, 0, s.user, c->f.normalize ? c->scale : nullptr);     // of the (unnormalised) predictor
+      potentials(c, s.user);
+    }
     f3_mega(c, s.user, F3_CORR, s.phi, c->f.normalize ? c->scale : nullptr, 0, n_wf, s.phi, s.cpart, s.c0dt, !fixed);
     if (!fixed) {
       const int64_t mG = f3_uses_t3(c) ? (n_wf + c->t3_gs - 1) / c->t3_gs : c->P.mG;
       const int slots = (int)(mG < F3_RING ? mG : F3_RING);
       LAUNCH(c, k_f3_dens_final, nb(4 * P.M, 256), 256, 0, s.user, c->m_acc, slots, (int64_t)(4 * P.M), P.M, c->raw);
+      if (gm) gdens(c, s.phi, 0, n_wf, gm, 0, s.user);                  // of phi_new (normalised)
       potentials(c, s.user);
     }
     f3_mega(c, s.user, F3_RHS, s.phi, nullptr, 0, n_wf, s.cpart, nullptr, 0.0, 0);

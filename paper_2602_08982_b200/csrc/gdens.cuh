@@ -15,6 +15,7 @@
 struct GdArgs {
   const cplx* psi;              // first spinor of the range, [n][2][M]
   const double *cpref, *w_a, *w_b;   // per spinor of the range
+  const double* scale;          // per spinor, nullable: the densities of scale_n psi_n (the unnormalised predictor)
   double kd[3][64];             // wave numbers of Eq. 25, natural order, Nyquist entry zeroed (odd derivative)
   double* part;                 // [G][3][2][2][M]
   int n, G;                     // spinors in the range, groups
@@ -69,7 +70,7 @@ __global__ void __launch_bounds__(128, 2) k_gdens(const __grid_constant__ GdArgs
   cplx x[32];
 #pragma unroll 1
   for (int n = n0; n < n1; ++n) {
-    const double cw = a.cpref[n] * wt[n];
+    const double sc = a.scale ? a.scale[n] : 1.0, cw = a.cpref[n] * wt[n] * (sc * sc);
     if (cw == 0.0) continue;                                      // uniform over the CTA (e.g. w_a = 0 with Eq. 8 weights)
     const cplx* src = a.psi + (size_t)(2 * n + sg) * M + base;
 #pragma unroll

@@ -282,12 +282,14 @@ static bool gdens_ok(const wslda_ctx* c) {
   const Plan& P = c->P;
   return P.nd == 3 && P.N[0] == P.N[1] && P.N[1] == P.N[2] && (P.N[0] == 32 || P.N[0] == 64) && !g_tune.disable_axis_split;
 }
-static void gdens(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_count, unsigned mask, int accumulate, cudaStream_t st) {
+static void gdens(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_count, unsigned mask, int accumulate, cudaStream_t st,
+                  const double* scale = nullptr) {
   const Plan& P = c->P;
   const int N = P.N[0];
   const int64_t M = P.M;
   GdArgs a;
   a.psi = psi + 2 * n_first * M; a.cpref = c->cpref + n_first; a.w_a = c->w_a + n_first; a.w_b = c->w_b + n_first;
+  a.scale = scale ? scale + n_first : nullptr;
   const double PI = 3.14159265358979323846264338327950288;
   for (int d = 0; d < 3; ++d) {
     const double len = N * c->dx[d];

@@ -878,6 +878,35 @@ def test_current_coupling_on_the_fused_32cubed_path(tuning, func_id, force_a1, n
     assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names
 
 
+@pytest.mark.parametrize("case", ["polarised", "polarised_currents", "symmetric_currents"])
+def test_fused_32cubed_step_with_gradient_densities(tuning, case):
+    """Functionals that consume tau and j inside the step on the fused 32^3 path: polarised ASLDA (alpha_sigma depends on p, so tau
+    enters V_sigma) and ASLDA with the current coupling (A_sigma = (1 - alpha_sigma) j_sigma / rho_sigma rebuilt at both stages):
+    the persistent stage kernels do the stages, the axis-by-axis gradient densities (gdens.cuh) follow each of them.  Steps and
+    fields against the oracle; the fused kernels and k_gdens really ran."""
+    tuning(group=5, fused_chunk=3, fused_streams=3)
+    w = wl.cfg4(n_side=32, n_wf=14, kin_form=1, n_steps=3)
+    if case.startswith("polarised"):
+        w.spin_symmetric = 0
+        w.w_a = 0.6 * np.asarray(w.w_b)                         # both spin densities populated, p != 0: alpha_a != alpha_b != 1
+    if case.endswith("currents"):
+        w = _with_currents(w, 481, amp=0.05)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, 3, selfstart=0)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    names_f = ["rho_a", "nu", "delta", "U_a", "U_b", "alpha_a"] + (["tau_a", "tau_b"] if case.startswith("polarised") else [])
+    names_f += ["ja_x", "jb_z", "Aa_x", "Ab_y", "V_a"] if case.endswith("currents") else []
+    for f in names_f:
+        ref = o.get_field(f)
+        assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names and "k_gdens" in names
+
+
 @pytest.mark.parametrize("case", ["aslda_polarised", "aslda_symmetric", "bdg_moving_frame", "fixed"])
 def test_current_coupling_selfconsistent_steps(case):
     """Self-consistent steps with the coupling: A_sigma = (1 - alpha_sigma) j_sigma / rho_sigma rebuilt at both stages of
