@@ -166,6 +166,10 @@ def run_reference(args):
     if rank != 0:
         return
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "polarised", False):
+        w.spin_symmetric = 0
+        w.w_a = 0.6 * np.asarray(w.w_b)
+        desc += " (polarised: w_a = 0.6 w_b, tau rebuilt every stage)"
     if getattr(args, "force_a1", False):
         w.force_a1 = 1
         desc += " (alpha = 1: force_a1)"
@@ -240,6 +244,10 @@ def run_gpu(args):
                                 device_id=torch.device("cuda", local))
     ws.build()
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "polarised", False):
+        w.spin_symmetric = 0
+        w.w_a = 0.6 * np.asarray(w.w_b)
+        desc += " (polarised: w_a = 0.6 w_b, tau rebuilt every stage)"
     if getattr(args, "force_a1", False):
         w.force_a1 = 1
         desc += " (alpha = 1: force_a1)"
@@ -543,6 +551,8 @@ def main():
     ap.add_argument("--velocity", type=float, default=0.0,
                     help="add seeded external velocity fields of this amplitude (NEXT-1 current / velocity coupling, Eq. 4c) to the workload")
     ap.add_argument("--force-a1", action="store_true", help="SLDA with alpha = 1 (the functional's force_a1 switch) on the chosen workload")
+    ap.add_argument("--polarised", action="store_true",
+                    help="both spin densities populated (w_a = 0.6 w_b, no spin folding): alpha_sigma depends on p and tau enters V_sigma")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")
