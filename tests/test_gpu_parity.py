@@ -878,6 +878,25 @@ def test_current_coupling_on_the_fused_32cubed_path(tuning, func_id, force_a1, n
     assert "k_f3m_mega_corr" in names and "k_f3m_mega_rhs" in names
 
 
+def test_fused_64cubed_step_polarised_aslda():
+    """Polarised ASLDA on 64^3: the persistent 64^3 stage kernels do the stages, tau comes from the axis-by-axis gradient
+    densities after each of them.  Two steps and the fields against the oracle; the fused kernels and k_gdens really ran."""
+    w = wl.cfg4(n_side=64, n_wf=4, kin_form=1, n_steps=2)
+    w.spin_symmetric = 0
+    w.w_a = 0.6 * np.asarray(w.w_b)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, 2, selfstart=0)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("rho_a", "rho_b", "nu", "delta", "U_a", "U_b", "alpha_a", "alpha_b", "tau_a", "tau_b"):
+        assert relerr(to_np(g.get_field(f)), o.get_field(f)) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f6_mega_corr" in names and "k_f6_mega_rhs" in names and "k_gdens" in names
+
+
 @pytest.mark.parametrize("case", ["polarised", "polarised_currents", "symmetric_currents"])
 def test_fused_32cubed_step_with_gradient_densities(tuning, case):
     """Functionals that consume tau and j inside the step on the fused 32^3 path: polarised ASLDA (alpha_sigma depends on p, so tau
