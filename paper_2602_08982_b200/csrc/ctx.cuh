@@ -605,8 +605,12 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->cpref, n_wf, 1.0 / c->Lperp);
   k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->scale, n_wf, 1.0);
   c->launches += 5;
-  cudaFuncSetAttribute(k_gdens<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
-  cudaFuncSetAttribute(k_gdens<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<32, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<32, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens<64, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
   const int big = 227 * 1024;
   cudaFuncSetAttribute(k_deriv_onchip, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
   cudaFuncSetAttribute(k_planes_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, big);

@@ -48,7 +48,9 @@ template <> struct GdLine<64> {
   }
 };
 
-template <int N>
+// WHAT: bit 0 = tau, bit 1 = j (a step that consumes only one of them skips the other's accumulators and, for tau alone, the
+// second read of the line)
+template <int N, int WHAT = 3>
 __global__ void __launch_bounds__(128, 2) k_gdens(const __grid_constant__ GdArgs a) {
   extern __shared__ double gd_acc[];                              // [2][32][128]: tau, j_d of this thread's 32 points
   const GdLine<N> L;
@@ -63,7 +65,7 @@ __global__ void __launch_bounds__(128, 2) k_gdens(const __grid_constant__ GdArgs
   double* aT = gd_acc + threadIdx.x;
   double* aJ = aT + 32 * 128;
 #pragma unroll
-  for (int j = 0; j < 32; ++j) { aT[j * 128] = 0.0; aJ[j * 128] = 0.0; }
+  for (int j = 0; j < 32; ++j) { if (WHAT & 1) aT[j * 128] = 0.0; if (WHAT & 2) aJ[j * 128] = 0.0; }
   const int per = (a.n + a.G - 1) / a.G, n0 = g * per, n1 = min(a.n, n0 + per);
   const double* wt = sg ? a.w_b : a.w_a;
   const double sgn = sg ? 1.0 : -1.0;                             // Eq. 7f: j_a = -sum Im[u grad u^*]; Eq. 7g: j_b = +sum Im[v grad v^*]
@@ -78,15 +80,20 @@ __global__ void __launch_bounds__(128, 2) k_gdens(const __grid_constant__ GdArgs
     L.deriv(x, a.kd[d]);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
-      const cplx w = src[(size_t)L.idx(j) * stride];              // again (L1 / L2): the line registers held the transform
-      aT[j * 128] += cw * (x[j].x * x[j].x + x[j].y * x[j].y);
-      aJ[j * 128] += sgn * cw * (w.y * x[j].x + w.x * x[j].y);    // Im[w conj(d w)] with x = conj(d w)
+      if (WHAT & 1) aT[j * 128] += cw * (x[j].x * x[j].x + x[j].y * x[j].y);
+      if (WHAT & 2) {
+        const cplx w = src[(size_t)L.idx(j) * stride];            // again (L1 / L2): the line registers held the transform
+        aJ[j * 128] += sgn * cw * (w.y * x[j].x + w.x * x[j].y);  // Im[w conj(d w)] with x = conj(d w)
+      }
     }
   }
   double* pT = a.part + ((((size_t)g * 3 + d) * 2 + sg) * 2) * M + base;
   double* pJ = pT + M;
 #pragma unroll
-  for (int j = 0; j < 32; ++j) { pT[(size_t)L.idx(j) * stride] = aT[j * 128]; pJ[(size_t)L.idx(j) * stride] = aJ[j * 128]; }
+  for (int j = 0; j < 32; ++j) {
+    if (WHAT & 1) pT[(size_t)L.idx(j) * stride] = aT[j * 128];
+    if (WHAT & 2) pJ[(size_t)L.idx(j) * stride] = aJ[j * 128];
+  }
 }
 
 // raw tau_sigma = sum_g sum_d part, raw j_sigma,d = sum_g part (index order); mask selects TAU / J planes

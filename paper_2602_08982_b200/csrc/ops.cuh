@@ -303,8 +303,11 @@ static void gdens(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_coun
   const int tiles = N * N / (N == 32 ? 128 : 64);
   const double lines = 3.0 * 2.0 * (double)N * N * (double)n_count;
   WORK(c, 32.0 * M * n_count, lines * 2.0 * 5.0 * N * P.lg[0]);
-  if (N == 32) LAUNCHN(c, "k_gdens", k_gdens<32>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
-  else LAUNCHN(c, "k_gdens", k_gdens<64>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
+  // (k_gdens_reduce only reads the planes of `mask`: a variant that skips the other kind leaves its partial planes stale)
+  const int what = ((mask & WSLDA_D_TAU) ? 1 : 0) | ((mask & WSLDA_D_J) ? 2 : 0);
+  void (*k)(GdArgs) = N == 32 ? (what == 1 ? k_gdens<32, 1> : what == 2 ? k_gdens<32, 2> : k_gdens<32, 3>)
+                              : (what == 1 ? k_gdens<64, 1> : what == 2 ? k_gdens<64, 2> : k_gdens<64, 3>);
+  LAUNCHN(c, "k_gdens", k, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
   LAUNCH(c, k_gdens_reduce, nb(M, 256), 256, 0, st, c->dpart, G, M, c->raw, mask, accumulate);
 }
 
