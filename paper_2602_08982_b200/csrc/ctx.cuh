@@ -106,7 +106,9 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
   P.off_scr = o; o += (size_t)P.nscr * P.scr_bytes;
   // fused 3-D path: Ny = Nz = 32, Nx in {8, 16, 32}, Eq. 14 or Eq. 40 operator
   P.fast = mode == 3 && P.N[1] == 32 && P.N[2] == 32 && (P.N[0] == 8 || P.N[0] == 16 || P.N[0] == 32) &&
-           f->kin_form != WSLDA_KIN_DIVGRAD && !f->quantum_friction &&
+           f->kin_form != WSLDA_KIN_DIVGRAD &&
+           // quantum friction changes the potentials only; its densities (j, B') come from the axis-by-axis kernels on cubic 32^3
+           (!f->quantum_friction || (P.N[0] == 32 && !g_tune.disable_persistent && !g_tune.disable_axis_split)) &&
            // the current / velocity coupling is fused only in the matrix-form 32^3 Eq. 40 stage kernels (mega3m.cuh)
            (!f->current_terms || (P.N[0] == 32 && f->kin_form == WSLDA_KIN_SYM40 && g_tune.dmma_stage >= F3M_DEFAULT_ON &&
                                   !g_tune.disable_persistent && !g_tune.disable_axis_split && !g_tune.enable_tma_stage));
@@ -605,6 +607,8 @@ extern "C" wslda_status wslda_ctx_create(wslda_ctx** out, const int dims[3], con
   k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->cpref, n_wf, 1.0 / c->Lperp);
   k_fill<<<(unsigned)((n_wf + T - 1) / T), T>>>(c->scale, n_wf, 1.0);
   c->launches += 5;
+  cudaFuncSetAttribute(k_gdens_bp<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
+  cudaFuncSetAttribute(k_gdens_bp<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
   cudaFuncSetAttribute(k_gdens<32, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
   cudaFuncSetAttribute(k_gdens<32, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);
   cudaFuncSetAttribute(k_gdens<32, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 32 * 128 * 8);

@@ -278,7 +278,7 @@ static bool f3_step_ok(const wslda_ctx* c) {
   if (c->f.func_id == WSLDA_FUNC_FIXED) return true;
   const unsigned m = step_mask(c);
   if (m == (WSLDA_D_RHO | WSLDA_D_NU)) return true;
-  return !(m & ~(WSLDA_D_RHO | WSLDA_D_NU | WSLDA_D_TAU | WSLDA_D_J)) && c->P.mega && gdens_ok(c);
+  return !(m & ~(WSLDA_D_RHO | WSLDA_D_NU | WSLDA_D_TAU | WSLDA_D_J | WSLDA_D_BP)) && c->P.mega && gdens_ok(c);
 }
 
 static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
@@ -308,6 +308,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
     if (!fixed) {
       f3_dens_final(c, used, s.user);
       if (gm) gdens(c, s.phi, 0, n_wf, gm, 0, s.user, c->f.normalize ? c->scale : nullptr);     // of the (unnormalised) predictor
+      if (step_mask(c) & WSLDA_D_BP) gdens_bp(c, s.phi, 0, n_wf, 0, s.user, c->f.normalize ? c->scale : nullptr);
       potentials(c, s.user);
     }
     f3_mega(c, s.user, F3_CORR, s.phi, c->f.normalize ? c->scale : nullptr, 0, n_wf, s.phi, s.cpart, s.c0dt, !fixed);
@@ -316,6 +317,7 @@ static void f3_abm_step(wslda_ctx* c, const F3Step& s) {
       const int slots = (int)(mG < F3_RING ? mG : F3_RING);
       LAUNCH(c, k_f3_dens_final, nb(4 * P.M, 256), 256, 0, s.user, c->m_acc, slots, (int64_t)(4 * P.M), P.M, c->raw);
       if (gm) gdens(c, s.phi, 0, n_wf, gm, 0, s.user);                  // of phi_new (normalised)
+      if (step_mask(c) & WSLDA_D_BP) gdens_bp(c, s.phi, 0, n_wf, 0, s.user);
       potentials(c, s.user);
     }
     f3_mega(c, s.user, F3_RHS, s.phi, nullptr, 0, n_wf, s.cpart, nullptr, 0.0, 0);

@@ -34,6 +34,13 @@ template <> struct GdLine<32> {
     for (int j = 0; j < 32; ++j) { const double f = k[j] * (1.0 / 32.0); x[j] = make_double2(-f * x[j].y, -f * x[j].x); }   // conj(i k X / N)
     fft_reg<32, false>(x);
   }
+  // x <- conj(d^2 w / d line^2); k2: squared wave numbers, natural order, Nyquist mode kept (even derivative)
+  __device__ __forceinline__ void deriv2(cplx* x, const double* k2) const {
+    fft_reg<32, false>(x);
+#pragma unroll
+    for (int j = 0; j < 32; ++j) { const double f = -k2[j] * (1.0 / 32.0); x[j] = make_double2(f * x[j].x, -f * x[j].y); }       // conj(-k^2 X / N)
+    fft_reg<32, false>(x);
+  }
 };
 template <> struct GdLine<64> {
   static constexpr int LINES = 64;
@@ -45,6 +52,12 @@ template <> struct GdLine<64> {
 #pragma unroll
     for (int j = 0; j < 32; ++j) { const double f = k[j + 32 * p] * (1.0 / 64.0); x[j] = make_double2(-f * x[j].y, -f * x[j].x); }
     f6_dif(x, p);                                                 // interleaved again: conj of the derivative at 2 j + p
+  }
+  __device__ __forceinline__ void deriv2(cplx* x, const double* k2) const {
+    f6_dit(x, p);
+#pragma unroll
+    for (int j = 0; j < 32; ++j) { const double f = -k2[j + 32 * p] * (1.0 / 64.0); x[j] = make_double2(f * x[j].x, -f * x[j].y); }
+    f6_dif(x, p);
   }
 };
 
@@ -114,4 +127,67 @@ __global__ void k_gdens_reduce(const double* part, int G, int64_t M, double* raw
 #pragma unroll
       for (int d = 0; d < 3; ++d) { double* r = raw + (int64_t)((sg ? DP_JB0 : DP_JA0) + d) * M + i; *r = (accumulate ? *r : 0.0) + j[d]; }
   }
+}
+
+// ---- the kinetic anomalous density B' = -1/2 sum_n wn [u lap v^* + v^* lap u] (Eq. 68; weights of nu, R29) the same
+// way: lap = sum of the second derivatives along the axes, each a pass over the lines of one axis.  The thread holding a line of u
+// adds v^* d_d^2 u, the one holding a line of v adds u (d_d^2 v)^* (the other component is read at the line's points); partial
+// planes [G][3][2][re | im][M] as above, summed in index order by k_gdens_bp_reduce.  a.kd holds the SQUARED wave numbers here.
+template <int N>
+__global__ void __launch_bounds__(128, 2) k_gdens_bp(const __grid_constant__ GdArgs a) {
+  extern __shared__ double gd_acc[];
+  const GdLine<N> L;
+  const int d = blockIdx.y >> 1, sg = blockIdx.y & 1, g = blockIdx.z;
+  const int line = blockIdx.x * GdLine<N>::LINES + L.q;
+  const int c0 = line / N, c1 = line - c0 * N;
+  const size_t M = (size_t)N * N * N;
+  size_t base, stride;
+  if (d == 0) { base = (size_t)c0 * N + c1; stride = (size_t)N * N; }
+  else if (d == 1) { base = (size_t)c0 * N * N + c1; stride = N; }
+  else { base = ((size_t)c0 * N + c1) * N; stride = 1; }
+  double* aR = gd_acc + threadIdx.x;
+  double* aI = aR + 32 * 128;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) { aR[j * 128] = 0.0; aI[j * 128] = 0.0; }
+  const int per = (a.n + a.G - 1) / a.G, n0 = g * per, n1 = min(a.n, n0 + per);
+  cplx x[32];
+#pragma unroll 1
+  for (int n = n0; n < n1; ++n) {
+    const double sc = a.scale ? a.scale[n] : 1.0, wn = -0.25 * a.cpref[n] * (a.w_b[n] - a.w_a[n]) * (sc * sc);   // -1/2 x 1/2 c_n (w_b - w_a)
+    if (wn == 0.0) continue;
+    const cplx* src = a.psi + (size_t)(2 * n + sg) * M + base;
+    const cplx* oth = a.psi + (size_t)(2 * n + 1 - sg) * M + base;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) x[j] = src[(size_t)L.idx(j) * stride];
+    L.deriv2(x, a.kd[d]);                                         // x = conj(d_d^2 w)
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const cplx o = oth[(size_t)L.idx(j) * stride];
+      // sg = 0: v^* d^2 u = conj(v x);  sg = 1: u (d^2 v)^* = u x
+      const double re = o.x * x[j].x - o.y * x[j].y, im = o.x * x[j].y + o.y * x[j].x;
+      aR[j * 128] += wn * re;
+      aI[j * 128] += (sg ? wn : -wn) * im;
+    }
+  }
+  double* pR = a.part + ((((size_t)g * 3 + d) * 2 + sg) * 2) * M + base;
+  double* pI = pR + M;
+#pragma unroll
+  for (int j = 0; j < 32; ++j) { pR[(size_t)L.idx(j) * stride] = aR[j * 128]; pI[(size_t)L.idx(j) * stride] = aI[j * 128]; }
+}
+
+__global__ void k_gdens_bp_reduce(const double* part, int G, int64_t M, double* raw, int accumulate) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  double re = 0.0, im = 0.0;
+  for (int g = 0; g < G; ++g)
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+      for (int sg = 0; sg < 2; ++sg) {
+        const double* p = part + ((((int64_t)g * 3 + d) * 2 + sg) * 2) * M + i;
+        re += p[0]; im += p[M];
+      }
+  double* r = raw + (int64_t)DP_BP_RE * M + i;
+  r[0] = (accumulate ? r[0] : 0.0) + re;
+  r[M] = (accumulate ? r[M] : 0.0) + im;
 }

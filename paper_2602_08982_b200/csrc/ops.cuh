@@ -311,6 +311,29 @@ static void gdens(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_coun
   LAUNCH(c, k_gdens_reduce, nb(M, 256), 256, 0, st, c->dpart, G, M, c->raw, mask, accumulate);
 }
 
+// B' (Eq. 68) of the same range the same way: second derivatives axis by axis (gdens.cuh)
+static void gdens_bp(wslda_ctx* c, const cplx* psi, int64_t n_first, int64_t n_count, int accumulate, cudaStream_t st,
+                     const double* scale = nullptr) {
+  const Plan& P = c->P;
+  const int N = P.N[0];
+  const int64_t M = P.M;
+  GdArgs a;
+  a.psi = psi + 2 * n_first * M; a.cpref = c->cpref + n_first; a.w_a = c->w_a + n_first; a.w_b = c->w_b + n_first;
+  a.scale = scale ? scale + n_first : nullptr;
+  for (int d = 0; d < 3; ++d)
+    for (int j = 0; j < 64; ++j) a.kd[d][j] = j < N ? c->hk2[d][j] : 0.0;       // squared wave numbers, Nyquist mode kept
+  a.part = c->dpart; a.n = (int)n_count;
+  int G = P.dG;
+  if (G > n_count) G = (int)n_count;
+  if (G < 1) G = 1;
+  a.G = G;
+  const int tiles = N * N / (N == 32 ? 128 : 64);
+  WORK(c, 32.0 * M * n_count, 3.0 * 2.0 * (double)N * N * (double)n_count * 2.0 * 5.0 * N * P.lg[0]);
+  if (N == 32) LAUNCHN(c, "k_gdens_bp", k_gdens_bp<32>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
+  else LAUNCHN(c, "k_gdens_bp", k_gdens_bp<64>, dim3(tiles, 6, G), 128, 2 * 32 * 128 * 8, st, a);
+  LAUNCH(c, k_gdens_bp_reduce, nb(M, 256), 256, 0, st, c->dpart, G, M, c->raw, accumulate);
+}
+
 extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t n_first, int64_t n_count, unsigned mask,
                                         int accumulate, void* stream) {
   if (!c || !psi_) return fail(c, WSLDA_EINVAL, "densities: null argument");
@@ -325,6 +348,11 @@ extern "C" wslda_status wslda_densities(wslda_ctx* c, const void* psi_, int64_t 
   if (n_count > 0 && (mask & (WSLDA_D_TAU | WSLDA_D_J)) && gdens_ok(c)) {     // cubic 32^3 / 64^3: gradients axis by axis
     gdens(c, (const cplx*)psi_, n_first, n_count, mask & (WSLDA_D_TAU | WSLDA_D_J), accumulate, st);
     mask &= ~(WSLDA_D_TAU | WSLDA_D_J);
+    if (!mask) return cuda_check(c, "densities");
+  }
+  if (n_count > 0 && (mask & WSLDA_D_BP) && gdens_ok(c)) {                     // B' by second derivatives axis by axis
+    gdens_bp(c, (const cplx*)psi_, n_first, n_count, accumulate, st);
+    mask &= ~WSLDA_D_BP;
     if (!mask) return cuda_check(c, "densities");
   }
   // without gradient fields no scratch is involved: the whole range is one "chunk" (one k_density launch)

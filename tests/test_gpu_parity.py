@@ -1038,6 +1038,51 @@ def test_kinetic_anomalous_density_matches_oracle(shape, dx, sym):
     assert relerr(to_np(g.get_field("bp")), o.get_field("bp")) < TOL_D
 
 
+@pytest.mark.parametrize("side,nwf", [(32, 21), (64, 3)])
+def test_kinetic_anomalous_density_axis_by_axis(side, nwf):
+    """B' on cubic 32^3 / 64^3 lattices comes from second derivatives taken axis by axis (k_gdens_bp): against the oracle, with
+    both spins populated, overwritten and accumulated over batches; the kernel really ran."""
+    w = wl.cfg4(n_side=side, n_wf=nwf, kin_form=1)
+    w.spin_symmetric = 0
+    w.w_a = 0.3 * np.asarray(w.w_b) + 0.1
+    psi = w.spinors()
+    o, g = make_oracle(w), make_gpu(w)
+    o.densities(psi)
+    dev = to_gpu(psi)
+    names = _kernels_of(g, lambda: g.densities(dev, which=ws.D_BP | ws.D_NU))
+    assert "k_gdens_bp" in names
+    ref = o.get_field("bp")
+    assert np.abs(ref).max() > 0
+    assert relerr(to_np(g.get_field("bp")), ref) < TOL_D and relerr(to_np(g.get_field("nu")), o.get_field("nu")) < TOL_D
+    g.densities(dev, n_first=0, n_count=2, which=ws.D_BP)
+    g.densities(dev, n_first=2, n_count=nwf - 2, which=ws.D_BP, accumulate=1)
+    assert relerr(to_np(g.get_field("bp")), ref) < TOL_D
+
+
+@pytest.mark.parametrize("case", ["symmetric", "polarised"])
+def test_quantum_friction_on_the_fused_32cubed_path(tuning, case):
+    """NEXT-3 on a fused path: on cubic 32^3 lattices the persistent stage kernels do the stages and j, B' (and tau) come from the
+    axis-by-axis density kernels after each of them; the friction terms are applied by the potential update as everywhere."""
+    tuning(group=5, fused_chunk=3, fused_streams=3)
+    w = wl.cfg4(n_side=32, n_wf=13, kin_form=1, n_steps=3)
+    if case == "polarised":
+        w.spin_symmetric = 0; w.w_a = 0.6 * np.asarray(w.w_b)
+    w.friction = dict(qf_alpha=6.0, qf_beta=5.0, qf_gamma=0.1, qf_rho0=0.03, qf_nreq=1.7)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, 3, selfstart=0)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("rho_a", "nu", "bp", "ja_x", "jb_z", "delta", "V_a", "U_b"):
+        ref = o.get_field(f)
+        assert np.abs(ref).max() > 0
+        assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f3m_mega_corr" in names and "k_gdens" in names and "k_gdens_bp" in names and "k_qf" in names
+
+
 @pytest.mark.parametrize("case", ["bdg", "aslda_polarised", "slda_symmetric_32"])
 def test_quantum_friction_steps_match_oracle(case):
     """Dissipative self-consistent steps: V^(d) from div j, Delta^(d) from the phases of nu and B' and from N - N_req,
