@@ -166,6 +166,9 @@ def run_reference(args):
     if rank != 0:
         return
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "friction", False):
+        w.friction = dict(qf_alpha=6.0, qf_beta=5.0, qf_gamma=0.1, qf_rho0=0.03, qf_nreq=float(np.sum(np.asarray(w.w_a) + np.asarray(w.w_b))))
+        desc += " + quantum friction (Eqs. 66-70)"
     if getattr(args, "polarised", False):
         w.spin_symmetric = 0
         w.w_a = 0.6 * np.asarray(w.w_b)
@@ -244,6 +247,9 @@ def run_gpu(args):
                                 device_id=torch.device("cuda", local))
     ws.build()
     w, desc = make_workload(args.config, args.n_wf, args.kin_form)
+    if getattr(args, "friction", False):
+        w.friction = dict(qf_alpha=6.0, qf_beta=5.0, qf_gamma=0.1, qf_rho0=0.03, qf_nreq=float(np.sum(np.asarray(w.w_a) + np.asarray(w.w_b))))
+        desc += " + quantum friction (Eqs. 66-70)"
     if getattr(args, "polarised", False):
         w.spin_symmetric = 0
         w.w_a = 0.6 * np.asarray(w.w_b)
@@ -553,6 +559,8 @@ def main():
     ap.add_argument("--force-a1", action="store_true", help="SLDA with alpha = 1 (the functional's force_a1 switch) on the chosen workload")
     ap.add_argument("--polarised", action="store_true",
                     help="both spin densities populated (w_a = 0.6 w_b, no spin folding): alpha_sigma depends on p and tau enters V_sigma")
+    ap.add_argument("--friction", action="store_true",
+                    help="quantum friction (NEXT-3, Eqs. 66-70): j and B' rebuilt at both stages, dissipative terms in V and Delta")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the spinor index over the ranks (strong scaling, density all-reduce) instead of replicas")

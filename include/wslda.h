@@ -67,8 +67,9 @@ typedef struct {
                                 and wslda_abm_step also rebuilds j at both stages.  0: h of Eq. 4c without it       */
   int quantum_friction;      /* 1: the dissipative potentials of Eqs. 66-70 are added at every
                                 potential update: V_sigma += -(qf_alpha / qf_rho0) div j_sigma, Delta += Delta [qf_beta
-                                sin(arg nu - arg B') + i qf_gamma (N - qf_nreq) / qf_nreq].  General path; the step then
-                                rebuilds j and B' (WSLDA_D_BP) as well.  Not with FUNC_FIXED                      */
+                                sin(arg nu - arg B') + i qf_gamma (N - qf_nreq) / qf_nreq].  The step then rebuilds j and
+                                B' (WSLDA_D_BP) as well: on cubic 32^3 lattices by the axis-by-axis density kernels
+                                beside the fused stage kernels, elsewhere on the general path.  Not with FUNC_FIXED  */
   double qf_alpha, qf_beta, qf_gamma;   /* alpha_qf (Eq. 66; 5-10), beta_qf (Eq. 67; about 5), gamma_qf (Eq. 70; about 0.1) */
   double qf_rho0, qf_nreq;   /* reference density rho_0 of Eq. 66, requested particle number N_req of Eq. 70 (> 0)  */
 } wslda_functional;
