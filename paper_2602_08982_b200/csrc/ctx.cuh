@@ -142,7 +142,9 @@ static int make_plan(const int dims[3], int mode, int64_t n_wf, const wslda_func
     P.mega_pack_bytes = align_up((size_t)M * 48) + 32768;            // + the folded derivative matrices of mega3m.cuh (second and first derivative)
     o += 3 * P.mega_ring_bytes + P.mega_part_bytes + P.mega_acc_bytes + P.mega_sync_bytes + P.mega_pack_bytes;
   }
-  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms && !f->quantum_friction;
+  // (quantum friction changes the potentials only: its densities come from the axis-by-axis kernels beside the stage kernels)
+  P.f6 = mode == 3 && P.N[0] == 64 && P.N[1] == 64 && P.N[2] == 64 && f->kin_form == WSLDA_KIN_SYM40 && !f->current_terms &&
+         (!f->quantum_friction || !g_tune.disable_axis_split);
   if (g_tune.disable_mega64) P.f6 = 0;
   P.off_f6 = o; P.f6_ring_bytes = P.f6_part_bytes = P.f6_acc_bytes = P.f6_sync_bytes = P.f6_pack_bytes = P.f6_partn_bytes = 0;
   if (P.f6) {

@@ -189,9 +189,10 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
     if (!fixed) potentials(c, st);
     oc_launch(c, st, OC_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0, c->eps);
   } else if (c->P.f6 && (fixed || mask == (WSLDA_D_RHO | WSLDA_D_NU) ||
-                         (mask == (WSLDA_D_RHO | WSLDA_D_NU | WSLDA_D_TAU) && gdens_ok(c)))) {   // 64^3 persistent kernels (mega64.cuh)
-    // (polarised ASLDA: tau by the axis-by-axis gradient densities after each stage, as on the 32^3 path)
-    const unsigned gm = fixed ? 0u : mask & WSLDA_D_TAU, pm = mask & (WSLDA_D_RHO | WSLDA_D_NU);
+                         (!(mask & ~(WSLDA_D_RHO | WSLDA_D_NU | WSLDA_D_TAU | WSLDA_D_J | WSLDA_D_BP)) && gdens_ok(c)))) {   // 64^3 persistent kernels (mega64.cuh)
+    // (polarised ASLDA, quantum friction: tau, j, B' by the axis-by-axis density kernels after each stage, as on the 32^3 path)
+    const unsigned gm = fixed ? 0u : mask & (WSLDA_D_TAU | WSLDA_D_J), pm = mask & (WSLDA_D_RHO | WSLDA_D_NU);
+    const bool bp = !fixed && (mask & WSLDA_D_BP);
     const double* scg = c->f.normalize ? c->scale : nullptr;
     if (fixed) {                                         // no density barrier: one predictor launch over the whole batch
       WORK(c, 32.0 * M * n_wf * (1 + c->m + 2), 0);
@@ -206,6 +207,7 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
         dens_chunk(c, b.phi + 2 * n0 * M, scg ? scg + n0 : nullptr, n0, cnt, pm, n0 > 0, st);
       }
       if (gm) gdens(c, b.phi, 0, n_wf, gm, 0, st, scg);
+      if (bp) gdens_bp(c, b.phi, 0, n_wf, 0, st, scg);
       potentials(c, st);
     }
     f6_mega(c, st, F3_CORR, b.phi, scg, 0, n_wf, b.phi, b.cpart, b.c0dt, !fixed);
@@ -213,6 +215,7 @@ extern "C" wslda_status wslda_abm_step(wslda_ctx* c, void* phi_, void** f_hist, 
       const int slots = (int)(n_wf < F6_RING ? n_wf : F6_RING);
       LAUNCH(c, k_f3_dens_final, nb(4 * M, 256), 256, 0, st, c->s_acc, slots, (int64_t)(4 * M), M, c->raw);
       if (gm) gdens(c, b.phi, 0, n_wf, gm, 0, st);
+      if (bp) gdens_bp(c, b.phi, 0, n_wf, 0, st);
       potentials(c, st);
     }
     f6_mega(c, st, F3_RHS, b.phi, nullptr, 0, n_wf, b.cpart, nullptr, 0.0, 0);

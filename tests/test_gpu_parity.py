@@ -1083,6 +1083,25 @@ def test_quantum_friction_on_the_fused_32cubed_path(tuning, case):
     assert "k_f3m_mega_corr" in names and "k_gdens" in names and "k_gdens_bp" in names and "k_qf" in names
 
 
+def test_quantum_friction_on_the_fused_64cubed_path():
+    """The same on 64^3: the persistent 64^3 stage kernels + k_gdens (j) + k_gdens_bp (B') + k_qf."""
+    w = wl.cfg4(n_side=64, n_wf=3, kin_form=1, n_steps=2)
+    w.friction = dict(qf_alpha=6.0, qf_beta=5.0, qf_gamma=0.1, qf_rho0=0.03, qf_nreq=1.7)
+    psi0 = w.spinors()
+    pg, po, fg, fo, o, g = run_both(w, psi0, 2, selfstart=0)
+    assert relerr(pg, po) < TOL_ABM and relerr(fg, fo) < TOL_ABM
+    for f in ("rho_a", "nu", "bp", "ja_x", "delta", "V_a", "U_b"):
+        ref = o.get_field(f)
+        assert np.abs(ref).max() > 0
+        assert relerr(to_np(g.get_field(f)), ref) < 1e-8, f
+    import torch
+    phi = to_gpu(psi0)
+    hist = [torch.zeros_like(phi) for _ in range(g.m)]
+    hist = g.abm_init(phi, hist, w.dt, 0)
+    names = _kernels_of(g, lambda: g.abm_step(phi, hist, w.dt))
+    assert "k_f6_mega_corr" in names and "k_gdens" in names and "k_gdens_bp" in names and "k_qf" in names
+
+
 @pytest.mark.parametrize("case", ["bdg", "aslda_polarised", "slda_symmetric_32"])
 def test_quantum_friction_steps_match_oracle(case):
     """Dissipative self-consistent steps: V^(d) from div j, Delta^(d) from the phases of nu and B' and from N - N_req,
